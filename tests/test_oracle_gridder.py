@@ -1,0 +1,162 @@
+"""P6, P7, P10, P11, P12 — the gridding oracle O4 pinned by worked examples and exact identities."""
+import numpy as np
+import pytest
+
+from oracle import gridder, wkernel
+from paper_1905_03213_b200 import synth
+
+
+def test_p6_index_map_worked_examples(golden):
+    N, Q = 64, 8
+    cell = 0.08 / N                      # any cell: the examples are given in units of du
+    du = 1.0 / (N * cell)
+    for S, x, j0, o in golden("p6_index_map.txt"):
+        got = gridder.index_map(float(x) * du, N, cell, int(S), Q)
+        assert got == (int(j0), int(o)), (S, x, got)
+
+
+def test_p7_plane_map_worked_examples(golden):
+    for w, p, cl in golden("p7_plane_map.txt"):
+        assert gridder.plane_of(float(w), 200.0, 16) == (int(p), bool(int(cl))), w
+
+
+def test_index_map_window_contains_position():
+    """Invariant: the kernel sample used for cell j is t = j Q - X with |t| <= S Q/2, so the
+    (quantised) position lies inside the window, centred to within one cell."""
+    rng = np.random.default_rng(7)
+    N, Q, cell = 256, 8, 2.0 ** -11
+    du = 1.0 / (N * cell)
+    for S in (4, 7, 8, 9, 16):
+        for x in rng.uniform(-100, 100, 200):
+            j0, o = gridder.index_map(x * du, N, cell, S, Q)
+            assert 0 <= o < Q
+            X = int(np.floor((x + N / 2) * Q + 0.5))
+            t_first = j0 * Q - X
+            t_last = (j0 + S - 1) * Q - X
+            assert t_first >= -S * Q // 2 + 1 and t_last <= S * Q // 2
+            centre = j0 + (S - 1) / 2.0
+            assert abs(centre - (x + N / 2)) <= 1.0
+
+
+@pytest.fixture(scope="module")
+def cfg1_small():
+    wl = synth.config1(nvis=4096)
+    st = wkernel.build_stack(wl.Nw, wl.w_max, wl.support, wl.oversample, wl.grid_N, wl.cell)
+    return wl, st
+
+
+def test_p10_single_visibility_footprint(cfg1_small):
+    wl, st = cfg1_small
+    K = st.as_array()
+    for k in (0, 17, 1234):
+        uvw = wl.uvw[k:k + 1]; vis = wl.vis[k:k + 1]; wt = np.full((1, 1), 0.75, np.float32)
+        g, stats = gridder.grid(uvw, vis, wt, wl.freq, st)
+        j0u, ou = gridder.index_map(uvw[0, 0], wl.grid_N, wl.cell, 7, 8)
+        j0v, ov = gridder.index_map(uvw[0, 1], wl.grid_N, wl.cell, 7, 8)
+        p, _ = gridder.plane_of(uvw[0, 2], wl.w_max, wl.Nw)
+        val = 0.75 * complex(vis[0, 0])
+        exp = np.zeros_like(g)
+        # complex product written in real form in the oracle: compare bitwise against the same real form
+        kk = K[p, ov, ou]
+        exp[j0v:j0v + 7, j0u:j0u + 7] = (val.real * kk.real - val.imag * kk.imag) + 1j * (val.real * kk.imag + val.imag * kk.real)
+        assert np.array_equal(g, exp)
+        assert stats == dict(n_gridded=1, n_skipped_oob=0, n_skipped_zero_weight=0, n_clamped_w=0, n_updates=49)
+
+
+def test_p11_flux_conservation(cfg1_small):
+    wl, st = cfg1_small
+    g, stats = gridder.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st)
+    sig = st.as_array().sum(axis=(3, 4))
+    tot = 0j
+    for k in range(wl.uvw.shape[0]):
+        _, ou = gridder.index_map(wl.uvw[k, 0], wl.grid_N, wl.cell, 7, 8)
+        _, ov = gridder.index_map(wl.uvw[k, 1], wl.grid_N, wl.cell, 7, 8)
+        p, _ = gridder.plane_of(wl.uvw[k, 2], wl.w_max, wl.Nw)
+        tot += complex(wl.vis[k, 0]) * sig[p, ov, ou]
+    assert abs(g.sum() - tot) <= 1e-12 * abs(tot)
+    assert stats["n_gridded"] == 4096 and stats["n_updates"] == 4096 * 49
+
+
+def test_p12_linearity_and_chunking(cfg1_small):
+    wl, st = cfg1_small
+    rng = np.random.default_rng(3)
+    v2 = (rng.standard_normal(wl.vis.shape) + 1j * rng.standard_normal(wl.vis.shape)).astype(np.complex64)
+    a, b = 2.0, -0.5                                     # exactly representable scalings
+    g1, _ = gridder.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st)
+    g2, _ = gridder.grid(wl.uvw, v2, wl.weight, wl.freq, st)
+    g12, _ = gridder.grid(wl.uvw, (a * wl.vis.astype(np.complex128) + b * v2).astype(np.complex64),
+                          wl.weight, wl.freq, st)
+    # the c64 rounding of the combined input limits this to ~1e-7 relative, the identity itself is exact
+    assert np.max(np.abs(g12 - (a * g1 + b * g2))) <= 5e-7 * np.max(np.abs(g12))
+    gw, _ = gridder.grid(wl.uvw, wl.vis, (3.0 * wl.weight).astype(np.float32), wl.freq, st)
+    assert np.max(np.abs(gw - 3.0 * g1)) <= 1e-12 * np.max(np.abs(g1))
+    h = wl.uvw.shape[0] // 2
+    gc, _ = gridder.grid(wl.uvw[:h], wl.vis[:h], wl.weight[:h], wl.freq, st)
+    gc, _ = gridder.grid(wl.uvw[h:], wl.vis[h:], wl.weight[h:], wl.freq, st, grid=gc)
+    assert np.max(np.abs(gc - g1)) <= 1e-12 * np.max(np.abs(g1))
+
+
+def test_openmp_mode_equals_serial(cfg1_small):
+    wl, st = cfg1_small
+    g1, s1 = gridder.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st)
+    g4, s4 = gridder.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    assert s1 == s4
+    assert np.max(np.abs(g1 - g4)) <= 1e-12 * np.max(np.abs(g1))
+
+
+def test_edge_cases_skip_clamp_flags_channels():
+    N, cell, Q, S, Nw, w_max = 64, 0.08 / 64, 8, 8, 4, 50.0
+    st = wkernel.build_stack(Nw, w_max, S, Q, N, cell)
+    du = 1.0 / 0.08
+    uvw = np.array([[0.0, 0.0, 0.0],          # fine
+                    [40 * du, 0.0, 0.0],       # window off the right edge -> skipped
+                    [-29 * du, 0.0, 0.0],      # j0u = 29-29 = 0: on the edge, kept
+                    [-29.1 * du, 0.0, 0.0],    # just off the left edge -> skipped
+                    [0.0, 28.4 * du, 10.0],    # j0v = 29+28 = 57: 57+8 > 64 -> skipped
+                    [0.0, 27.4 * du, 10.0],    # j0v + S = 64 -> kept
+                    [du, du, 80.0],            # |w| > w_max -> clamped to plane 3
+                    [du, du, -80.0]])          # clamped to plane 0
+    vis = np.ones((8, 1), np.complex64)
+    wt = np.ones((8, 1), np.float32)
+    g, s = gridder.grid(uvw, vis, wt, np.array([synth.C0]), st)
+    assert s == dict(n_gridded=5, n_skipped_oob=3, n_skipped_zero_weight=0, n_clamped_w=2, n_updates=5 * 64)
+    wt[0, 0] = 0.0
+    g, s = gridder.grid(uvw, vis, wt, np.array([synth.C0]), st)
+    assert s["n_skipped_zero_weight"] == 1 and s["n_gridded"] == 4
+    # empty input
+    g, s = gridder.grid(np.zeros((0, 3)), np.zeros((0, 1), np.complex64), np.zeros((0, 1), np.float32),
+                        np.array([synth.C0]), st)
+    assert s["n_gridded"] == 0 and not g.any()
+    # two channels = the same rows gridded at two scaled positions (G1)
+    uvw_m = np.array([[3.0, -2.0, 1.0]])
+    freq = np.array([synth.C0 * 2.0, synth.C0 * 5.0])
+    g2, _ = gridder.grid(uvw_m, np.array([[1 + 2j, 3 - 1j]], np.complex64), np.ones((1, 2), np.float32), freq, st)
+    ga, _ = gridder.grid(uvw_m * 2.0, np.array([[1 + 2j]], np.complex64), np.ones((1, 1), np.float32),
+                         np.array([synth.C0]), st)
+    gb, _ = gridder.grid(uvw_m * 5.0, np.array([[3 - 1j]], np.complex64), np.ones((1, 1), np.float32),
+                         np.array([synth.C0]), st, grid=ga)
+    assert np.array_equal(g2, gb)
+
+
+def test_ragged_stack_gridding_matches_per_plane_uniform():
+    """A ragged stack grids each visibility with its own plane's S_p (K6 + G3 with S = S_p)."""
+    N, cell, Q, Nw, w_max = 128, 0.2 / 128, 4, 4, 400.0
+    sup = wkernel.ragged_support(Nw, w_max, N, cell, 8, 32)
+    assert len(set(sup.tolist())) > 1
+    st = wkernel.build_stack(Nw, w_max, sup, Q, N, cell)
+    rng = np.random.default_rng(5)
+    n = 64
+    uvw = np.stack([rng.uniform(-100, 100, n), rng.uniform(-100, 100, n), rng.uniform(-400, 400, n)], 1)
+    vis = (rng.standard_normal((n, 1)) + 1j * rng.standard_normal((n, 1))).astype(np.complex64)
+    wt = np.ones((n, 1), np.float32)
+    g, s = gridder.grid(uvw, vis, wt, np.array([synth.C0]), st)
+    exp = np.zeros_like(g); upd = 0
+    for k in range(n):
+        p, _ = gridder.plane_of(uvw[k, 2], w_max, Nw)
+        S = int(sup[p])
+        j0u, ou = gridder.index_map(uvw[k, 0], N, cell, S, Q)
+        j0v, ov = gridder.index_map(uvw[k, 1], N, cell, S, Q)
+        exp[j0v:j0v + S, j0u:j0u + S] += complex(vis[k, 0]) * st.plane(p)[ov, ou]
+        upd += S * S
+    assert s["n_updates"] == upd and s["n_gridded"] == n
+    assert np.max(np.abs(g - exp)) <= 1e-13 * np.max(np.abs(exp))
