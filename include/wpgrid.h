@@ -1,0 +1,142 @@
+/* wpgrid.h — C ABI of the B200-native w-projection convolutional gridder.
+ *
+ * Hot path of arxiv 1905.03213 (Lao, An et al. 2019).  Citations are lines of
+ * the paper text and the readings in DESIGN.md §2 (R1-R20), which
+ * define what the paper leaves unstated.
+ *
+ * Conventions
+ *   - d_* arguments are DEVICE pointers owned by the caller; h_* are HOST
+ *     pointers.  The library never frees or keeps them.  Inputs are not modified.
+ *   - All work is enqueued on the context's CUDA stream.  Calls return without
+ *     synchronising unless a host output (wpg_stats, a host grid) is requested.
+ *   - Return value: WPG_OK (0) or a negative error code; text of the last error
+ *     via wpg_last_error().  Nothing throws or aborts across this boundary.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails
+ *     with WPG_ECUDA.
+ *   - Complex numbers are interleaved (re, im): "c64" = 2 x float, "c128" = 2 x double.
+ *   - Grid layout: grid[jv][ju], row-major, v the slow axis, N x N complex;
+ *     cell (N/2, N/2) is u = v = 0.
+ *   - Kernel stack layout: K[p][ov][ou][iv][iu], innermost iu; plane p starts at
+ *     element plane_offset[p] and holds Q*Q*S_p*S_p complex coefficients.
+ *   - Limits: grid_N <= 8192, S_p <= 64, Nw <= 256, S_p * Q even.
+ */
+#ifndef WPGRID_H
+#define WPGRID_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wpg_ctx wpg_ctx;              /* opaque: device id, stream, cuFFT plan cache, host scratch */
+
+typedef enum { WPG_F32 = 0, WPG_F64 = 1 } wpg_prec;   /* grid + coefficients c64 / c128 */
+
+enum { WPG_OK = 0, WPG_EINVAL = -1, WPG_ENOMEM = -2, WPG_ECUDA = -3 };
+
+/* Description of a kernel stack (the "imaging parameters" of PAPER.md:108). */
+typedef struct {
+    int Nw;                        /* number of w-planes */
+    int oversample;                /* Q */
+    int grid_N;                    /* N */
+    double w_max;                  /* wavelengths; planes are bin-centred on [-w_max, w_max] (R6) */
+    double cell;                   /* radians per image pixel; FoV = N*cell, du = 1/FoV */
+    int support_max;               /* S for uniform stacks, max S_p for ragged ones */
+    const int *support;            /* HOST [Nw] per-plane S_p, or NULL = uniform support_max */
+    const int64_t *plane_offset;   /* HOST [Nw+1] element offsets, or NULL = uniform p*Q*Q*S*S */
+} wpg_kdesc;
+
+typedef struct {
+    int64_t n_gridded;             /* visibilities gridded */
+    int64_t n_skipped_oob;         /* window not fully inside the grid (R8) */
+    int64_t n_skipped_zero_weight; /* weight == 0 (flagged, R9) */
+    int64_t n_clamped_w;           /* gridded with |w| > w_max, clamped to the edge plane (R6, R19) */
+    int64_t n_updates;             /* sum of S_p^2 over gridded visibilities (the metric's unit) */
+} wpg_stats;
+
+/* ---- context ---------------------------------------------------------------------------- */
+/* device: CUDA ordinal.  cuda_stream: a cudaStream_t (NULL = legacy default stream). */
+int  wpg_create(wpg_ctx **out, int device, void *cuda_stream);
+void wpg_destroy(wpg_ctx *ctx);
+const char *wpg_last_error(const wpg_ctx *ctx);   /* ctx may be NULL: last error of a failed wpg_create */
+int  wpg_version(void);
+
+/* Tuning knobs (all have defaults): "order" 0 = auto, 1 = plane-major, 2 = tile-major sort key;
+ * "segment" = max records per gridder work item; "ctas_per_sm" for the persistent gridder.
+ * Unknown name -> WPG_EINVAL. */
+int  wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value);
+
+/* ---- a0: W-kernel stack (setup, untimed) — PAPER.md:30 "new convolution kernel function";
+ *      DESIGN.md R1-R3, R5-R7, steps K1-K6 -------------------------------------------------- */
+/* Taper psi(nu) (R2) at n host points; independent Legendre-series implementation. */
+int  wpg_taper(const double *h_nu, int64_t n, double *h_out);
+/* Per-plane support by rule K6 (R20) and the matching plane offsets.  Host outputs. */
+int  wpg_ragged_support(int Nw, double w_max, int grid_N, double cell, int oversample,
+                        int S_min, int S_max, int *h_support_out /*[Nw]*/,
+                        int64_t *h_plane_offset_out /*[Nw+1]*/);
+int64_t wpg_wkernel_elems(int Nw, int support, int oversample);          /* Nw*Q*Q*S*S */
+/* Build the stack described by *desc (uniform if desc->support == NULL) into d_kernels_out
+ * (caller-allocated, c64 for WPG_F32 — rounded from fp64 — or c128 for WPG_F64).
+ * All arithmetic is fp64 on the device. */
+int  wpg_wkernel_build(wpg_ctx *ctx, const wpg_kdesc *desc, wpg_prec prec, void *d_kernels_out);
+
+/* ---- a1 + a2: binning and gridding — PAPER.md:30, 62-84 ------------------------------------ */
+/* Bytes of device scratch wpg_grid needs for this problem size. */
+size_t wpg_grid_workspace_bytes(const wpg_ctx *ctx, int64_t nrow, int nchan, const wpg_kdesc *desc,
+                                wpg_prec prec);
+/* grid += gridding of all (row, chan) visibilities (O4 G1-G7).
+ *   d_vis    c64   [nrow][nchan]
+ *   d_uvw    f64   [nrow][3], metres (R10)
+ *   d_weight f32   [nrow][nchan], 0 = flagged
+ *   d_freq   f64   [nchan], Hz      (wavelength inputs: nchan = 1, freq = {299792458})
+ *   d_kernels      c64 | c128 stack matching desc and prec
+ *   d_grid   c64 | c128 [N][N], ACCUMULATED INTO (caller zeroes)
+ *   h_stats_or_null: if non-NULL the call synchronises the stream and fills the counters. */
+int  wpg_grid(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+              const double *d_freq, int64_t nrow, int nchan, const void *d_kernels,
+              const wpg_kdesc *desc, wpg_prec prec, void *d_grid,
+              void *d_workspace, size_t workspace_bytes, wpg_stats *h_stats_or_null);
+/* Same result by the naive design: one global atomic per update, no sorting (the measured
+ * "atomic roofline" the tiled gridder must beat; "write access ... in an atomic manner"). */
+int  wpg_grid_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                    const double *d_freq, int64_t nrow, int nchan, const void *d_kernels,
+                    const wpg_kdesc *desc, wpg_prec prec, void *d_grid, wpg_stats *h_stats_or_null);
+/* End-to-end variant with HOST buffers: copies the inputs to device scratch owned by the
+ * context (grown on demand), zero-fills a device grid, runs wpg_grid, copies the grid to
+ * h_grid_out (overwritten, [N][N] c64|c128) and synchronises.  d_kernels stays on the device. */
+int  wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uvw, const float *h_weight,
+                   const double *h_freq, int64_t nrow, int nchan, const void *d_kernels,
+                   const wpg_kdesc *desc, wpg_prec prec, void *h_grid_out, wpg_stats *h_stats_or_null);
+
+/* Binning alone (step a1), for tests and profiling: fills the workspace exactly as wpg_grid
+ * does and reports where things are.  Offsets are in bytes from d_workspace. */
+typedef struct {
+    int64_t n_records;       /* valid visibilities = sorted records */
+    int64_t n_keys;          /* number of sort keys */
+    int64_t n_items;         /* gridder work items */
+    int32_t tile;            /* tile edge in cells */
+    int32_t ntile;           /* tiles per axis */
+    int32_t order;           /* 1 plane-major, 2 tile-major */
+    int32_t record_bytes;    /* 16 (fp32) or 24 (fp64) */
+    int64_t off_records;     /* records sorted by key: {re, im, pos, koff} */
+    int64_t off_bucket_start;/* uint32 [n_keys + 1] */
+    int64_t off_items;       /* work items, 16 bytes each */
+} wpg_bin_info;
+int  wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+             const double *d_freq, int64_t nrow, int nchan, const wpg_kdesc *desc, wpg_prec prec,
+             void *d_workspace, size_t workspace_bytes, wpg_bin_info *h_info_out,
+             wpg_stats *h_stats_or_null);
+
+/* ---- a3: dirty image — PAPER.md:52, 88 (IFFT of the grid), R11 (grid correction) ---------- */
+size_t wpg_dirty_image_workspace_bytes(int grid_N, wpg_prec prec);
+/* image[jm][jl] = Re(centred inverse FFT of grid) * N^2-normalised / weight_sum / taper;
+ * d_image real fp32|fp64 [N][N]; d_grid is not modified. */
+int  wpg_dirty_image(wpg_ctx *ctx, const void *d_grid, const wpg_kdesc *desc, double weight_sum,
+                     wpg_prec prec, void *d_image, void *d_workspace, size_t workspace_bytes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WPGRID_H */

@@ -1,0 +1,306 @@
+// C-ABI entry points of libwpgrid.so: context, argument checks, workspace planning, sequencing.
+// The arithmetic lives in wpg_bin.cu (a1), wpg_grid.cu (a2), wpg_wkernel.cu (a0), wpg_image.cu (a3).
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "wpg_common.h"
+
+static thread_local std::string g_create_err;
+
+int wpg_fail(wpg_ctx *ctx, int code, const char *fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf; else g_create_err = buf;
+    return code;
+}
+
+extern "C" int wpg_version(void) { return 100; }
+
+extern "C" int wpg_create(wpg_ctx **out, int device, void *cuda_stream) {
+    if (!out) return wpg_fail(nullptr, WPG_EINVAL, "wpg_create: out is NULL");
+    *out = nullptr;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0)
+        return wpg_fail(nullptr, WPG_ECUDA, "wpg_create: no CUDA device (%s); there is no CPU fallback",
+                        e == cudaSuccess ? "count = 0" : cudaGetErrorString(e));
+    if (device < 0 || device >= ndev) return wpg_fail(nullptr, WPG_EINVAL, "wpg_create: bad device %d", device);
+    wpg_ctx *ctx = new wpg_ctx();
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    if (cudaSetDevice(device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        delete ctx;
+        return wpg_fail(nullptr, WPG_ECUDA, "wpg_create: cannot select device %d", device);
+    }
+    *out = ctx;
+    return WPG_OK;
+}
+
+extern "C" void wpg_destroy(wpg_ctx *ctx) {
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    if (ctx->plan) cufftDestroy(ctx->plan);
+    if (ctx->d_taper) cudaFree(ctx->d_taper);
+    if (ctx->d_host_scratch) cudaFree(ctx->d_host_scratch);
+    delete ctx;
+}
+
+extern "C" const char *wpg_last_error(const wpg_ctx *ctx) {
+    return ctx ? ctx->err.c_str() : g_create_err.c_str();
+}
+
+extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
+    if (!ctx || !name) return WPG_EINVAL;
+    if (!strcmp(name, "order")) { if (value < 0 || value > 2) return wpg_fail(ctx, WPG_EINVAL, "order must be 0..2"); ctx->opt_order = (int)value; }
+    else if (!strcmp(name, "segment")) { if (value < 0 || value > 65535) return wpg_fail(ctx, WPG_EINVAL, "segment must be 0..65535"); ctx->opt_segment = (int)value; }
+    else if (!strcmp(name, "ctas_per_sm")) { if (value < 0 || value > 32) return wpg_fail(ctx, WPG_EINVAL, "ctas_per_sm must be 0..32"); ctx->opt_ctas_per_sm = (int)value; }
+    else if (!strcmp(name, "tile")) { if (value < 0 || value > WPG_MAX_S) return wpg_fail(ctx, WPG_EINVAL, "tile must be 0..64"); ctx->opt_tile = (int)value; }
+    else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
+    return WPG_OK;
+}
+
+int wpg_check_desc(wpg_ctx *ctx, const wpg_kdesc *d) {
+    if (!d) return wpg_fail(ctx, WPG_EINVAL, "kernel descriptor is NULL");
+    if (d->Nw < 1 || d->Nw > WPG_MAX_NW) return wpg_fail(ctx, WPG_EINVAL, "Nw = %d outside 1..%d", d->Nw, WPG_MAX_NW);
+    if (d->oversample < 1 || d->oversample > 64) return wpg_fail(ctx, WPG_EINVAL, "oversample = %d outside 1..64", d->oversample);
+    if (d->grid_N < 2 || d->grid_N > WPG_MAX_N) return wpg_fail(ctx, WPG_EINVAL, "grid_N = %d outside 2..%d", d->grid_N, WPG_MAX_N);
+    if (!(d->cell > 0.0)) return wpg_fail(ctx, WPG_EINVAL, "cell must be > 0");
+    if (!(d->w_max >= 0.0)) return wpg_fail(ctx, WPG_EINVAL, "w_max must be >= 0");
+    if ((d->support == nullptr) != (d->plane_offset == nullptr))
+        return wpg_fail(ctx, WPG_EINVAL, "support and plane_offset must both be given or both be NULL");
+    int64_t off = 0;
+    for (int p = 0; p < d->Nw; ++p) {
+        int S = d->support ? d->support[p] : d->support_max;
+        if (S < 1 || S > WPG_MAX_S) return wpg_fail(ctx, WPG_EINVAL, "support[%d] = %d outside 1..%d", p, S, WPG_MAX_S);
+        if (S > d->grid_N) return wpg_fail(ctx, WPG_EINVAL, "support %d larger than the grid %d", S, d->grid_N);
+        if ((S * d->oversample) % 2) return wpg_fail(ctx, WPG_EINVAL, "support*oversample = %d*%d must be even", S, d->oversample);
+        if (S > d->support_max) return wpg_fail(ctx, WPG_EINVAL, "support[%d] = %d exceeds support_max %d", p, S, d->support_max);
+        if (d->plane_offset && d->plane_offset[p] != off)
+            return wpg_fail(ctx, WPG_EINVAL, "plane_offset[%d] = %lld, expected %lld (planes are concatenated)", p,
+                            (long long)d->plane_offset[p], (long long)off);
+        off += (int64_t)d->oversample * d->oversample * S * S;
+    }
+    if (d->plane_offset && d->plane_offset[d->Nw] != off) return wpg_fail(ctx, WPG_EINVAL, "plane_offset[Nw] inconsistent");
+    if (off >= (int64_t)1 << 31) return wpg_fail(ctx, WPG_EINVAL, "kernel stack has %lld elements, limit 2^31", (long long)off);
+    return WPG_OK;
+}
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg_prec prec,
+                  PlaneTab *tab, BinParams *bp, WorkspaceLayout *ws) {
+    int rc = wpg_check_desc(ctx, d);
+    if (rc) return rc;
+    if (nrow < 0 || nchan < 1) return wpg_fail(ctx, WPG_EINVAL, "nrow = %lld, nchan = %d", (long long)nrow, nchan);
+    if (prec != WPG_F32 && prec != WPG_F64) return wpg_fail(ctx, WPG_EINVAL, "bad precision %d", (int)prec);
+    int64_t nvis = nrow * nchan;
+    if (nvis >= ((int64_t)1 << 32) - 2) return wpg_fail(ctx, WPG_EINVAL, "nrow*nchan = %lld exceeds 2^32 - 2 per call; chunk the input", (long long)nvis);
+    memset(tab, 0, sizeof *tab);
+    int Smin = WPG_MAX_S + 1, Smax = 0;
+    int64_t off = 0;
+    std::vector<int> distinct;
+    for (int p = 0; p < d->Nw; ++p) {
+        int S = d->support ? d->support[p] : d->support_max;
+        tab->off[p] = (int32_t)off;
+        tab->S[p] = (uint8_t)S;
+        off += (int64_t)d->oversample * d->oversample * S * S;
+        Smin = std::min(Smin, S); Smax = std::max(Smax, S);
+        if (std::find(distinct.begin(), distinct.end(), S) == distinct.end()) distinct.push_back(S);
+    }
+    tab->off[d->Nw] = (int32_t)off;
+    std::sort(distinct.begin(), distinct.end());
+
+    memset(bp, 0, sizeof *bp);
+    bp->nrow = nrow; bp->nchan = nchan;
+    bp->N = d->grid_N; bp->Q = d->oversample; bp->Nw = d->Nw;
+    bp->w_max = d->w_max;
+    bp->dw = 2.0 * d->w_max / (double)d->Nw;
+    double fov = (double)d->grid_N * d->cell;
+    bp->du = 1.0 / fov;
+    bp->halfN = (double)(d->grid_N / 2);
+    bp->tile = ctx->opt_tile ? std::min(ctx->opt_tile, Smin) : Smin;
+    bp->ntile = (d->grid_N + bp->tile - 1) / bp->tile;
+    bp->segment = ctx->opt_segment ? ctx->opt_segment : 512;
+    int64_t ntile2 = (int64_t)bp->ntile * bp->ntile;
+    int order = ctx->opt_order;
+    if (order == 0) {
+        // expected records per (plane, tile) bucket if ~40% of the tiles are occupied
+        double per_bucket = (double)nvis / ((double)d->Nw * (double)ntile2 * 0.4);
+        order = per_bucket >= 12.0 ? 1 : 2;
+    }
+    if (order == 1 && (int64_t)d->Nw * ntile2 > ((int64_t)1 << 27)) order = 2;
+    bp->order = order;
+    if (order == 1) {
+        bp->ncls = d->Nw;
+        for (int p = 0; p < d->Nw; ++p) { tab->cls[p] = (uint16_t)p; tab->clsS[p] = tab->S[p]; }
+    } else {
+        bp->ncls = (int)distinct.size();
+        for (int p = 0; p < d->Nw; ++p)
+            tab->cls[p] = (uint16_t)(std::find(distinct.begin(), distinct.end(), (int)tab->S[p]) - distinct.begin());
+        for (size_t c = 0; c < distinct.size(); ++c) tab->clsS[c] = (uint8_t)distinct[c];
+    }
+    int64_t nkeys = (int64_t)bp->ncls * ntile2;
+    if (nkeys > ((int64_t)1 << 28)) return wpg_fail(ctx, WPG_EINVAL, "sort key space %lld too large", (long long)nkeys);
+    bp->nkeys = (uint32_t)nkeys;
+
+    memset(ws, 0, sizeof *ws);
+    ws->nkeys = (uint32_t)nkeys;
+    ws->nblocks_scan = (uint32_t)((nkeys + 1 + 4095) / 4096);
+    ws->max_items = std::min<int64_t>(nvis, nkeys) + nvis / bp->segment + 1;
+    size_t rec = prec == WPG_F32 ? sizeof(Rec<float>) : sizeof(Rec<double>);
+    size_t o = 0;
+    ws->off_counters = o; o += align_up(sizeof(Counters));
+    ws->off_hist = o;     o += align_up((size_t)(nkeys + 1) * 4);
+    ws->off_blocksum = o; o += align_up((size_t)ws->nblocks_scan * 8 + 8);
+    ws->off_key = o;      o += align_up((size_t)nvis * 4);
+    ws->off_rank = o;     o += align_up((size_t)nvis * 4);
+    ws->off_pre = o;      o += align_up((size_t)nvis * 8);
+    ws->off_records = o;  o += align_up((size_t)nvis * rec);
+    ws->off_items = o;    o += align_up((size_t)ws->max_items * sizeof(Item));
+    ws->total = o;
+    return WPG_OK;
+}
+
+extern "C" size_t wpg_grid_workspace_bytes(const wpg_ctx *ctx, int64_t nrow, int nchan, const wpg_kdesc *desc,
+                                           wpg_prec prec) {
+    PlaneTab tab; BinParams bp; WorkspaceLayout ws;
+    wpg_ctx tmp;
+    if (ctx) { tmp.opt_order = ctx->opt_order; tmp.opt_segment = ctx->opt_segment; tmp.opt_tile = ctx->opt_tile; }
+    if (wpg_make_plan(&tmp, desc, nrow, nchan, prec, &tab, &bp, &ws)) return 0;
+    return ws.total;
+}
+
+static int read_stats(wpg_ctx *ctx, const Counters *d_c, wpg_stats *out, Counters *h_opt) {
+    Counters h;
+    WPG_CUDA(ctx, cudaMemcpyAsync(&h, d_c, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
+    WPG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (out) {
+        out->n_gridded = (int64_t)h.n_gridded; out->n_skipped_oob = (int64_t)h.n_skipped_oob;
+        out->n_skipped_zero_weight = (int64_t)h.n_skipped_zero_weight;
+        out->n_clamped_w = (int64_t)h.n_clamped_w; out->n_updates = (int64_t)h.n_updates;
+    }
+    if (h_opt) *h_opt = h;
+    return WPG_OK;
+}
+
+static int check_ptrs(wpg_ctx *ctx, const void *vis, const void *uvw, const void *wt, const void *freq, int64_t nrow) {
+    if (!ctx) return WPG_EINVAL;
+    if (nrow > 0 && (!vis || !uvw || !wt)) return wpg_fail(ctx, WPG_EINVAL, "NULL input pointer");
+    if (!freq) return wpg_fail(ctx, WPG_EINVAL, "freq is NULL");
+    return WPG_OK;
+}
+
+static int bin_common(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                      const double *d_freq, int64_t nrow, int nchan, const wpg_kdesc *desc, wpg_prec prec,
+                      void *d_workspace, size_t workspace_bytes, PlaneTab *tab, BinParams *bp, WorkspaceLayout *ws) {
+    int rc = check_ptrs(ctx, d_vis, d_uvw, d_weight, d_freq, nrow);
+    if (rc) return rc;
+    rc = wpg_make_plan(ctx, desc, nrow, nchan, prec, tab, bp, ws);
+    if (rc) return rc;
+    if (!d_workspace || workspace_bytes < ws->total)
+        return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, ws->total);
+    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    char *w = (char *)d_workspace;
+    // counters + histogram are contiguous at the head of the workspace
+    WPG_CUDA(ctx, cudaMemsetAsync(w, 0, ws->off_blocksum, ctx->stream));
+    return wpg_launch_bin(ctx, d_vis, d_uvw, d_weight, d_freq, *tab, *bp, *ws, prec, w);
+}
+
+extern "C" int wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                       const double *d_freq, int64_t nrow, int nchan, const wpg_kdesc *desc, wpg_prec prec,
+                       void *d_workspace, size_t workspace_bytes, wpg_bin_info *info, wpg_stats *h_stats) {
+    PlaneTab tab; BinParams bp; WorkspaceLayout ws;
+    int rc = bin_common(ctx, d_vis, d_uvw, d_weight, d_freq, nrow, nchan, desc, prec, d_workspace, workspace_bytes, &tab, &bp, &ws);
+    if (rc) return rc;
+    Counters h;
+    rc = read_stats(ctx, (const Counters *)((char *)d_workspace + ws.off_counters), h_stats, &h);
+    if (rc) return rc;
+    if (info) {
+        info->n_records = h.n_records; info->n_keys = ws.nkeys; info->n_items = h.n_items;
+        info->tile = bp.tile; info->ntile = bp.ntile; info->order = bp.order;
+        info->record_bytes = prec == WPG_F32 ? 16 : 24;
+        info->off_records = (int64_t)ws.off_records; info->off_bucket_start = (int64_t)ws.off_hist;
+        info->off_items = (int64_t)ws.off_items;
+    }
+    return WPG_OK;
+}
+
+extern "C" int wpg_grid(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                        const double *d_freq, int64_t nrow, int nchan, const void *d_kernels,
+                        const wpg_kdesc *desc, wpg_prec prec, void *d_grid,
+                        void *d_workspace, size_t workspace_bytes, wpg_stats *h_stats) {
+    if (!ctx) return WPG_EINVAL;
+    if (!d_kernels || !d_grid) return wpg_fail(ctx, WPG_EINVAL, "kernels or grid pointer is NULL");
+    PlaneTab tab; BinParams bp; WorkspaceLayout ws;
+    int rc = bin_common(ctx, d_vis, d_uvw, d_weight, d_freq, nrow, nchan, desc, prec, d_workspace, workspace_bytes, &tab, &bp, &ws);
+    if (rc) return rc;
+    rc = wpg_launch_grid(ctx, tab, bp, ws, prec, d_kernels, d_grid, (char *)d_workspace, desc->support_max);
+    if (rc) return rc;
+    if (h_stats) return read_stats(ctx, (const Counters *)((char *)d_workspace + ws.off_counters), h_stats, nullptr);
+    return WPG_OK;
+}
+
+extern "C" int wpg_grid_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                              const double *d_freq, int64_t nrow, int nchan, const void *d_kernels,
+                              const wpg_kdesc *desc, wpg_prec prec, void *d_grid, wpg_stats *h_stats) {
+    int rc = check_ptrs(ctx, d_vis, d_uvw, d_weight, d_freq, nrow);
+    if (rc) return rc;
+    if (!d_kernels || !d_grid) return wpg_fail(ctx, WPG_EINVAL, "kernels or grid pointer is NULL");
+    PlaneTab tab; BinParams bp; WorkspaceLayout ws;
+    rc = wpg_make_plan(ctx, desc, nrow, nchan, prec, &tab, &bp, &ws);
+    if (rc) return rc;
+    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    Counters *d_c = nullptr;
+    WPG_CUDA(ctx, cudaMallocAsync((void **)&d_c, sizeof(Counters), ctx->stream));
+    WPG_CUDA(ctx, cudaMemsetAsync(d_c, 0, sizeof(Counters), ctx->stream));
+    rc = wpg_launch_naive(ctx, d_vis, d_uvw, d_weight, d_freq, tab, bp, prec, d_kernels, d_grid, d_c);
+    if (!rc && h_stats) rc = read_stats(ctx, d_c, h_stats, nullptr);
+    cudaFreeAsync(d_c, ctx->stream);
+    return rc;
+}
+
+extern "C" int wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uvw, const float *h_weight,
+                             const double *h_freq, int64_t nrow, int nchan, const void *d_kernels,
+                             const wpg_kdesc *desc, wpg_prec prec, void *h_grid_out, wpg_stats *h_stats) {
+    int rc = check_ptrs(ctx, h_vis, h_uvw, h_weight, h_freq, nrow);
+    if (rc) return rc;
+    if (!d_kernels || !h_grid_out) return wpg_fail(ctx, WPG_EINVAL, "kernels or grid pointer is NULL");
+    PlaneTab tab; BinParams bp; WorkspaceLayout ws;
+    rc = wpg_make_plan(ctx, desc, nrow, nchan, prec, &tab, &bp, &ws);
+    if (rc) return rc;
+    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    int64_t nvis = nrow * nchan;
+    size_t cplx = prec == WPG_F32 ? 8 : 16;
+    size_t b_vis = align_up((size_t)nvis * 8), b_uvw = align_up((size_t)nrow * 24), b_wt = align_up((size_t)nvis * 4),
+           b_freq = align_up((size_t)nchan * 8), b_grid = align_up((size_t)desc->grid_N * desc->grid_N * cplx);
+    size_t need = b_vis + b_uvw + b_wt + b_freq + b_grid + ws.total;
+    if (need > ctx->host_scratch_bytes) {
+        WPG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        if (ctx->d_host_scratch) cudaFree(ctx->d_host_scratch);
+        ctx->d_host_scratch = nullptr; ctx->host_scratch_bytes = 0;
+        cudaError_t e = cudaMalloc(&ctx->d_host_scratch, need);
+        if (e != cudaSuccess) return wpg_fail(ctx, WPG_ENOMEM, "cannot allocate %zu bytes of device scratch: %s", need, cudaGetErrorString(e));
+        ctx->host_scratch_bytes = need;
+    }
+    char *base = (char *)ctx->d_host_scratch;
+    char *dv = base, *du = dv + b_vis, *dw = du + b_uvw, *df = dw + b_wt, *dg = df + b_freq, *dws = dg + b_grid;
+    cudaStream_t s = ctx->stream;
+    WPG_CUDA(ctx, cudaMemcpyAsync(dv, h_vis, (size_t)nvis * 8, cudaMemcpyHostToDevice, s));
+    WPG_CUDA(ctx, cudaMemcpyAsync(du, h_uvw, (size_t)nrow * 24, cudaMemcpyHostToDevice, s));
+    WPG_CUDA(ctx, cudaMemcpyAsync(dw, h_weight, (size_t)nvis * 4, cudaMemcpyHostToDevice, s));
+    WPG_CUDA(ctx, cudaMemcpyAsync(df, h_freq, (size_t)nchan * 8, cudaMemcpyHostToDevice, s));
+    WPG_CUDA(ctx, cudaMemsetAsync(dg, 0, (size_t)desc->grid_N * desc->grid_N * cplx, s));
+    rc = wpg_grid(ctx, dv, (const double *)du, (const float *)dw, (const double *)df, nrow, nchan, d_kernels, desc,
+                  prec, dg, dws, ws.total, nullptr);
+    if (rc) return rc;
+    WPG_CUDA(ctx, cudaMemcpyAsync(h_grid_out, dg, (size_t)desc->grid_N * desc->grid_N * cplx, cudaMemcpyDeviceToHost, s));
+    if (h_stats) return read_stats(ctx, (const Counters *)(dws + ws.off_counters), h_stats, nullptr);
+    WPG_CUDA(ctx, cudaStreamSynchronize(s));
+    return WPG_OK;
+}

@@ -1,0 +1,100 @@
+// Step a3 — dirty image: centre-origin inverse 2-D FFT of the grid, real part, / sum of weights,
+// / taper ("the master node performs an IFFT on the ... gridding result";
+// DESIGN.md O5, R11).  The fftshift/ifftshift pair is folded into (-1)^(i+j) sign checkerboards
+// before and after a plain cuFFT transform (N even), so no data is moved for the shift:
+//   img[n] = (-1)^(n1+n2) * IFFT_unnormalised[(-1)^(k1+k2) g[k]]   (the constant (-1)^N is 1).
+#include "wpg_common.h"
+
+namespace {
+
+constexpr double kTaperFloor = 1e-3;
+
+template <typename C>
+__global__ void __launch_bounds__(256)
+checkerboard_copy(const C *__restrict__ g, C *__restrict__ out, int N) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= N) return;
+    C v = g[(size_t)j * N + i];
+    if ((i + j) & 1) { v.x = -v.x; v.y = -v.y; }
+    out[(size_t)j * N + i] = v;
+}
+
+template <typename C, typename T>
+__global__ void __launch_bounds__(256)
+correct_kernel(const C *__restrict__ f, T *__restrict__ img, const double *__restrict__ taper, int N, double inv_wsum) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= N) return;
+    double t = taper[i] * taper[j];
+    double v = (double)f[(size_t)j * N + i].x;
+    if ((i + j) & 1) v = -v;
+    img[(size_t)j * N + i] = t >= kTaperFloor ? (T)(v * inv_wsum / t) : (T)0;
+}
+
+const char *cufft_str(cufftResult r) {
+    switch (r) {
+        case CUFFT_SUCCESS: return "CUFFT_SUCCESS";
+        case CUFFT_ALLOC_FAILED: return "CUFFT_ALLOC_FAILED";
+        case CUFFT_INVALID_VALUE: return "CUFFT_INVALID_VALUE";
+        case CUFFT_INTERNAL_ERROR: return "CUFFT_INTERNAL_ERROR";
+        case CUFFT_EXEC_FAILED: return "CUFFT_EXEC_FAILED";
+        case CUFFT_SETUP_FAILED: return "CUFFT_SETUP_FAILED";
+        case CUFFT_INVALID_SIZE: return "CUFFT_INVALID_SIZE";
+        default: return "CUFFT error";
+    }
+}
+
+}  // namespace
+
+extern "C" size_t wpg_dirty_image_workspace_bytes(int grid_N, wpg_prec prec) {
+    if (grid_N < 2) return 0;
+    return (size_t)grid_N * grid_N * (prec == WPG_F32 ? 8 : 16);
+}
+
+extern "C" int wpg_dirty_image(wpg_ctx *ctx, const void *d_grid, const wpg_kdesc *desc, double weight_sum,
+                               wpg_prec prec, void *d_image, void *d_workspace, size_t workspace_bytes) {
+    if (!ctx) return WPG_EINVAL;
+    int rc = wpg_check_desc(ctx, desc);
+    if (rc) return rc;
+    if (!d_grid || !d_image) return wpg_fail(ctx, WPG_EINVAL, "grid or image pointer is NULL");
+    if (prec != WPG_F32 && prec != WPG_F64) return wpg_fail(ctx, WPG_EINVAL, "bad precision");
+    const int N = desc->grid_N;
+    if (N % 2) return wpg_fail(ctx, WPG_EINVAL, "dirty_image needs an even grid size, got %d", N);
+    if (!(weight_sum > 0.0)) return wpg_fail(ctx, WPG_EINVAL, "weight_sum must be > 0");
+    size_t need = wpg_dirty_image_workspace_bytes(N, prec);
+    if (!d_workspace || workspace_bytes < need)
+        return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, need);
+    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (ctx->plan_N != N || ctx->plan_prec != (int)prec) {
+        if (ctx->plan) { cufftDestroy(ctx->plan); ctx->plan = 0; ctx->plan_N = 0; }
+        cufftResult r = cufftPlan2d(&ctx->plan, N, N, prec == WPG_F32 ? CUFFT_C2C : CUFFT_Z2Z);
+        if (r != CUFFT_SUCCESS) { ctx->plan = 0; return wpg_fail(ctx, WPG_ECUDA, "cufftPlan2d: %s", cufft_str(r)); }
+        ctx->plan_N = N; ctx->plan_prec = (int)prec;
+    }
+    cufftResult r = cufftSetStream(ctx->plan, ctx->stream);
+    if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftSetStream: %s", cufft_str(r));
+    if (ctx->taper_N != N) {
+        if (ctx->d_taper) { cudaFree(ctx->d_taper); ctx->d_taper = nullptr; ctx->taper_N = 0; }
+        std::vector<double> nu(N), t(N);
+        double fov = (double)N * desc->cell;
+        for (int j = 0; j < N; ++j) nu[j] = 2.0 * ((j - N / 2) * desc->cell) / fov;
+        wpg_pswf_eval(nu.data(), N, t.data());
+        WPG_CUDA(ctx, cudaMalloc((void **)&ctx->d_taper, (size_t)N * 8));
+        WPG_CUDA(ctx, cudaMemcpy(ctx->d_taper, t.data(), (size_t)N * 8, cudaMemcpyHostToDevice));
+        ctx->taper_N = N;
+    }
+    dim3 gr((N + 255) / 256, N);
+    cudaStream_t s = ctx->stream;
+    if (prec == WPG_F32) {
+        checkerboard_copy<float2><<<gr, 256, 0, s>>>((const float2 *)d_grid, (float2 *)d_workspace, N);
+        r = cufftExecC2C(ctx->plan, (cufftComplex *)d_workspace, (cufftComplex *)d_workspace, CUFFT_INVERSE);
+        if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftExecC2C: %s", cufft_str(r));
+        correct_kernel<float2, float><<<gr, 256, 0, s>>>((const float2 *)d_workspace, (float *)d_image, ctx->d_taper, N, 1.0 / weight_sum);
+    } else {
+        checkerboard_copy<double2><<<gr, 256, 0, s>>>((const double2 *)d_grid, (double2 *)d_workspace, N);
+        r = cufftExecZ2Z(ctx->plan, (cufftDoubleComplex *)d_workspace, (cufftDoubleComplex *)d_workspace, CUFFT_INVERSE);
+        if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftExecZ2Z: %s", cufft_str(r));
+        correct_kernel<double2, double><<<gr, 256, 0, s>>>((const double2 *)d_workspace, (double *)d_image, ctx->d_taper, N, 1.0 / weight_sum);
+    }
+    WPG_CUDA(ctx, cudaGetLastError());
+    return WPG_OK;
+}

@@ -1,0 +1,258 @@
+"""GPU <-> oracle parity (-m gpu).  Everything goes through the C ABI (libwpgrid.so) via the
+thin binding.  Tolerances (north_star / DESIGN.md R17): max|g - g_oracle| <= 1e-4 max|g_oracle|
+for fp32 and <= 1e-10 max|g_oracle| for fp64; integer outputs (counters, records) bit-exact."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import gridder as ogrid
+from oracle import image as oimage
+from oracle import wkernel as owk
+from paper_1905_03213_b200 import synth, wpgrid
+
+TOL = {wpgrid.F32: 1e-4, wpgrid.F64: 1e-10}
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    c = wpgrid.Context(0)
+    yield c
+    c.close()
+
+
+def dev(wl):
+    return (torch.from_numpy(wl.vis).cuda(), torch.from_numpy(wl.uvw).cuda(),
+            torch.from_numpy(wl.weight).cuda(), torch.from_numpy(wl.freq).cuda())
+
+
+def oracle_stack(wl):
+    sup = wl.support
+    if not np.isscalar(sup):
+        sup = owk.ragged_support(wl.Nw, wl.w_max, wl.grid_N, wl.cell, sup[1], sup[2])
+    return owk.build_stack(wl.Nw, wl.w_max, sup, wl.oversample, wl.grid_N, wl.cell)
+
+
+def upload(ctx, st, prec):
+    sup = int(st.support[0]) if st.uniform else st.support
+    return ctx.stack_from_host(st.data, st.Nw, st.w_max, sup, st.oversample, st.grid_N, st.cell, prec)
+
+
+def relerr(g, ref):
+    return float(np.max(np.abs(g.astype(np.complex128) - ref)) / np.max(np.abs(ref)))
+
+
+def check_all_paths(ctx, wl, st, ref, rstats, precs=(wpgrid.F32, wpgrid.F64), orders=(1, 2), segments=(0,)):
+    d = dev(wl)
+    for prec in precs:
+        ks = upload(ctx, st, prec)
+        g, s = ctx.grid_naive(*d, ks, stats=True)
+        assert s == rstats
+        assert relerr(g.cpu().numpy(), ref) <= TOL[prec], ("naive", prec)
+        for order in orders:
+            for seg in segments:
+                ctx.set_option("order", order); ctx.set_option("segment", seg)
+                g, s = ctx.grid(*d, ks, stats=True)
+                assert s == rstats, (order, seg)
+                e = relerr(g.cpu().numpy(), ref)
+                assert e <= TOL[prec], ("tiled", prec, order, seg, e)
+    ctx.set_option("order", 0); ctx.set_option("segment", 0)
+
+
+# ------------------------------------------------------------------ config 1 (full size)
+@pytest.fixture(scope="module")
+def cfg1():
+    wl = synth.config1()
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st)
+    return wl, st, ref, rstats
+
+
+def test_config1_gridder_parity(ctx, cfg1):
+    wl, st, ref, rstats = cfg1
+    check_all_paths(ctx, wl, st, ref, rstats, segments=(0, 7, 100))
+
+
+def test_config1_wkernel_build_parity(ctx, cfg1):
+    wl, st, _, _ = cfg1
+    K = st.data
+    k64 = ctx.wkernel_build(wl.Nw, wl.w_max, wl.support, wl.oversample, wl.grid_N, wl.cell, wpgrid.F64)
+    assert np.max(np.abs(k64.data.cpu().numpy() - K)) <= 1e-10 * np.max(np.abs(K))
+    k32 = ctx.wkernel_build(wl.Nw, wl.w_max, wl.support, wl.oversample, wl.grid_N, wl.cell, wpgrid.F32)
+    assert np.max(np.abs(k32.data.cpu().numpy() - K)) <= 1e-6 * np.max(np.abs(K))
+
+
+def test_config1_end_to_end_image(ctx, cfg1):
+    """wkernel_build -> grid -> dirty_image entirely in the library vs the oracle chain."""
+    wl, st, ref, _ = cfg1
+    d = dev(wl)
+    wsum = float(wl.weight.sum())
+    ref_img = oimage.dirty_image(ref, wl.cell, wsum)
+    for prec, tol in ((wpgrid.F32, 1e-4), (wpgrid.F64, 1e-9)):
+        ks = ctx.wkernel_build(wl.Nw, wl.w_max, wl.support, wl.oversample, wl.grid_N, wl.cell, prec)
+        g, _ = ctx.grid(*d, ks)
+        assert relerr(g.cpu().numpy(), ref) <= (2e-4 if prec == wpgrid.F32 else 1e-9)
+        img = ctx.dirty_image(g, ks, wsum).cpu().numpy().astype(np.float64)
+        assert np.max(np.abs(img - ref_img)) <= tol * np.max(np.abs(ref_img))
+        # the image step alone, fed the oracle's grid
+        gi = torch.from_numpy(ref.astype(np.complex64 if prec == wpgrid.F32 else np.complex128)).cuda()
+        img = ctx.dirty_image(gi, ks, wsum).cpu().numpy().astype(np.float64)
+        # (fp32: the division by a taper as small as 1e-3 amplifies the FFT's rounding near the edge)
+        assert np.max(np.abs(img - ref_img)) <= (1e-4 if prec == wpgrid.F32 else 1e-12) * np.max(np.abs(ref_img))
+        assert np.array_equal(img == 0.0, ref_img == 0.0)
+
+
+def test_grid_host_variant_matches(ctx, cfg1):
+    wl, st, ref, rstats = cfg1
+    ks = upload(ctx, st, wpgrid.F32)
+    out, s = ctx.grid_host(wl.vis, wl.uvw, wl.weight, wl.freq, ks, stats=True)
+    assert s == rstats and relerr(out, ref) <= 1e-4
+    out2, _ = ctx.grid_host(wl.vis, wl.uvw, wl.weight, wl.freq, ks)       # grid is overwritten, not accumulated
+    assert relerr(out2, ref) <= 1e-4
+
+
+# ------------------------------------------------------------------ binning (bit-exact)
+def test_binning_records_match_oracle_index_map(ctx):
+    wl = synth.config1(nvis=20000)
+    st = oracle_stack(wl)
+    ks = upload(ctx, st, wpgrid.F32)
+    d = dev(wl)
+    S, Q, N = 7, 8, wl.grid_N
+    exp = []
+    for k in range(wl.uvw.shape[0]):
+        j0u, ou = ogrid.index_map(wl.uvw[k, 0], N, wl.cell, S, Q)
+        j0v, ov = ogrid.index_map(wl.uvw[k, 1], N, wl.cell, S, Q)
+        p, _ = ogrid.plane_of(wl.uvw[k, 2], wl.w_max, wl.Nw)
+        exp.append((j0u | (j0v << 13) | ((S - 1) << 26), (p * Q * Q + ov * Q + ou) * S * S,
+                    np.float32(wl.vis[k, 0].real).view(np.uint32), np.float32(wl.vis[k, 0].imag).view(np.uint32)))
+    exp = sorted(exp)
+    for order in (1, 2):
+        ctx.set_option("order", order)
+        ws, info, stats = ctx.bin(*d, ks)
+        assert info["n_records"] == 20000 and info["order"] == order and info["tile"] == 7
+        raw = ws.cpu().numpy()
+        rec = raw[info["off_records"]:info["off_records"] + 16 * 20000].view(np.uint32).reshape(-1, 4)
+        got = sorted((int(r[2]), int(r[3]), int(r[0]), int(r[1])) for r in rec)
+        assert got == [tuple(int(x) for x in e) for e in exp]
+        # records are grouped by key: bucket_start is monotone and ends at n_records; items cover every record once
+        bs = raw[info["off_bucket_start"]:info["off_bucket_start"] + 4 * (info["n_keys"] + 1)].view(np.uint32)
+        assert bs[0] == 0 and bs[-1] == 20000 and np.all(np.diff(bs.astype(np.int64)) >= 0)
+        items = raw[info["off_items"]:info["off_items"] + 16 * info["n_items"]].view(np.uint32).reshape(-1, 4)
+        cover = np.zeros(20000, np.int32)
+        for b, c, org, s_ in items:
+            cover[b:b + c] += 1
+            u0, v0 = int(org) & 0xFFFF, int(org) >> 16
+            ju = rec[b:b + c, 2] & 0x1FFF; jv = (rec[b:b + c, 2] >> 13) & 0x1FFF
+            assert s_ == 7 and np.all((ju >= u0) & (ju < u0 + 7) & (jv >= v0) & (jv < v0 + 7))
+        assert np.all(cover == 1)
+    ctx.set_option("order", 0)
+
+
+# ------------------------------------------------------------------ edge cases
+def test_edge_cases(ctx):
+    N, cell, Q, S, Nw, w_max = 64, 0.08 / 64, 8, 8, 4, 50.0
+    st = owk.build_stack(Nw, w_max, S, Q, N, cell)
+    du = 1.0 / 0.08
+    uvw = np.array([[0.0, 0.0, 0.0], [40 * du, 0.0, 0.0], [-29 * du, 0.0, 0.0], [-29.1 * du, 0.0, 0.0],
+                    [0.0, 28.4 * du, 10.0], [0.0, 27.4 * du, 10.0], [du, du, 80.0], [du, du, -80.0],
+                    [1e30, 0.0, 0.0], [0.0, -1e30, 1e30]])
+    n = uvw.shape[0]
+    vis = (np.arange(n) + 1 + 1j * np.arange(n)).astype(np.complex64)[:, None]
+    wt = np.ones((n, 1), np.float32); wt[5, 0] = 0.0
+    freq = np.array([synth.C0])
+    ref, rstats = ogrid.grid(uvw, vis, wt, freq, st)
+    wl = synth.Workload("edge", uvw, freq, vis, wt, N, cell, Nw, w_max, S, Q)
+    check_all_paths(ctx, wl, st, ref, rstats)
+    # empty input: nothing happens, counters are zero
+    ks = upload(ctx, st, wpgrid.F32)
+    z = (torch.zeros((0, 1), dtype=torch.complex64).cuda(), torch.zeros((0, 3), dtype=torch.float64).cuda(),
+         torch.zeros((0, 1), dtype=torch.float32).cuda(), torch.from_numpy(freq).cuda())
+    g, s = ctx.grid(*z, ks, stats=True)
+    assert not g.any() and all(v == 0 for v in s.values())
+    # everything flagged
+    d = dev(wl)
+    g, s = ctx.grid(d[0], d[1], torch.zeros_like(d[2]), d[3], ks, stats=True)
+    assert not g.any() and s["n_skipped_zero_weight"] == n and s["n_gridded"] == 0
+    # accumulation into a non-zero grid (chunking, P12)
+    g0 = torch.from_numpy(ref.astype(np.complex64)).cuda()
+    g, _ = ctx.grid(*d, ks, grid=g0.clone())
+    assert relerr(g.cpu().numpy(), 2 * ref) <= 1e-4
+
+
+def test_errors_cross_the_abi_as_codes(ctx):
+    st = owk.build_stack(2, 10.0, 8, 8, 64, 0.001)
+    ks = upload(ctx, st, wpgrid.F32)
+    wl = synth.config1(nvis=16)
+    d = dev(wl)
+    with pytest.raises(wpgrid.WpgError) as e:
+        ctx.grid(*d, ks, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == wpgrid.ENOMEM
+    with pytest.raises(wpgrid.WpgError) as e:
+        ctx.wkernel_build(4, 10.0, 7, 3, 64, 0.001)        # S*Q odd
+    assert e.value.code == wpgrid.EINVAL
+    with pytest.raises(wpgrid.WpgError) as e:
+        ctx.set_option("nonsense", 1)
+    assert e.value.code == wpgrid.EINVAL
+
+
+def test_multichannel_and_weights(ctx):
+    rng = np.random.default_rng(21)
+    N, cell, Q, S, Nw = 256, 0.1 / 256, 8, 8, 8
+    nrow, nchan = 3000, 4
+    uvw = np.stack([rng.uniform(-600, 600, nrow), rng.uniform(-600, 600, nrow), rng.uniform(-40, 40, nrow)], 1)
+    freq = np.linspace(0.9, 1.3, nchan) * synth.C0 / 0.5          # wavelengths 0.5/0.9 ... m
+    w_max = 100.0
+    vis = (rng.standard_normal((nrow, nchan)) + 1j * rng.standard_normal((nrow, nchan))).astype(np.complex64)
+    wt = rng.uniform(0.0, 2.0, (nrow, nchan)).astype(np.float32)
+    wt[rng.uniform(size=wt.shape) < 0.1] = 0.0
+    st = owk.build_stack(Nw, w_max, S, Q, N, cell)
+    ref, rstats = ogrid.grid(uvw, vis, wt, freq, st)
+    assert rstats["n_skipped_zero_weight"] > 0 and rstats["n_skipped_oob"] > 0 and rstats["n_clamped_w"] > 0
+    wl = synth.Workload("mc", uvw, freq, vis, wt, N, cell, Nw, w_max, S, Q)
+    check_all_paths(ctx, wl, st, ref, rstats)
+
+
+# ------------------------------------------------------------------ the other configs, scaled
+@pytest.mark.parametrize("S", [4, 7, 8, 12, 16])
+def test_config3_supports(ctx, S):
+    """Config-3 sweep points at reduced visibility count (N = 1024, every support of the sweep
+    plus the odd 7): several tiles, ragged tails, fp32 and fp64, both sort orders."""
+    wl = synth.config3(N=1024, S=S, nvis=150_000)
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    assert rstats["n_gridded"] == 150_000
+    check_all_paths(ctx, wl, st, ref, rstats)
+
+
+def test_config2_scaled(ctx):
+    wl = synth.config2(nvis=400_000)
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    check_all_paths(ctx, wl, st, ref, rstats, precs=(wpgrid.F32,))
+    ks = ctx.wkernel_build(wl.Nw, wl.w_max, wl.support, wl.oversample, wl.grid_N, wl.cell, wpgrid.F64)
+    assert np.max(np.abs(ks.data.cpu().numpy() - st.data)) <= 1e-10 * np.max(np.abs(st.data))
+
+
+def test_config4_ragged_scaled(ctx):
+    """SKA-low-like layout, ragged support 8..32, 8 channels, N = 8192; 2 dumps (2.1e6 visibilities)."""
+    wl = synth.config4(n_dump=2, values="random")
+    st = oracle_stack(wl)
+    assert st.support.min() >= 8 and len(set(st.support.tolist())) >= 4
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    sup, off = wpgrid.ragged_support(wl.Nw, wl.w_max, wl.grid_N, wl.cell, wl.oversample, 8, 32)
+    assert np.array_equal(sup, st.support) and np.array_equal(off, st.plane_offset)
+    check_all_paths(ctx, wl, st, ref, rstats, precs=(wpgrid.F32,))
+    # the library's own ragged stack
+    ks = ctx.wkernel_build(wl.Nw, wl.w_max, sup, wl.oversample, wl.grid_N, wl.cell, wpgrid.F64)
+    assert np.max(np.abs(ks.data.cpu().numpy() - st.data)) <= 1e-10 * np.max(np.abs(st.data))
+
+
+def test_config5_scaled_both_precisions(ctx):
+    wl = synth.config5(nvis=300_000)
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    check_all_paths(ctx, wl, st, ref, rstats)
