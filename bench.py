@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the w-projection gridding hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+                    [--workload config2|config1|config3:N:S|config5] [--nvis n] [--prec f32|f64]
+
+One "step" = one pass of the whole hot path over one batch of synthetic
+visibilities that is already resident in HBM: grid zero-fill -> binning (a1) -> gridder (a2) ->
+dirty image (a3).  a0 (wkernel_build) is setup and untimed.  The metric is grid-point updates/s
+(sum of S_p^2 over the gridded visibilities / time).  Inputs (360 MB at config 2) are larger than
+the 126 MB L2, so no explicit L2 flush is needed between iterations (stated in `config`).
+
+Multi-GPU: the path does not shard (north_star: "no sharding and no collectives"), so --gpus N
+under torchrun runs N independent replicas ("replicas only") and reports their sum.
+
+`--impl reference` times the oracle (oracle/, plain fp64 C loops) on the host cores on a bounded
+prefix of the same workload; rank 0 only.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "grid-point updates/sec (vis x support^2)"
+UNIT = "updates/s"
+# FP32 FMA peak used for the "alu" roofline: 148 SMs x 128 FP32 lanes x 2 flop x
+# 1.965 GHz (max SM clock, MEASURED_PEAKS.json / B200_PROFILING.md); FP64 is half of that.
+SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
+FLOP_PER_UPDATE = 8          # one complex multiply-add = 4 real FMA
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--nvis", type=int, default=0, help="override the visibility count (0 = the config's)")
+    ap.add_argument("--prec", default="f32", choices=["f32", "f64"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--option", action="append", default=[], help="library option name=value (tuning)")
+    return ap.parse_args()
+
+
+def make_workload(spec, nvis, device):
+    from paper_1905_03213_b200 import synth
+    kw = {"nvis": nvis} if nvis else {}
+    parts = spec.split(":")
+    if parts[0] == "config1":
+        return synth.config1(**kw)
+    if parts[0] == "config2":
+        return synth.config2(device=device, **kw)
+    if parts[0] == "config3":
+        N = int(parts[1]) if len(parts) > 1 else 2048
+        S = int(parts[2]) if len(parts) > 2 else 8
+        return synth.config3(N=N, S=S, **kw)
+    if parts[0] == "config5":
+        return synth.config5(device=device, **kw)
+    raise SystemExit("unknown workload %r" % spec)
+
+
+def workload_config(wl, prec):
+    return {"workload": wl.name, "grid_N": wl.grid_N, "nvis": int(wl.nvis), "nchan": int(wl.freq.size),
+            "Nw": wl.Nw, "support": wl.support if np.isscalar(wl.support) else list(wl.support),
+            "oversample": wl.oversample, "precision": prec,
+            "step": "grid zero-fill + binning (a1) + gridder (a2) + dirty_image (a3); wkernel_build (a0) untimed",
+            "l2": "inputs (%.0f MB) larger than the 126 MB L2; no explicit flush" %
+                  ((wl.uvw.nbytes + wl.vis.nbytes + wl.weight.nbytes) / 1e6)}
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._halt = threading.Event()
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:          # NVML missing: report that, do not fake numbers
+            self.nv, self.err = None, repr(e)
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._halt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._halt.wait(0.005)
+
+    def stop(self):
+        self._halt.set()
+        self.join(timeout=2)
+        if self.nv is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable: " + self.err]}
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# --------------------------------------------------------------------------- oracle legs
+def oracle_stack(wl):
+    from oracle import wkernel as owk
+    sup = wl.support
+    if not np.isscalar(sup):
+        sup = owk.ragged_support(wl.Nw, wl.w_max, wl.grid_N, wl.cell, sup[1], sup[2])
+    return owk.build_stack(wl.Nw, wl.w_max, sup, wl.oversample, wl.grid_N, wl.cell)
+
+
+def oracle_threads(wl):
+    from oracle import gridder as ogrid
+    cores = os.cpu_count() or 1
+    # private grid per thread (the paper's CPU method): cap the memory at ~8 GB
+    cap = max(1, int(8e9 // (wl.grid_N * wl.grid_N * 16)))
+    return max(1, min(cores, ogrid.max_threads(), cap, 64))
+
+
+def time_oracle(wl, st, rows, threads):
+    from oracle import gridder as ogrid
+    t0 = time.perf_counter()
+    _, stats = ogrid.grid(wl.uvw[:rows], wl.vis[:rows], wl.weight[:rows], wl.freq, st, threads=threads)
+    return time.perf_counter() - t0, stats["n_updates"]
+
+
+def cpu_baseline(wl, target_s=12.0):
+    """The oracle as it stands on the host cores, on a prefix of the same workload sized for
+    about `target_s` seconds (throughput per update makes a prefix legitimate)."""
+    st = oracle_stack(wl)
+    threads = oracle_threads(wl)
+    nrow = wl.uvw.shape[0]
+    probe = min(nrow, 200_000)
+    dt, upd = time_oracle(wl, st, probe, threads)
+    rate = upd / max(dt, 1e-9)
+    per_row = max(upd / probe, 1.0)
+    rows = int(min(nrow, max(probe, target_s * rate / per_row)))
+    # a workload the oracle finishes in well under target_s is passed over several times
+    t_sum, upd_sum, passes = 0.0, 0, 0
+    while passes == 0 or (rows == nrow and t_sum < target_s and passes < 50):
+        dt, upd = time_oracle(wl, st, rows, threads)
+        t_sum += dt; upd_sum += upd; passes += 1
+    return {"value": upd_sum / t_sum, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "%d pass(es) over the first %d of %d rows (%d updates per pass) of %s, fp64, "
+                      "OpenMP private grids, %.1f s in total" % (passes, rows, nrow, upd_sum // passes, wl.name, t_sum)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = make_workload(args.workload, args.nvis, None)
+    st = oracle_stack(wl)
+    threads = oracle_threads(wl)
+    nrow = wl.uvw.shape[0]
+    probe = min(nrow, 200_000)
+    dt, upd = time_oracle(wl, st, probe, threads)
+    total = max(1, args.steps + args.warmup)
+    budget_s = min(20.0, 150.0 / total)                      # whole run within a few minutes
+    rows = int(min(nrow, max(probe, budget_s * (upd / dt) / max(upd / probe, 1.0))))
+    for _ in range(args.warmup):
+        time_oracle(wl, st, rows, threads)
+    t_sum, upd_sum = 0.0, 0
+    for _ in range(args.steps):
+        dt, upd = time_oracle(wl, st, rows, threads)
+        t_sum += dt; upd_sum += upd
+    value = upd_sum / t_sum
+    sample = "each step = first %d of %d rows of %s, fp64 oracle, OpenMP private grids" % (rows, nrow, wl.name)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_sum / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(wl, "f64"),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+# --------------------------------------------------------------------------- the CUDA arm
+def traffic_from_profiles(workload, prec):
+    """dram bytes per gridder launch from the committed ncu --set full capture, if there is one."""
+    path = os.path.join(ROOT, "profiles", "gridder_traffic.json")
+    try:
+        with open(path) as f:
+            return json.load(f).get("%s/%s" % (workload, prec), {}).get("dram_bytes_per_launch")
+    except (OSError, ValueError):
+        return None
+
+
+def run_b200(args):
+    import torch
+    from paper_1905_03213_b200 import wpgrid
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus > 1 and world != args.gpus:
+        raise SystemExit("--gpus %d needs torchrun with %d ranks (WORLD_SIZE=%d)" % (args.gpus, args.gpus, world))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libwpgrid has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    dev = torch.device("cuda", local)
+    prec = wpgrid.F32 if args.prec == "f32" else wpgrid.F64
+    wl = make_workload(args.workload, args.nvis, dev)
+    ctx = wpgrid.Context(local)
+    for o in args.option:
+        k, v = o.split("=")
+        ctx.set_option(k, int(v))
+    ctx.set_option("timing", 1)
+    sup = wl.support
+    if not np.isscalar(sup):
+        sup, _ = wpgrid.ragged_support(wl.Nw, wl.w_max, wl.grid_N, wl.cell, wl.oversample, sup[1], sup[2])
+    stack = ctx.wkernel_build(wl.Nw, wl.w_max, sup, wl.oversample, wl.grid_N, wl.cell, prec)      # a0, untimed
+
+    # inputs resident in HBM before the timed region
+    d_vis = torch.from_numpy(wl.vis).to(dev); d_uvw = torch.from_numpy(wl.uvw).to(dev)
+    d_wt = torch.from_numpy(wl.weight).to(dev); d_freq = torch.from_numpy(wl.freq).to(dev)
+    nrow, nchan = wl.uvw.shape[0], wl.freq.size
+    wsum = float(wl.weight.sum())
+    grid = ctx.new_grid(stack)
+    ws = torch.empty(ctx.grid_workspace_bytes(nrow, nchan, stack), dtype=torch.uint8, device=dev)
+    iws = torch.empty(int(ctx.lib.wpg_dirty_image_workspace_bytes(wl.grid_N, prec)), dtype=torch.uint8, device=dev)
+
+    def step():
+        grid.zero_()
+        ctx.grid(d_vis, d_uvw, d_wt, d_freq, stack, grid=grid, workspace=ws)
+        return ctx.dirty_image(grid, stack, wsum, workspace=iws)
+
+    _, stats = ctx.grid(d_vis, d_uvw, d_wt, d_freq, stack, grid=ctx.new_grid(stack), workspace=ws, stats=True)
+    n_updates = stats["n_updates"]
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    ctx.phase_ms()                                     # drop the warm-up phase timings
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = ctx.launch_count()
+    barrier()
+    sampler.start()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = ctx.launch_count() - launches0
+    ms_total = e0.elapsed_time(e1)
+    bin_ms, grid_ms = ctx.phase_ms()
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * n_updates / (ms_step * 1e-3)
+
+    # ---- e2e: host buffers through wpg_grid_host, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        h = [torch.from_numpy(x).pin_memory() for x in (wl.vis, wl.uvw, wl.weight, wl.freq)]
+        N = wl.grid_N
+        h_grid = torch.empty((N, N), dtype=torch.complex64 if prec == wpgrid.F32 else torch.complex128).pin_memory()
+        h_img = torch.empty((N, N), dtype=torch.float32 if prec == wpgrid.F32 else torch.float64).pin_memory()
+        for _ in range(2):
+            ctx.grid_host(*h, stack, out=h_grid, image_out=h_img, weight_sum=wsum)
+        ksteps = max(3, min(args.steps, 10))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ksteps):
+            ctx.grid_host(*h, stack, out=h_grid, image_out=h_img, weight_sum=wsum)   # synchronises
+        dt = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([dt], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * n_updates * ksteps / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(sum(x.numel() * x.element_size() for x in h)),
+               "d2h_bytes_per_step": int(h_grid.numel() * h_grid.element_size() + h_img.numel() * h_img.element_size()),
+               "ms_per_step": 1e3 * dt / ksteps, "steps": ksteps,
+               "call": "wpg_grid_host (pinned host buffers -> host grid + image)"}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the gridder): plain FP32/FP64 ALU work, DESIGN.md §7
+    peak_tflops = SM_COUNT * FP32_LANES * 2 * SM_MAX_GHZ / 1e3 / (1 if prec == wpgrid.F32 else 2)
+    achieved = n_updates * FLOP_PER_UPDATE / (grid_ms * 1e-3) / 1e12
+    roofline = {"bound": "alu", "kernel": "gridder (a2)", "achieved": achieved, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                "traffic": traffic_from_profiles(wl.name, args.prec),
+                "peak_source": "derived: 148 SM x 128 lanes x 2 flop x 1.965 GHz%s (DESIGN.md §7)"
+                               % ("" if prec == wpgrid.F32 else " / 2 for fp64"),
+                "gridder_ms": grid_ms, "binning_ms": bin_ms,
+                "gridder_updates_per_s": n_updates / (grid_ms * 1e-3),
+                "flop_per_update": FLOP_PER_UPDATE, "updates_per_launch": n_updates}
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            hbm_gbs = json.load(f)["hbm_gbs"]; src = "measured"
+    except (OSError, ValueError, KeyError):
+        hbm_gbs, src = 6650.0, "fallback"
+    in_bytes = wl.uvw.nbytes + wl.vis.nbytes + wl.weight.nbytes
+    roofline["binning_hbm"] = {"input_GBps": in_bytes / (bin_ms * 1e-3) / 1e9, "peak": hbm_gbs, "peak_source": src}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": args.prec, "data": "synthetic", "config": workload_config(wl, args.prec),
+           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+           "stats": stats, "multi_gpu": "replicas only" if world > 1 else "single GPU"}
+    if not args.no_cpu_baseline and world == 1:
+        out["cpu_baseline"] = cpu_baseline(wl)
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_b200(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -64,9 +64,20 @@ const char *wpg_last_error(const wpg_ctx *ctx);   /* ctx may be NULL: last error
 int  wpg_version(void);
 
 /* Tuning knobs (all have defaults): "order" 0 = auto, 1 = plane-major, 2 = tile-major sort key;
- * "segment" = max records per gridder work item; "ctas_per_sm" for the persistent gridder.
+ * "segment" = max records per gridder work item; "ctas_per_sm" for the persistent gridder;
+ * "tile" = sort tile edge in cells (0 = default); "timing" 0/1 (see wpg_phase_ms).
  * Unknown name -> WPG_EINVAL. */
 int  wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value);
+
+/* Instrumentation (bench.py's roofline and gpu_launches figures).
+ * wpg_launch_count: number of this library's own CUDA kernels the context has launched so far
+ * (memsets, copies and cuFFT's internal kernels are not counted).
+ * Option "timing" = 1 makes wpg_grid record CUDA events on the context's stream before the
+ * binning pass, between binning and gridder, and after the gridder; wpg_phase_ms then waits for
+ * the last event and returns {binning ms, gridder ms} averaged over the wpg_grid calls made
+ * since the previous wpg_phase_ms (WPG_EINVAL if there were none; at most 4096 are kept). */
+int64_t wpg_launch_count(const wpg_ctx *ctx);
+int  wpg_phase_ms(wpg_ctx *ctx, double *h_out2);
 
 /* ---- a0: W-kernel stack (setup, untimed) — PAPER.md:30 "new convolution kernel function";
  *      DESIGN.md R1-R3, R5-R7, steps K1-K6 -------------------------------------------------- */
@@ -105,10 +116,13 @@ int  wpg_grid_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const 
                     const wpg_kdesc *desc, wpg_prec prec, void *d_grid, wpg_stats *h_stats_or_null);
 /* End-to-end variant with HOST buffers: copies the inputs to device scratch owned by the
  * context (grown on demand), zero-fills a device grid, runs wpg_grid, copies the grid to
- * h_grid_out (overwritten, [N][N] c64|c128) and synchronises.  d_kernels stays on the device. */
+ * h_grid_out (overwritten, [N][N] c64|c128) and synchronises.  d_kernels stays on the device.
+ * If h_image_out_or_null is non-NULL the dirty image (wpg_dirty_image with weight_sum) is formed
+ * on the device as well and copied to it ([N][N] fp32|fp64). */
 int  wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uvw, const float *h_weight,
                    const double *h_freq, int64_t nrow, int nchan, const void *d_kernels,
-                   const wpg_kdesc *desc, wpg_prec prec, void *h_grid_out, wpg_stats *h_stats_or_null);
+                   const wpg_kdesc *desc, wpg_prec prec, void *h_grid_out, wpg_stats *h_stats_or_null,
+                   void *h_image_out_or_null, double weight_sum);
 
 /* Binning alone (step a1), for tests and profiling: fills the workspace exactly as wpg_grid
  * does and reports where things are.  Offsets are in bytes from d_workspace. */

@@ -45,6 +45,7 @@ extern "C" int wpg_create(wpg_ctx **out, int device, void *cuda_stream) {
 extern "C" void wpg_destroy(wpg_ctx *ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    for (auto &e : ctx->ev) cudaEventDestroy(e);
     if (ctx->plan) cufftDestroy(ctx->plan);
     if (ctx->d_taper) cudaFree(ctx->d_taper);
     if (ctx->d_host_scratch) cudaFree(ctx->d_host_scratch);
@@ -61,6 +62,7 @@ extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
     else if (!strcmp(name, "segment")) { if (value < 0 || value > 65535) return wpg_fail(ctx, WPG_EINVAL, "segment must be 0..65535"); ctx->opt_segment = (int)value; }
     else if (!strcmp(name, "ctas_per_sm")) { if (value < 0 || value > 32) return wpg_fail(ctx, WPG_EINVAL, "ctas_per_sm must be 0..32"); ctx->opt_ctas_per_sm = (int)value; }
     else if (!strcmp(name, "tile")) { if (value < 0 || value > WPG_MAX_S) return wpg_fail(ctx, WPG_EINVAL, "tile must be 0..64"); ctx->opt_tile = (int)value; }
+    else if (!strcmp(name, "timing")) { ctx->opt_timing = value != 0; }
     else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
     return WPG_OK;
 }
@@ -196,6 +198,39 @@ static int check_ptrs(wpg_ctx *ctx, const void *vis, const void *uvw, const void
     return WPG_OK;
 }
 
+extern "C" int64_t wpg_launch_count(const wpg_ctx *ctx) { return ctx ? ctx->n_launches : 0; }
+
+extern "C" int wpg_phase_ms(wpg_ctx *ctx, double *out) {
+    if (!ctx || !out) return WPG_EINVAL;
+    if (!ctx->ev_used) return wpg_fail(ctx, WPG_EINVAL, "no timed wpg_grid call (set option \"timing\" = 1 first)");
+    WPG_CUDA(ctx, cudaEventSynchronize(ctx->ev[3 * ctx->ev_used - 1]));
+    double a = 0.0, b = 0.0;
+    for (size_t i = 0; i < ctx->ev_used; ++i) {
+        float x = 0.f, y = 0.f;
+        WPG_CUDA(ctx, cudaEventElapsedTime(&x, ctx->ev[3 * i], ctx->ev[3 * i + 1]));
+        WPG_CUDA(ctx, cudaEventElapsedTime(&y, ctx->ev[3 * i + 1], ctx->ev[3 * i + 2]));
+        a += x; b += y;
+    }
+    out[0] = a / (double)ctx->ev_used; out[1] = b / (double)ctx->ev_used;
+    ctx->ev_used = 0;
+    return WPG_OK;
+}
+
+// Event i (0 start, 1 after binning, 2 after gridder) of the current timed call.
+static int mark(wpg_ctx *ctx, int i) {
+    if (!ctx->opt_timing) return WPG_OK;
+    if (i == 0 && ctx->ev_used >= 4096) ctx->ev_used = 0;       // pool bound: start over
+    size_t k = 3 * ctx->ev_used + (size_t)i;
+    while (ctx->ev.size() <= k) {
+        cudaEvent_t e;
+        WPG_CUDA(ctx, cudaEventCreate(&e));
+        ctx->ev.push_back(e);
+    }
+    WPG_CUDA(ctx, cudaEventRecord(ctx->ev[k], ctx->stream));
+    if (i == 2) ctx->ev_used += 1;
+    return WPG_OK;
+}
+
 static int bin_common(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
                       const double *d_freq, int64_t nrow, int nchan, const wpg_kdesc *desc, wpg_prec prec,
                       void *d_workspace, size_t workspace_bytes, PlaneTab *tab, BinParams *bp, WorkspaceLayout *ws) {
@@ -206,6 +241,7 @@ static int bin_common(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, cons
     if (!d_workspace || workspace_bytes < ws->total)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, ws->total);
     WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    if ((rc = mark(ctx, 0))) return rc;
     char *w = (char *)d_workspace;
     // counters + histogram are contiguous at the head of the workspace
     WPG_CUDA(ctx, cudaMemsetAsync(w, 0, ws->off_blocksum, ctx->stream));
@@ -240,8 +276,10 @@ extern "C" int wpg_grid(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, co
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     int rc = bin_common(ctx, d_vis, d_uvw, d_weight, d_freq, nrow, nchan, desc, prec, d_workspace, workspace_bytes, &tab, &bp, &ws);
     if (rc) return rc;
+    if ((rc = mark(ctx, 1))) return rc;
     rc = wpg_launch_grid(ctx, tab, bp, ws, prec, d_kernels, d_grid, (char *)d_workspace, desc->support_max);
     if (rc) return rc;
+    if ((rc = mark(ctx, 2))) return rc;
     if (h_stats) return read_stats(ctx, (const Counters *)((char *)d_workspace + ws.off_counters), h_stats, nullptr);
     return WPG_OK;
 }
@@ -267,7 +305,8 @@ extern "C" int wpg_grid_naive(wpg_ctx *ctx, const void *d_vis, const double *d_u
 
 extern "C" int wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uvw, const float *h_weight,
                              const double *h_freq, int64_t nrow, int nchan, const void *d_kernels,
-                             const wpg_kdesc *desc, wpg_prec prec, void *h_grid_out, wpg_stats *h_stats) {
+                             const wpg_kdesc *desc, wpg_prec prec, void *h_grid_out, wpg_stats *h_stats,
+                             void *h_image_out, double weight_sum) {
     int rc = check_ptrs(ctx, h_vis, h_uvw, h_weight, h_freq, nrow);
     if (rc) return rc;
     if (!d_kernels || !h_grid_out) return wpg_fail(ctx, WPG_EINVAL, "kernels or grid pointer is NULL");
@@ -279,7 +318,9 @@ extern "C" int wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uv
     size_t cplx = prec == WPG_F32 ? 8 : 16;
     size_t b_vis = align_up((size_t)nvis * 8), b_uvw = align_up((size_t)nrow * 24), b_wt = align_up((size_t)nvis * 4),
            b_freq = align_up((size_t)nchan * 8), b_grid = align_up((size_t)desc->grid_N * desc->grid_N * cplx);
-    size_t need = b_vis + b_uvw + b_wt + b_freq + b_grid + ws.total;
+    size_t b_img = h_image_out ? align_up(wpg_dirty_image_workspace_bytes(desc->grid_N, prec)) +
+                                     align_up((size_t)desc->grid_N * desc->grid_N * (cplx / 2)) : 0;
+    size_t need = b_vis + b_uvw + b_wt + b_freq + b_grid + std::max(ws.total, b_img);
     if (need > ctx->host_scratch_bytes) {
         WPG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         if (ctx->d_host_scratch) cudaFree(ctx->d_host_scratch);
@@ -300,7 +341,17 @@ extern "C" int wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uv
                   prec, dg, dws, ws.total, nullptr);
     if (rc) return rc;
     WPG_CUDA(ctx, cudaMemcpyAsync(h_grid_out, dg, (size_t)desc->grid_N * desc->grid_N * cplx, cudaMemcpyDeviceToHost, s));
-    if (h_stats) return read_stats(ctx, (const Counters *)(dws + ws.off_counters), h_stats, nullptr);
+    if (h_stats) {                                  // before the image step reuses the workspace
+        rc = read_stats(ctx, (const Counters *)(dws + ws.off_counters), h_stats, nullptr);
+        if (rc) return rc;
+    }
+    if (h_image_out) {
+        size_t b_fft = align_up(wpg_dirty_image_workspace_bytes(desc->grid_N, prec));
+        char *dimg = dws + b_fft;
+        rc = wpg_dirty_image(ctx, dg, desc, weight_sum, prec, dimg, dws, b_fft);
+        if (rc) return rc;
+        WPG_CUDA(ctx, cudaMemcpyAsync(h_image_out, dimg, (size_t)desc->grid_N * desc->grid_N * (cplx / 2), cudaMemcpyDeviceToHost, s));
+    }
     WPG_CUDA(ctx, cudaStreamSynchronize(s));
     return WPG_OK;
 }

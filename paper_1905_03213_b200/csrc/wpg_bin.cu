@@ -207,6 +207,7 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
             scatter_kernel<double><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_weight, key, rank, pre, hist, nvis,
                                                        (Rec<double> *)(w + ws.off_records));
     }
+    ctx->n_launches += nb ? 5 : 3;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }

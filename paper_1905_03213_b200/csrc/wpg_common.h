@@ -68,6 +68,11 @@ struct wpg_ctx {
     int opt_segment = 0;      // 0 default
     int opt_ctas_per_sm = 0;  // 0 default
     int opt_tile = 0;         // 0 = min support
+    int opt_timing = 0;       // 1: wpg_grid brackets its phases with CUDA events
+    // instrumentation
+    int64_t n_launches = 0;   // kernels of this library launched so far
+    std::vector<cudaEvent_t> ev;   // triplets: start, after binning, after gridder (pool, reused)
+    size_t ev_used = 0;            // triplets recorded since the last wpg_phase_ms
     // cuFFT plan cache
     cufftHandle plan = 0; int plan_N = 0; int plan_prec = -1;
     // taper table cache for dirty_image

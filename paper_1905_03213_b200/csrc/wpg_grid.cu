@@ -164,6 +164,7 @@ int launch_tiles(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     grid_tiles_kernel<T, RMAX, MINB><<<blocks, kGridThreads, 0, ctx->stream>>>(
         (const Rec<T> *)(w + ws.off_records), (const Item *)(w + ws.off_items),
         (const Counters *)(w + ws.off_counters), (const C *)K, (C *)grid, bp.N, nchunk);
+    ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }
@@ -196,6 +197,7 @@ int wpg_launch_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const
     else
         grid_naive_kernel<double><<<blocks, 256, 0, ctx->stream>>>((const float2 *)d_vis, d_uvw, d_weight, d_freq, tab, bp,
                                                                     (const double2 *)K, (double2 *)grid, d_c);
+    ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }

@@ -95,6 +95,7 @@ extern "C" int wpg_dirty_image(wpg_ctx *ctx, const void *d_grid, const wpg_kdesc
         if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftExecZ2Z: %s", cufft_str(r));
         correct_kernel<double2, double><<<gr, 256, 0, s>>>((const double2 *)d_workspace, (double *)d_image, ctx->d_taper, N, 1.0 / weight_sum);
     }
+    ctx->n_launches += 2;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }

@@ -206,6 +206,7 @@ static int build_tables(wpg_ctx *ctx, int S, int Q, double fov, const std::vecto
     fill_twiddles<<<dim3((Nk + 63) / 64, SQ), 64, 0, s>>>((double2 *)E.p, SQ, Nk, Q);
     dft_rows<<<dim3((SQ + 127) / 128, Nk, npl), 128, 0, s>>>((const double2 *)F.p, (const double2 *)E.p, (double2 *)G.p, Nk, SQ);
     dft_cols<<<dim3((SQ + 127) / 128, SQ, npl), 128, 0, s>>>((const double2 *)G.p, (const double2 *)E.p, (double2 *)Ct.p, Nk, SQ);
+    ctx->n_launches += 4;
     WPG_CUDA(ctx, cudaGetLastError());
     WPG_CUDA(ctx, cudaStreamSynchronize(s));      // the temporaries die with this scope
     return WPG_OK;
@@ -265,6 +266,7 @@ extern "C" int wpg_wkernel_build(wpg_ctx *ctx, const wpg_kdesc *desc, wpg_prec p
             slice_kernel<float2, float><<<gr, 256, 0, ctx->stream>>>((const double2 *)Ct.p, (float2 *)d_out, (const int *)dpo.p, S, Q, 1.0 / s_norm);
         else
             slice_kernel<double2, double><<<gr, 256, 0, ctx->stream>>>((const double2 *)Ct.p, (double2 *)d_out, (const int *)dpo.p, S, Q, 1.0 / s_norm);
+        ctx->n_launches += 1;
         WPG_CUDA(ctx, cudaGetLastError());
         WPG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     }

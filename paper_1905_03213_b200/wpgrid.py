@@ -20,7 +20,7 @@ EXPORTS = (
     "wpg_create", "wpg_destroy", "wpg_last_error", "wpg_version", "wpg_set_option", "wpg_taper",
     "wpg_ragged_support", "wpg_wkernel_elems", "wpg_wkernel_build", "wpg_grid_workspace_bytes",
     "wpg_grid", "wpg_grid_naive", "wpg_grid_host", "wpg_bin", "wpg_dirty_image_workspace_bytes",
-    "wpg_dirty_image",
+    "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms",
 )
 
 
@@ -83,12 +83,14 @@ def load():
     lib.wpg_grid.restype = cint
     lib.wpg_grid_naive.argtypes = [vp, vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, stp]
     lib.wpg_grid_naive.restype = cint
-    lib.wpg_grid_host.argtypes = [vp, vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, stp]
+    lib.wpg_grid_host.argtypes = [vp, vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, stp, vp, dbl]
     lib.wpg_grid_host.restype = cint
     lib.wpg_bin.argtypes = [vp, vp, vp, vp, vp, i64, cint, kd, cint, vp, sz, ctypes.POINTER(BinInfo), stp]
     lib.wpg_bin.restype = cint
     lib.wpg_dirty_image_workspace_bytes.argtypes = [cint, cint]; lib.wpg_dirty_image_workspace_bytes.restype = sz
     lib.wpg_dirty_image.argtypes = [vp, vp, kd, dbl, cint, vp, vp, sz]; lib.wpg_dirty_image.restype = cint
+    lib.wpg_launch_count.argtypes = [vp]; lib.wpg_launch_count.restype = i64
+    lib.wpg_phase_ms.argtypes = [vp, ctypes.POINTER(dbl)]; lib.wpg_phase_ms.restype = cint
     _lib = lib
     return lib
 
@@ -178,6 +180,15 @@ class Context:
     def set_option(self, name, value):
         self._check(self.lib.wpg_set_option(self.h, name.encode(), int(value)))
 
+    def launch_count(self):
+        return int(self.lib.wpg_launch_count(self.h))
+
+    def phase_ms(self):
+        """(binning ms, gridder ms) of the last wpg_grid call made with option "timing" = 1."""
+        out = (ctypes.c_double * 2)()
+        self._check(self.lib.wpg_phase_ms(self.h, out))
+        return float(out[0]), float(out[1])
+
     # ---- a0
     def wkernel_build(self, Nw, w_max, support, oversample, grid_N, cell, prec=F32):
         t = self.torch
@@ -242,8 +253,9 @@ class Context:
                                             ctypes.byref(st) if stats else None))
         return grid, (st.as_dict() if stats else None)
 
-    def grid_host(self, vis, uvw, weight, freq, stack, out=None, stats=False):
-        """Host numpy (or pinned torch CPU) inputs -> host grid; H2D/D2H copies happen inside the call."""
+    def grid_host(self, vis, uvw, weight, freq, stack, out=None, stats=False, image_out=None, weight_sum=0.0):
+        """Host numpy (or pinned torch CPU) inputs -> host grid (and, if image_out is given, the
+        dirty image); H2D/D2H copies happen inside the call."""
         def ptr(x):
             return x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data
         nrow, nchan = int(uvw.shape[0]), int(freq.shape[0])
@@ -253,7 +265,8 @@ class Context:
         st = Stats()
         self._check(self.lib.wpg_grid_host(self.h, ptr(vis), ptr(uvw), ptr(weight), ptr(freq), nrow, nchan,
                                            stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec,
-                                           ptr(out), ctypes.byref(st) if stats else None))
+                                           ptr(out), ctypes.byref(st) if stats else None,
+                                           ptr(image_out) if image_out is not None else None, float(weight_sum)))
         return out, (st.as_dict() if stats else None)
 
     def bin(self, vis, uvw, weight, freq, stack, workspace=None):
