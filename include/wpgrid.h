@@ -18,7 +18,7 @@
  *     cell (N/2, N/2) is u = v = 0.
  *   - Kernel stack layout: K[p][ov][ou][iv][iu], innermost iu; plane p starts at
  *     element plane_offset[p] and holds Q*Q*S_p*S_p complex coefficients.
- *   - Limits: grid_N <= 8192, S_p <= 64, Nw <= 256, S_p * Q even.
+ *   - Limits: grid_N <= 8192, S_p <= 32, at most 32 distinct S_p, Nw <= 256, S_p * Q even.
  */
 #ifndef WPGRID_H
 #define WPGRID_H
@@ -63,9 +63,10 @@ void wpg_destroy(wpg_ctx *ctx);
 const char *wpg_last_error(const wpg_ctx *ctx);   /* ctx may be NULL: last error of a failed wpg_create */
 int  wpg_version(void);
 
-/* Tuning knobs (all have defaults): "order" 0 = auto, 1 = plane-major, 2 = tile-major sort key;
- * "segment" = max records per gridder work item; "ctas_per_sm" for the persistent gridder;
- * "tile" = sort tile edge in cells (0 = default); "timing" 0/1 (see wpg_phase_ms).
+/* Tuning knobs (all have defaults, 0 = default): "segment" = records per gridder work item;
+ * "ctas_per_sm" = gridder CTAs per SM; "key_bits" = log2 cap of the binning sort-key space
+ * (default 26: the key is (support class, j0v, j0u) at full resolution unless that exceeds the cap,
+ * then low bits of j0u are dropped); "timing" 0/1 (see wpg_phase_ms).
  * Unknown name -> WPG_EINVAL. */
 int  wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value);
 
@@ -128,15 +129,13 @@ int  wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uvw, const f
  * does and reports where things are.  Offsets are in bytes from d_workspace. */
 typedef struct {
     int64_t n_records;       /* valid visibilities = sorted records */
-    int64_t n_keys;          /* number of sort keys */
-    int64_t n_items;         /* gridder work items */
-    int32_t tile;            /* tile edge in cells */
-    int32_t ntile;           /* tiles per axis */
-    int32_t order;           /* 1 plane-major, 2 tile-major */
+    int64_t n_keys;          /* number of sort keys = n_classes * keys_per_class */
+    int32_t n_classes;       /* distinct supports; key = (class * N + j0v) * ceil(N / 2^u_shift) + (j0u >> u_shift) */
+    int32_t u_shift;
     int32_t record_bytes;    /* 16 (fp32) or 24 (fp64) */
-    int64_t off_records;     /* records sorted by key: {re, im, pos, koff} */
+    int32_t keys_per_class;
+    int64_t off_records;     /* records sorted by key: {re, im, pos = j0u | j0v << 16, koff} */
     int64_t off_bucket_start;/* uint32 [n_keys + 1] */
-    int64_t off_items;       /* work items, 16 bytes each */
 } wpg_bin_info;
 int  wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
              const double *d_freq, int64_t nrow, int nchan, const wpg_kdesc *desc, wpg_prec prec,

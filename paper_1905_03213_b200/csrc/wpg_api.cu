@@ -58,10 +58,9 @@ extern "C" const char *wpg_last_error(const wpg_ctx *ctx) {
 
 extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
     if (!ctx || !name) return WPG_EINVAL;
-    if (!strcmp(name, "order")) { if (value < 0 || value > 2) return wpg_fail(ctx, WPG_EINVAL, "order must be 0..2"); ctx->opt_order = (int)value; }
-    else if (!strcmp(name, "segment")) { if (value < 0 || value > 65535) return wpg_fail(ctx, WPG_EINVAL, "segment must be 0..65535"); ctx->opt_segment = (int)value; }
+    if (!strcmp(name, "segment")) { if (value < 0 || value > (1 << 20)) return wpg_fail(ctx, WPG_EINVAL, "segment must be 0..2^20"); ctx->opt_segment = (int)value; }
     else if (!strcmp(name, "ctas_per_sm")) { if (value < 0 || value > 32) return wpg_fail(ctx, WPG_EINVAL, "ctas_per_sm must be 0..32"); ctx->opt_ctas_per_sm = (int)value; }
-    else if (!strcmp(name, "tile")) { if (value < 0 || value > WPG_MAX_S) return wpg_fail(ctx, WPG_EINVAL, "tile must be 0..64"); ctx->opt_tile = (int)value; }
+    else if (!strcmp(name, "key_bits")) { if (value != 0 && (value < 8 || value > 28)) return wpg_fail(ctx, WPG_EINVAL, "key_bits must be 0 or 8..28"); ctx->opt_key_bits = (int)value; }
     else if (!strcmp(name, "timing")) { ctx->opt_timing = value != 0; }
     else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
     return WPG_OK;
@@ -104,7 +103,6 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     int64_t nvis = nrow * nchan;
     if (nvis >= ((int64_t)1 << 32) - 2) return wpg_fail(ctx, WPG_EINVAL, "nrow*nchan = %lld exceeds 2^32 - 2 per call; chunk the input", (long long)nvis);
     memset(tab, 0, sizeof *tab);
-    int Smin = WPG_MAX_S + 1, Smax = 0;
     int64_t off = 0;
     std::vector<int> distinct;
     for (int p = 0; p < d->Nw; ++p) {
@@ -112,11 +110,15 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
         tab->off[p] = (int32_t)off;
         tab->S[p] = (uint8_t)S;
         off += (int64_t)d->oversample * d->oversample * S * S;
-        Smin = std::min(Smin, S); Smax = std::max(Smax, S);
         if (std::find(distinct.begin(), distinct.end(), S) == distinct.end()) distinct.push_back(S);
     }
     tab->off[d->Nw] = (int32_t)off;
     std::sort(distinct.begin(), distinct.end());
+    if ((int)distinct.size() > WPG_MAX_CLS)
+        return wpg_fail(ctx, WPG_EINVAL, "%d distinct supports, limit %d", (int)distinct.size(), WPG_MAX_CLS);
+    for (int p = 0; p < d->Nw; ++p)
+        tab->cls[p] = (uint8_t)(std::find(distinct.begin(), distinct.end(), (int)tab->S[p]) - distinct.begin());
+    for (size_t c = 0; c < distinct.size(); ++c) tab->clsS[c] = (uint8_t)distinct[c];
 
     memset(bp, 0, sizeof *bp);
     bp->nrow = nrow; bp->nchan = nchan;
@@ -126,45 +128,30 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     double fov = (double)d->grid_N * d->cell;
     bp->du = 1.0 / fov;
     bp->halfN = (double)(d->grid_N / 2);
-    bp->tile = ctx->opt_tile ? std::min(ctx->opt_tile, Smin) : Smin;
-    bp->ntile = (d->grid_N + bp->tile - 1) / bp->tile;
-    bp->segment = ctx->opt_segment ? ctx->opt_segment : 512;
-    int64_t ntile2 = (int64_t)bp->ntile * bp->ntile;
-    int order = ctx->opt_order;
-    if (order == 0) {
-        // expected records per (plane, tile) bucket if ~40% of the tiles are occupied
-        double per_bucket = (double)nvis / ((double)d->Nw * (double)ntile2 * 0.4);
-        order = per_bucket >= 12.0 ? 1 : 2;
-    }
-    if (order == 1 && (int64_t)d->Nw * ntile2 > ((int64_t)1 << 27)) order = 2;
-    bp->order = order;
-    if (order == 1) {
-        bp->ncls = d->Nw;
-        for (int p = 0; p < d->Nw; ++p) { tab->cls[p] = (uint16_t)p; tab->clsS[p] = tab->S[p]; }
-    } else {
-        bp->ncls = (int)distinct.size();
-        for (int p = 0; p < d->Nw; ++p)
-            tab->cls[p] = (uint16_t)(std::find(distinct.begin(), distinct.end(), (int)tab->S[p]) - distinct.begin());
-        for (size_t c = 0; c < distinct.size(); ++c) tab->clsS[c] = (uint8_t)distinct[c];
-    }
-    int64_t nkeys = (int64_t)bp->ncls * ntile2;
-    if (nkeys > ((int64_t)1 << 28)) return wpg_fail(ctx, WPG_EINVAL, "sort key space %lld too large", (long long)nkeys);
+    bp->ncls = (int)distinct.size();
+    // sort key = (class, j0v, j0u >> ushift): full resolution unless the key space would exceed 2^key_bits
+    const int64_t cap = (int64_t)1 << (ctx->opt_key_bits ? ctx->opt_key_bits : 26);
+    int ushift = 0;
+    while ((int64_t)bp->ncls * d->grid_N * (((int64_t)d->grid_N + (1 << ushift) - 1) >> ushift) > cap && ushift < 13) ++ushift;
+    bp->ushift = ushift;
+    bp->nug = (d->grid_N + (1 << ushift) - 1) >> ushift;
+    bp->keys_per_class = (uint32_t)((int64_t)d->grid_N * bp->nug);
+    int64_t nkeys = (int64_t)bp->ncls * bp->keys_per_class;
+    if (nkeys > ((int64_t)1 << 30)) return wpg_fail(ctx, WPG_EINVAL, "sort key space %lld too large", (long long)nkeys);
     bp->nkeys = (uint32_t)nkeys;
 
     memset(ws, 0, sizeof *ws);
     ws->nkeys = (uint32_t)nkeys;
     ws->nblocks_scan = (uint32_t)((nkeys + 1 + 4095) / 4096);
-    ws->max_items = std::min<int64_t>(nvis, nkeys) + nvis / bp->segment + 1;
     size_t rec = prec == WPG_F32 ? sizeof(Rec<float>) : sizeof(Rec<double>);
     size_t o = 0;
     ws->off_counters = o; o += align_up(sizeof(Counters));
-    ws->off_hist = o;     o += align_up((size_t)(nkeys + 1) * 4);
-    ws->off_blocksum = o; o += align_up((size_t)ws->nblocks_scan * 8 + 8);
+    ws->off_hist = o;     o += align_up((size_t)(nkeys + 4) * 4);
+    ws->off_blocksum = o; o += align_up((size_t)ws->nblocks_scan * 4 + 8);
     ws->off_key = o;      o += align_up((size_t)nvis * 4);
     ws->off_rank = o;     o += align_up((size_t)nvis * 4);
     ws->off_pre = o;      o += align_up((size_t)nvis * 8);
     ws->off_records = o;  o += align_up((size_t)nvis * rec);
-    ws->off_items = o;    o += align_up((size_t)ws->max_items * sizeof(Item));
     ws->total = o;
     return WPG_OK;
 }
@@ -173,7 +160,7 @@ extern "C" size_t wpg_grid_workspace_bytes(const wpg_ctx *ctx, int64_t nrow, int
                                            wpg_prec prec) {
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     wpg_ctx tmp;
-    if (ctx) { tmp.opt_order = ctx->opt_order; tmp.opt_segment = ctx->opt_segment; tmp.opt_tile = ctx->opt_tile; }
+    if (ctx) { tmp.opt_segment = ctx->opt_segment; tmp.opt_key_bits = ctx->opt_key_bits; }
     if (wpg_make_plan(&tmp, desc, nrow, nchan, prec, &tab, &bp, &ws)) return 0;
     return ws.total;
 }
@@ -258,11 +245,10 @@ extern "C" int wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, con
     rc = read_stats(ctx, (const Counters *)((char *)d_workspace + ws.off_counters), h_stats, &h);
     if (rc) return rc;
     if (info) {
-        info->n_records = h.n_records; info->n_keys = ws.nkeys; info->n_items = h.n_items;
-        info->tile = bp.tile; info->ntile = bp.ntile; info->order = bp.order;
-        info->record_bytes = prec == WPG_F32 ? 16 : 24;
+        info->n_records = h.n_records; info->n_keys = ws.nkeys;
+        info->n_classes = bp.ncls; info->u_shift = bp.ushift;
+        info->record_bytes = prec == WPG_F32 ? 16 : 24; info->keys_per_class = (int32_t)bp.keys_per_class;
         info->off_records = (int64_t)ws.off_records; info->off_bucket_start = (int64_t)ws.off_hist;
-        info->off_items = (int64_t)ws.off_items;
     }
     return WPG_OK;
 }
@@ -277,7 +263,7 @@ extern "C" int wpg_grid(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, co
     int rc = bin_common(ctx, d_vis, d_uvw, d_weight, d_freq, nrow, nchan, desc, prec, d_workspace, workspace_bytes, &tab, &bp, &ws);
     if (rc) return rc;
     if ((rc = mark(ctx, 1))) return rc;
-    rc = wpg_launch_grid(ctx, tab, bp, ws, prec, d_kernels, d_grid, (char *)d_workspace, desc->support_max);
+    rc = wpg_launch_grid(ctx, tab, bp, ws, prec, d_kernels, d_grid, (char *)d_workspace);
     if (rc) return rc;
     if ((rc = mark(ctx, 2))) return rc;
     if (h_stats) return read_stats(ctx, (const Counters *)((char *)d_workspace + ws.off_counters), h_stats, nullptr);

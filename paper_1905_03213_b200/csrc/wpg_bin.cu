@@ -1,9 +1,11 @@
 // Step a1 — visibility binning: uvw -> (plane, window start, sub-cell offsets), sort key,
-// histogram, exclusive prefix scan, scatter into key-sorted 16/24-byte records, work-item list.
+// histogram, exclusive prefix scan, scatter into key-sorted 16/24-byte records.
 //
 // The paper's analogue is the re-order of PAPER.md:62-78: count array C, exclusive prefix sum
-// Eq. (2), scatter — keyed there by baseline (Eq. 1), here by (w-plane | support class, uv tile)
-// so that the gridder (wpg_grid.cu) can keep a tile's cells in registers.
+// Eq. (2), scatter — keyed there by baseline (Eq. 1) so that consecutive samples of a baseline hit
+// the same grid point.  Here the key is (support class, window start j0v, j0u), i.e.
+// the visibilities are ordered by the grid point they hit, whatever baseline they came from: runs
+// of equal window start are what the gridder (wpg_grid.cu) accumulates in registers.
 #include "wpg_common.h"
 
 namespace {
@@ -39,12 +41,10 @@ bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weigh
                 c_oob = 1;
             } else {
                 c_grid = 1; c_clamp = r.clamped; c_upd = r.S * r.S;
-                unsigned tid = (unsigned)(r.j0v / P.tile) * P.ntile + (unsigned)(r.j0u / P.tile);
-                unsigned cls = T.cls[r.p];
-                key = P.order == 1 ? cls * (unsigned)(P.ntile * P.ntile) + tid : tid * (unsigned)P.ncls + cls;
+                key = (unsigned)T.cls[r.p] * P.keys_per_class + (unsigned)r.j0v * (unsigned)P.nug +
+                      ((unsigned)r.j0u >> P.ushift);
                 rank_out[i] = atomicAdd(&hist[key], 1u);
-                pre_out[i] = make_uint2((unsigned)r.j0u | ((unsigned)r.j0v << 13) | ((unsigned)(r.S - 1) << 26),
-                                        wpg_koff(r, P, T));
+                pre_out[i] = make_uint2((unsigned)r.j0u | ((unsigned)r.j0v << 16), wpg_koff(r, P, T));
             }
         }
         key_out[i] = key;
@@ -56,107 +56,83 @@ bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weigh
     warp_count(&ctr->n_updates, c_upd);
 }
 
-__device__ __forceinline__ unsigned nseg_of(unsigned cnt, unsigned seg) { return (cnt + seg - 1) / seg; }
-
-// Block-wide inclusive scan of one uint2 per thread (1024 threads); returns the inclusive value,
-// *total receives the block total.
-__device__ __forceinline__ uint2 block_scan_incl(uint2 v, uint2 *total) {
-    __shared__ uint2 wsum[32];
+// Block-wide inclusive scan of one unsigned per thread (1024 threads); returns the inclusive
+// value, *total receives the block total.
+__device__ __forceinline__ unsigned block_scan_incl(unsigned v, unsigned *total) {
+    __shared__ unsigned wsum[32];
     int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
-        unsigned a = __shfl_up_sync(0xffffffffu, v.x, d), b = __shfl_up_sync(0xffffffffu, v.y, d);
-        if (lane >= d) { v.x += a; v.y += b; }
+        unsigned a = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += a;
     }
     if (lane == 31) wsum[wid] = v;
     __syncthreads();
     if (wid == 0) {
-        uint2 w = wsum[lane];
+        unsigned w = wsum[lane];
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            unsigned a = __shfl_up_sync(0xffffffffu, w.x, d), b = __shfl_up_sync(0xffffffffu, w.y, d);
-            if (lane >= d) { w.x += a; w.y += b; }
+            unsigned a = __shfl_up_sync(0xffffffffu, w, d);
+            if (lane >= d) w += a;
         }
         wsum[lane] = w;
     }
     __syncthreads();
-    if (wid > 0) { v.x += wsum[wid - 1].x; v.y += wsum[wid - 1].y; }
+    if (wid > 0) v += wsum[wid - 1];
     *total = wsum[31];
     __syncthreads();
     return v;
 }
 
-// Scan phase A: per-block totals of (count, number of work items).
+// Scan phase A: per-block totals of the counts.
 __global__ void __launch_bounds__(1024)
-scan_reduce_kernel(const unsigned *__restrict__ hist, unsigned nkeys, unsigned seg, uint2 *__restrict__ blocksum) {
+scan_reduce_kernel(const unsigned *__restrict__ hist, unsigned nkeys, unsigned *__restrict__ blocksum) {
     unsigned k0 = blockIdx.x * kScanBlock + threadIdx.x * 4;
-    uint2 v = make_uint2(0, 0);
+    unsigned v = 0;
+    if (k0 + 3 < nkeys) {
+        uint4 q = *reinterpret_cast<const uint4 *>(hist + k0);
+        v = q.x + q.y + q.z + q.w;
+    } else {
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        unsigned k = k0 + j;
-        unsigned c = k < nkeys ? hist[k] : 0;
-        v.x += c; v.y += nseg_of(c, seg);
+        for (int j = 0; j < 4; ++j) v += (k0 + j < nkeys) ? hist[k0 + j] : 0;
     }
-    uint2 tot;
+    unsigned tot;
     block_scan_incl(v, &tot);
     if (threadIdx.x == 0) blocksum[blockIdx.x] = tot;
 }
 
-// Scan phase B: exclusive scan of the block totals (single block), totals to the counters.
+// Scan phase B: exclusive scan of the block totals (single block), total to the counters.
 __global__ void __launch_bounds__(1024)
-scan_blocksums_kernel(uint2 *__restrict__ blocksum, unsigned nblocks, Counters *__restrict__ ctr) {
-    uint2 carry = make_uint2(0, 0);
+scan_blocksums_kernel(unsigned *__restrict__ blocksum, unsigned nblocks, Counters *__restrict__ ctr) {
+    unsigned carry = 0;
     for (unsigned b0 = 0; b0 < nblocks; b0 += 1024) {
         unsigned b = b0 + threadIdx.x;
-        uint2 v = b < nblocks ? blocksum[b] : make_uint2(0, 0);
-        uint2 tot;
-        uint2 inc = block_scan_incl(v, &tot);
-        if (b < nblocks) blocksum[b] = make_uint2(carry.x + inc.x - v.x, carry.y + inc.y - v.y);
-        carry.x += tot.x; carry.y += tot.y;
+        unsigned v = b < nblocks ? blocksum[b] : 0;
+        unsigned tot;
+        unsigned inc = block_scan_incl(v, &tot);
+        if (b < nblocks) blocksum[b] = carry + inc - v;
+        carry += tot;
     }
-    if (threadIdx.x == 0) { ctr->n_records = carry.x; ctr->n_items = carry.y; }
+    if (threadIdx.x == 0) ctr->n_records = carry;
 }
 
-// Scan phase C: bucket_start (in place over the histogram) and the work items of each key.
+// Scan phase C: bucket_start, in place over the histogram (bucket_start[nkeys] = total).
 __global__ void __launch_bounds__(1024)
-scan_apply_kernel(unsigned *__restrict__ hist, unsigned nkeys, const uint2 *__restrict__ blocksum,
-                  const __grid_constant__ PlaneTab T, const __grid_constant__ BinParams P,
-                  Item *__restrict__ items) {
+scan_apply_kernel(unsigned *__restrict__ hist, unsigned nkeys, const unsigned *__restrict__ blocksum) {
     unsigned k0 = blockIdx.x * kScanBlock + threadIdx.x * 4;
     unsigned c[4];
-    uint2 v = make_uint2(0, 0);
+    unsigned v = 0;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        unsigned k = k0 + j;
-        c[j] = k < nkeys ? hist[k] : 0;
-        v.x += c[j]; v.y += nseg_of(c[j], P.segment);
+        c[j] = (k0 + j < nkeys) ? hist[k0 + j] : 0;
+        v += c[j];
     }
-    uint2 tot;
-    uint2 inc = block_scan_incl(v, &tot);
-    uint2 off = blocksum[blockIdx.x];
-    unsigned start = off.x + inc.x - v.x, istart = off.y + inc.y - v.y;
-    unsigned ntile2 = (unsigned)(P.ntile * P.ntile);
+    unsigned tot;
+    unsigned inc = block_scan_incl(v, &tot);
+    unsigned start = blocksum[blockIdx.x] + inc - v;
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        unsigned k = k0 + j;
-        if (k <= nkeys) hist[k] = start;             // hist[nkeys] = total
-        if (k < nkeys && c[j]) {
-            unsigned cls, tid;
-            if (P.order == 1) { cls = k / ntile2; tid = k - cls * ntile2; }
-            else { tid = k / (unsigned)P.ncls; cls = k - tid * (unsigned)P.ncls; }
-            unsigned tv = tid / (unsigned)P.ntile, tu = tid - tv * (unsigned)P.ntile;
-            unsigned ns = nseg_of(c[j], P.segment);
-            unsigned len = (c[j] + ns - 1) / ns;
-            for (unsigned s = 0; s < ns; ++s) {
-                Item it;
-                it.rec_begin = start + s * len;
-                it.count = min(len, c[j] - s * len);
-                it.origin = (tu * (unsigned)P.tile) | ((tv * (unsigned)P.tile) << 16);
-                it.S = T.clsS[cls];
-                items[istart + s] = it;
-            }
-            istart += ns;
-        }
+        if (k0 + j <= nkeys) hist[k0 + j] = start;
         start += c[j];
     }
 }
@@ -189,16 +165,15 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
     long long nvis = bp.nrow * bp.nchan;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     unsigned *hist = (unsigned *)(w + ws.off_hist);
-    uint2 *blocksum = (uint2 *)(w + ws.off_blocksum);
+    unsigned *blocksum = (unsigned *)(w + ws.off_blocksum);
     unsigned *key = (unsigned *)(w + ws.off_key), *rank = (unsigned *)(w + ws.off_rank);
     uint2 *pre = (uint2 *)(w + ws.off_pre);
-    Item *items = (Item *)(w + ws.off_items);
     cudaStream_t s = ctx->stream;
     unsigned nb = (unsigned)((nvis + 255) / 256);
     if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, d_freq, tab, bp, ctr, hist, key, rank, pre);
-    scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, (unsigned)bp.segment, blocksum);
+    scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
-    scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum, tab, bp, items);
+    scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     if (nb) {
         if (prec == WPG_F32)
             scatter_kernel<float><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_weight, key, rank, pre, hist, nvis,

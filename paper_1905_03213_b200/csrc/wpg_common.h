@@ -11,16 +11,17 @@
 #define WPG_C0 299792458.0
 #define WPG_MAX_NW 256
 #define WPG_MAX_N 8192
-#define WPG_MAX_S 64
+#define WPG_MAX_S 32
+#define WPG_MAX_CLS 32
 #define WPG_NO_KEY 0xFFFFFFFFu
 
 // Per-plane table, passed to kernels by value (__grid_constant__): element offset of the plane in
-// the stack, its full support S_p and its sort class.
+// the stack, its full support S_p and its sort class (planes of equal support share a class).
 struct PlaneTab {
     int32_t off[WPG_MAX_NW + 1];
-    uint16_t cls[WPG_MAX_NW];
     uint8_t S[WPG_MAX_NW];
-    uint8_t clsS[WPG_MAX_NW];      // support of each sort class
+    uint8_t cls[WPG_MAX_NW];
+    uint8_t clsS[WPG_MAX_CLS];     // support of each sort class, ascending
 };
 
 // Everything the position math (G1-G3) and the sort key need.
@@ -29,32 +30,29 @@ struct BinParams {
     int nchan;
     int N, Q, Nw;
     double w_max, dw, du, halfN;   // dw = 2 w_max / Nw, du = 1/(N cell), halfN = N/2
-    int tile, ntile;               // tile edge (cells), tiles per axis
-    int order;                     // 1 plane(class)-major, 2 tile-major
-    int ncls;                      // number of sort classes
-    int segment;                   // max records per work item
-    uint32_t nkeys;
+    int ushift;                    // the key drops this many low bits of j0u (0 unless the key space is capped)
+    int nug;                       // ceil(N / 2^ushift): key columns per grid row
+    int ncls;                      // number of sort classes (distinct supports)
+    uint32_t keys_per_class;       // N * nug
+    uint32_t nkeys;                // ncls * keys_per_class
 };
 
-// Sorted record.  pos = j0u | j0v << 13 | (S-1) << 26; koff = element offset of the
-// S x S coefficient slice K[p][ov][ou] inside the stack.
+// Sorted record.  pos = j0u | j0v << 16 (window start, cells); koff = element offset
+// of the S x S coefficient slice K[p][ov][ou] inside the stack.
 template <typename T> struct Rec { T re, im; uint32_t pos, koff; };
 static_assert(sizeof(Rec<float>) == 16, "fp32 record is 16 B");
 static_assert(sizeof(Rec<double>) == 24, "fp64 record is 24 B");
 
-// Work item: a run of records of one sort key (one tile, one support).
-struct Item { uint32_t rec_begin, count, origin /* u0 | v0 << 16 */, S; };
-
 // Device counters block at the head of the workspace.
 struct Counters {
     unsigned long long n_gridded, n_skipped_oob, n_skipped_zero_weight, n_clamped_w, n_updates;
-    unsigned int n_items, n_records, pad0, pad1;
+    unsigned int n_records, pad0, pad1, pad2;
+    unsigned int cursor[WPG_MAX_CLS];   // work-item cursors of the gridder launches (one per sort class)
 };
 
 struct WorkspaceLayout {
-    size_t off_counters, off_key, off_rank, off_pre, off_records, off_hist, off_blocksum, off_items;
+    size_t off_counters, off_key, off_rank, off_pre, off_records, off_hist, off_blocksum;
     size_t total;
-    int64_t max_items;
     uint32_t nkeys, nblocks_scan;
 };
 
@@ -64,10 +62,9 @@ struct wpg_ctx {
     int sm_count = 148;
     std::string err;
     // options
-    int opt_order = 0;        // 0 auto
-    int opt_segment = 0;      // 0 default
-    int opt_ctas_per_sm = 0;  // 0 default
-    int opt_tile = 0;         // 0 = min support
+    int opt_segment = 0;      // records per gridder work item, 0 = default
+    int opt_ctas_per_sm = 0;  // gridder CTAs per SM, 0 = default
+    int opt_key_bits = 0;     // cap of the sort key space (log2), 0 = default 26
     int opt_timing = 0;       // 1: wpg_grid brackets its phases with CUDA events
     // instrumentation
     int64_t n_launches = 0;   // kernels of this library launched so far
@@ -101,7 +98,7 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
                    const double *d_freq, const PlaneTab &tab, const BinParams &bp,
                    const WorkspaceLayout &ws, wpg_prec prec, char *d_ws);
 int wpg_launch_grid(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws,
-                    wpg_prec prec, const void *d_kernels, void *d_grid, char *d_ws, int maxS);
+                    wpg_prec prec, const void *d_kernels, void *d_grid, char *d_ws);
 int wpg_launch_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
                      const double *d_freq, const PlaneTab &tab, const BinParams &bp, wpg_prec prec,
                      const void *d_kernels, void *d_grid, Counters *d_counters);

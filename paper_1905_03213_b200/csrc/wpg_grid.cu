@@ -4,13 +4,16 @@
 //  * grid_naive_kernel — one global reduction per update straight from the raw inputs (the design
 //    whose ceiling is the atomic roofline; "write access to the global memory ... in an
 //    atomic manner").  Independent of the binning pass, so it also cross-checks it.
-//  * grid_tiles_kernel — the paper's register accumulator ("accumulated and
-//    buffered in a register ... written into the global memory when the processing moves on"),
-//    re-cut for key-sorted records: a warp walks the records of one work item (one uv tile, one
-//    support S); lane <-> support-cell residue (b, a) = cell position modulo S relative to the tile
-//    origin.  Because the window start stays inside a tile of edge <= S, each residue can only land
-//    on 2 x 2 grid cells, so 4 register accumulators per residue hold the whole item and the global
-//    reductions (red.global.add.v2.f32 / .f64) happen once per item instead of once per update.
+//  * grid_runs_kernel — the paper's register accumulator (one thread per support
+//    cell; contributions "accumulated and buffered in a register" while consecutive samples hit the
+//    same grid point, "written into the global memory when the processing moves on"), fed with the
+//    position-sorted records of wpg_bin.cu instead of per-baseline time series.  A warp walks a
+//    fixed-length segment of the sorted records; lane-slot <-> support-cell residue (b, a): the one
+//    cell of the S x S window whose grid coordinates are congruent to (b, a) modulo S.  While the
+//    window start does not change the cell and the coefficient offset of every lane stay put, so a
+//    run of visibilities costs one coefficient load and two packed FMAs per update; when the window
+//    moves, only the lanes whose cell changed flush (red.global.add.v2.f32 / .f64).
+//    Coefficients are read through L1 from the L2-resident stack, one record ahead of their use.
 #include "wpg_common.h"
 
 namespace {
@@ -19,12 +22,30 @@ template <typename T> struct Cplx;
 template <> struct Cplx<float> { using type = float2; };
 template <> struct Cplx<double> { using type = double2; };
 
-__device__ __forceinline__ void red_add(float2 *addr, float re, float im) {
-    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(re), "f"(im) : "memory");
+__device__ __forceinline__ void red_add(float2 *addr, float2 v) {
+    asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(v.x), "f"(v.y) : "memory");
 }
-__device__ __forceinline__ void red_add(double2 *addr, double re, double im) {
-    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&addr->x), "d"(re) : "memory");
-    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&addr->y), "d"(im) : "memory");
+__device__ __forceinline__ void red_add(double2 *addr, double2 v) {
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&addr->x), "d"(v.x) : "memory");
+    asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&addr->y), "d"(v.y) : "memory");
+}
+
+// acc += (re + i im) * c
+__device__ __forceinline__ void cmac(float2 &acc, float re, float im, float2 c) {
+    // two packed FMAs (FFMA2): (acc.x, acc.y) += c.x * (re, im);  += c.y * (-im, re)
+    unsigned long long A, V1, V2, CX, CY;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(A) : "f"(acc.x), "f"(acc.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(V1) : "f"(re), "f"(im));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(V2) : "f"(-im), "f"(re));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(CX) : "f"(c.x));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(CY) : "f"(c.y));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(A) : "l"(V1), "l"(CX));
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(A) : "l"(V2), "l"(CY));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(acc.x), "=f"(acc.y) : "l"(A));
+}
+__device__ __forceinline__ void cmac(double2 &acc, double re, double im, double2 c) {
+    acc.x = fma(re, c.x, acc.x); acc.x = fma(-im, c.y, acc.x);
+    acc.y = fma(re, c.y, acc.y); acc.y = fma(im, c.x, acc.y);
 }
 
 // ------------------------------------------------------------------------------------ naive
@@ -56,7 +77,9 @@ grid_naive_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw
         for (int c = lane; c < S2; c += 32) {
             int iv = c / S, iu = c - iv * S;
             C k = Ks[c];
-            red_add(grid + (long long)(r.j0v + iv) * P.N + (r.j0u + iu), re * k.x - im * k.y, re * k.y + im * k.x);
+            C p;
+            p.x = re * k.x - im * k.y; p.y = re * k.y + im * k.x;
+            red_add(grid + (long long)(r.j0v + iv) * P.N + (r.j0u + iu), p);
         }
     }
     if (lane == 0) {
@@ -68,122 +91,207 @@ grid_naive_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw
     }
 }
 
-// ------------------------------------------------------------------------------------ tiled
-template <typename T> __device__ __forceinline__ Rec<T> load_rec(const Rec<T> *p);
-template <> __device__ __forceinline__ Rec<float> load_rec<float>(const Rec<float> *p) {
-    float4 q = __ldg(reinterpret_cast<const float4 *>(p));
-    Rec<float> r;
-    r.re = q.x; r.im = q.y; r.pos = __float_as_uint(q.z); r.koff = __float_as_uint(q.w);
-    return r;
-}
-template <> __device__ __forceinline__ Rec<double> load_rec<double>(const Rec<double> *p) {
-    Rec<double> r;                                              // 24-byte records: 8-byte aligned only
-    r.re = __ldg(&p->re); r.im = __ldg(&p->im);
-    uint2 t = __ldg(reinterpret_cast<const uint2 *>(&p->pos));
-    r.pos = t.x; r.koff = t.y;
-    return r;
-}
+// ------------------------------------------------------------------------------------ runs
+// One lane's copy of a batch of 32 sorted records, handed out one by one with shuffles.
+template <typename T> struct RecBatch;
+template <> struct RecBatch<float> {
+    uint4 q;
+    __device__ __forceinline__ void load(const Rec<float> *p, bool ok) {
+        q = ok ? __ldg(reinterpret_cast<const uint4 *>(p)) : make_uint4(0, 0, 0, 0);
+    }
+    __device__ __forceinline__ void get(int j, float &re, float &im, unsigned &pos, unsigned &koff) const {
+        re = __uint_as_float(__shfl_sync(0xffffffffu, q.x, j));
+        im = __uint_as_float(__shfl_sync(0xffffffffu, q.y, j));
+        pos = __shfl_sync(0xffffffffu, q.z, j);
+        koff = __shfl_sync(0xffffffffu, q.w, j);
+    }
+};
+template <> struct RecBatch<double> {
+    double re_, im_; uint2 t;                                     // 24-byte records: 8-byte aligned only
+    __device__ __forceinline__ void load(const Rec<double> *p, bool ok) {
+        re_ = ok ? __ldg(&p->re) : 0.0; im_ = ok ? __ldg(&p->im) : 0.0;
+        t = ok ? __ldg(reinterpret_cast<const uint2 *>(&p->pos)) : make_uint2(0, 0);
+    }
+    __device__ __forceinline__ void get(int j, double &re, double &im, unsigned &pos, unsigned &koff) const {
+        re = __shfl_sync(0xffffffffu, re_, j);
+        im = __shfl_sync(0xffffffffu, im_, j);
+        pos = __shfl_sync(0xffffffffu, t.x, j);
+        koff = __shfl_sync(0xffffffffu, t.y, j);
+    }
+};
 
-constexpr int kGridThreads = 256;
+constexpr int kRunThreads = 256;
 
-template <typename T, int RMAX, int MINB>
-__global__ void __launch_bounds__(kGridThreads, MINB)
-grid_tiles_kernel(const Rec<T> *__restrict__ rec, const Item *__restrict__ items,
-                  const Counters *__restrict__ ctr, const typename Cplx<T>::type *__restrict__ K,
-                  typename Cplx<T>::type *__restrict__ grid, int N, int nchunk) {
+// SCT: compile-time support (a power of two) or 0 = S_rt.  NSLOT >= ceil(S^2 / 32).
+template <typename T, int SCT, int NSLOT, int MINB>
+__global__ void __launch_bounds__(kRunThreads, MINB)
+grid_runs_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
+                 unsigned key_lo, unsigned key_hi, int S_rt, unsigned *__restrict__ cursor,
+                 const typename Cplx<T>::type *__restrict__ K, typename Cplx<T>::type *__restrict__ grid,
+                 int N, unsigned seg) {
     using C = typename Cplx<T>::type;
+    constexpr bool PIPE = NSLOT <= 8;         // coefficients of record i+1 are fetched while record i is added
+    const int S = SCT ? SCT : S_rt;
+    const int S2 = S * S;
     const int lane = threadIdx.x & 31;
-    const unsigned nwarp = (gridDim.x * blockDim.x) >> 5;
-    const unsigned long long nunits = (unsigned long long)ctr->n_items * (unsigned)nchunk;
-    for (unsigned long long unit = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; unit < nunits; unit += nwarp) {
-        const unsigned item = (unsigned)(unit / (unsigned)nchunk);
-        const int chunk = (int)(unit - (unsigned long long)item * (unsigned)nchunk);
-        const uint4 itq = __ldg(reinterpret_cast<const uint4 *>(items + item));
-        const int S = (int)itq.w, S2 = S * S;
-        const int r0 = chunk * 32 * RMAX;
-        if (r0 >= S2) continue;
-        const int u0 = (int)(itq.z & 0xFFFFu), v0 = (int)(itq.z >> 16);
-        const int kmax = min(RMAX, (S2 - r0 + 31) >> 5);
-        int a[RMAX], b[RMAX];
-        T acc[RMAX][4][2];
+    const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
+    const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
+
+    int ra[NSLOT], rb[NSLOT];                  // this lane-slot's residue (b, a); rb = -1: idle slot
 #pragma unroll
-        for (int k = 0; k < RMAX; ++k) {
-            int r = r0 + k * 32 + lane;
-            bool valid = r < S2;
-            b[k] = valid ? r / S : -1;               // b = -1 marks an idle slot
-            a[k] = valid ? r - b[k] * S : 0;
+    for (int k = 0; k < NSLOT; ++k) {
+        int r = k * 32 + lane;
+        rb[k] = r < S2 ? r / S : -1;
+        ra[k] = r < S2 ? r - rb[k] * S : 0;
+    }
+
+    for (;;) {
+        unsigned item = 0;
+        if (lane == 0) item = atomicAdd(cursor, 1u);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= nitems) break;
+        const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
+
+        C acc[NSLOT];
+        int cell[NSLOT], coff[NSLOT];
+        C cnext[PIPE ? NSLOT : 1];
 #pragma unroll
-            for (int s = 0; s < 4; ++s) acc[k][s][0] = acc[k][s][1] = (T)0;
+        for (int k = 0; k < NSLOT; ++k) { acc[k].x = acc[k].y = (T)0; cell[k] = 0; coff[k] = 0; }
+
+        RecBatch<T> batch;
+        T re, im; unsigned pos, koff;
+        batch.load(rec + i0 + lane, i0 + lane < i1);
+        batch.get(0, re, im, pos, koff);
+        // place every lane-slot on its cell of the first window
+        {
+            const int j0u = (int)(pos & 0xFFFFu), j0v = (int)(pos >> 16);
+            const int ju = SCT ? (j0u & (S - 1)) : j0u % S, jv = SCT ? (j0v & (S - 1)) : j0v % S;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) {
+                int iu = ra[k] - ju; iu += iu < 0 ? S : 0;
+                int iv = rb[k] - jv; iv += iv < 0 ? S : 0;
+                coff[k] = iv * S + iu;
+                cell[k] = (j0v + iv) * N + j0u + iu;
+                if (PIPE && rb[k] >= 0) cnext[k] = __ldg(K + koff + coff[k]);
+            }
         }
-        const Rec<T> *rp = rec + itq.x;
-        const unsigned cnt = itq.y;
-        Rec<T> cur = load_rec<T>(rp);
-        for (unsigned i = 0; i < cnt; ++i) {
-            Rec<T> nxt = cur;
-            if (i + 1 < cnt) nxt = load_rec<T>(rp + i + 1);
-            const int du = (int)(cur.pos & 0x1FFFu) - u0, dv = (int)((cur.pos >> 13) & 0x1FFFu) - v0;
-            const C *Ks = K + cur.koff;
+        for (unsigned i = i0; i < i1; ++i) {
+            const T cre = re, cim = im;
+            const unsigned cpos = pos, ckoff = koff;
+            C ccur[PIPE ? NSLOT : 1];
+            if (PIPE) {
 #pragma unroll
-            for (int k = 0; k < RMAX; ++k) {
-                if (k < kmax && b[k] >= 0) {
-                    const bool hu = a[k] < du, hv = b[k] < dv;
-                    const int iu = a[k] - du + (hu ? S : 0), iv = b[k] - dv + (hv ? S : 0);
-                    const C c = __ldg(Ks + iv * S + iu);
-                    const T pr = cur.re * c.x - cur.im * c.y, pi = cur.re * c.y + cur.im * c.x;
-                    const int sel = (hv ? 2 : 0) + (hu ? 1 : 0);
+                for (int k = 0; k < NSLOT; ++k) ccur[k] = cnext[k];
+            }
+            const bool has_next = i + 1 < i1;
+            bool moved = false;
+            int ncell[PIPE ? NSLOT : 1];
+            if (has_next) {
+                const unsigned j = (i + 1 - i0) & 31u;
+                if (j == 0) batch.load(rec + i + 1 + lane, i + 1 + lane < i1);
+                batch.get((int)j, re, im, pos, koff);
+                moved = pos != cpos;                                   // warp-uniform
+                if (PIPE && moved) {
+                    const int j0u = (int)(pos & 0xFFFFu), j0v = (int)(pos >> 16);
+                    const int ju = SCT ? (j0u & (S - 1)) : j0u % S, jv = SCT ? (j0v & (S - 1)) : j0v % S;
 #pragma unroll
-                    for (int s = 0; s < 4; ++s)
-                        if (sel == s) { acc[k][s][0] += pr; acc[k][s][1] += pi; }
+                    for (int k = 0; k < NSLOT; ++k) {
+                        int iu = ra[k] - ju; iu += iu < 0 ? S : 0;
+                        int iv = rb[k] - jv; iv += iv < 0 ? S : 0;
+                        coff[k] = iv * S + iu;                         // (the current record's loads are already out)
+                        ncell[k] = (j0v + iv) * N + j0u + iu;
+                    }
+                }
+                if (PIPE) {
+#pragma unroll
+                    for (int k = 0; k < NSLOT; ++k)
+                        if (rb[k] >= 0) cnext[k] = __ldg(K + koff + coff[k]);
                 }
             }
-            cur = nxt;
-        }
-        // flush: one reduction per touched cell of the 2S x 2S neighbourhood
+            // the current record
+            if (PIPE) {
 #pragma unroll
-        for (int k = 0; k < RMAX; ++k) {
-            if (k < kmax && b[k] >= 0) {
+                for (int k = 0; k < NSLOT; ++k)
+                    if (rb[k] >= 0) cmac(acc[k], cre, cim, ccur[k]);
+            } else {
+                // large supports: no lookahead; offsets of the CURRENT window are still in coff[]
 #pragma unroll
-                for (int s = 0; s < 4; ++s) {
-                    if (acc[k][s][0] != (T)0 || acc[k][s][1] != (T)0) {
-                        int cu = u0 + a[k] + ((s & 1) ? S : 0), cv = v0 + b[k] + ((s & 2) ? S : 0);
-                        red_add(grid + (long long)cv * N + cu, acc[k][s][0], acc[k][s][1]);
+                for (int k = 0; k < NSLOT; ++k)
+                    if (rb[k] >= 0) cmac(acc[k], cre, cim, __ldg(K + ckoff + coff[k]));
+            }
+            // the window moves: lanes whose cell changes write their sum out
+            if (moved) {
+                const int j0u = (int)(pos & 0xFFFFu), j0v = (int)(pos >> 16);
+                const int ju = SCT ? (j0u & (S - 1)) : j0u % S, jv = SCT ? (j0v & (S - 1)) : j0v % S;
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    int nc;
+                    if (PIPE) {
+                        nc = ncell[k];
+                    } else {
+                        int iu = ra[k] - ju; iu += iu < 0 ? S : 0;
+                        int iv = rb[k] - jv; iv += iv < 0 ? S : 0;
+                        coff[k] = iv * S + iu;
+                        nc = (j0v + iv) * N + j0u + iu;
+                    }
+                    if (rb[k] >= 0 && nc != cell[k]) {
+                        if (acc[k].x != (T)0 || acc[k].y != (T)0) red_add(grid + cell[k], acc[k]);
+                        acc[k].x = acc[k].y = (T)0;
+                        cell[k] = nc;
                     }
                 }
             }
         }
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k)
+            if (rb[k] >= 0 && (acc[k].x != (T)0 || acc[k].y != (T)0)) red_add(grid + cell[k], acc[k]);
     }
 }
 
-template <typename T, int RMAX, int MINB>
-int launch_tiles(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid,
-                 char *w, int maxS) {
+template <typename T, int SCT, int NSLOT, int MINB>
+int launch_runs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+                int cls, int S) {
     using C = typename Cplx<T>::type;
-    int nchunk = (maxS * maxS + 32 * RMAX - 1) / (32 * RMAX);
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
     int blocks = ctx->sm_count * per_sm;
-    grid_tiles_kernel<T, RMAX, MINB><<<blocks, kGridThreads, 0, ctx->stream>>>(
-        (const Rec<T> *)(w + ws.off_records), (const Item *)(w + ws.off_items),
-        (const Counters *)(w + ws.off_counters), (const C *)K, (C *)grid, bp.N, nchunk);
+    unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
+    Counters *ctr = (Counters *)(w + ws.off_counters);
+    grid_runs_kernel<T, SCT, NSLOT, MINB><<<blocks, kRunThreads, 0, ctx->stream>>>(
+        (const Rec<T> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
+        (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, &ctr->cursor[cls],
+        (const C *)K, (C *)grid, bp.N, seg);
     ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }
 
+template <typename T>
+int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+                 int cls, int S) {
+    constexpr bool F = sizeof(T) == 4;
+    if (S == 8) return launch_runs<T, 8, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
+    if (S == 16) return launch_runs<T, 16, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
+    if (S == 4) return launch_runs<T, 4, 1, F ? 6 : 4>(ctx, bp, ws, K, grid, w, cls, S);
+    int nslot = (S * S + 31) / 32;
+    if (nslot <= 2) return launch_runs<T, 0, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
+    if (nslot <= 5) return launch_runs<T, 0, 5, F ? 3 : 2>(ctx, bp, ws, K, grid, w, cls, S);
+    if (nslot <= 8) return launch_runs<T, 0, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
+    if (nslot <= 18) return launch_runs<T, 0, 18, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
+    return launch_runs<T, 0, 32, 1>(ctx, bp, ws, K, grid, w, cls, S);
+}
+
 }  // namespace
 
-int wpg_launch_grid(wpg_ctx *ctx, const PlaneTab &, const BinParams &bp, const WorkspaceLayout &ws,
-                    wpg_prec prec, const void *K, void *grid, char *w, int maxS) {
+int wpg_launch_grid(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws,
+                    wpg_prec prec, const void *K, void *grid, char *w) {
     if (bp.nrow == 0) return WPG_OK;
-    int S2 = maxS * maxS;
-    if (prec == WPG_F32) {
-        if (S2 <= 32) return launch_tiles<float, 1, 6>(ctx, bp, ws, K, grid, w, maxS);
-        if (S2 <= 64) return launch_tiles<float, 2, 4>(ctx, bp, ws, K, grid, w, maxS);
-        if (S2 <= 128) return launch_tiles<float, 4, 3>(ctx, bp, ws, K, grid, w, maxS);
-        return launch_tiles<float, 8, 2>(ctx, bp, ws, K, grid, w, maxS);
+    for (int cls = 0; cls < bp.ncls; ++cls) {
+        int S = tab.clsS[cls];
+        int rc = prec == WPG_F32 ? launch_class<float>(ctx, bp, ws, K, grid, w, cls, S)
+                                 : launch_class<double>(ctx, bp, ws, K, grid, w, cls, S);
+        if (rc) return rc;
     }
-    if (S2 <= 32) return launch_tiles<double, 1, 4>(ctx, bp, ws, K, grid, w, maxS);
-    if (S2 <= 64) return launch_tiles<double, 2, 3>(ctx, bp, ws, K, grid, w, maxS);
-    return launch_tiles<double, 4, 2>(ctx, bp, ws, K, grid, w, maxS);
+    return WPG_OK;
 }
 
 int wpg_launch_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,

@@ -46,21 +46,21 @@ def relerr(g, ref):
     return float(np.max(np.abs(g.astype(np.complex128) - ref)) / np.max(np.abs(ref)))
 
 
-def check_all_paths(ctx, wl, st, ref, rstats, precs=(wpgrid.F32, wpgrid.F64), orders=(1, 2), segments=(0,)):
+def check_all_paths(ctx, wl, st, ref, rstats, precs=(wpgrid.F32, wpgrid.F64), key_bits=(0,), segments=(0,)):
     d = dev(wl)
     for prec in precs:
         ks = upload(ctx, st, prec)
         g, s = ctx.grid_naive(*d, ks, stats=True)
         assert s == rstats
         assert relerr(g.cpu().numpy(), ref) <= TOL[prec], ("naive", prec)
-        for order in orders:
+        for kb in key_bits:
             for seg in segments:
-                ctx.set_option("order", order); ctx.set_option("segment", seg)
+                ctx.set_option("key_bits", kb); ctx.set_option("segment", seg)
                 g, s = ctx.grid(*d, ks, stats=True)
-                assert s == rstats, (order, seg)
+                assert s == rstats, (kb, seg)
                 e = relerr(g.cpu().numpy(), ref)
-                assert e <= TOL[prec], ("tiled", prec, order, seg, e)
-    ctx.set_option("order", 0); ctx.set_option("segment", 0)
+                assert e <= TOL[prec], ("runs", prec, kb, seg, e)
+    ctx.set_option("key_bits", 0); ctx.set_option("segment", 0)
 
 
 # ------------------------------------------------------------------ config 1 (full size)
@@ -74,7 +74,7 @@ def cfg1():
 
 def test_config1_gridder_parity(ctx, cfg1):
     wl, st, ref, rstats = cfg1
-    check_all_paths(ctx, wl, st, ref, rstats, segments=(0, 7, 100))
+    check_all_paths(ctx, wl, st, ref, rstats, key_bits=(0, 12, 8), segments=(0, 1, 7, 100, 100000))
 
 
 def test_config1_wkernel_build_parity(ctx, cfg1):
@@ -127,29 +127,27 @@ def test_binning_records_match_oracle_index_map(ctx):
         j0u, ou = ogrid.index_map(wl.uvw[k, 0], N, wl.cell, S, Q)
         j0v, ov = ogrid.index_map(wl.uvw[k, 1], N, wl.cell, S, Q)
         p, _ = ogrid.plane_of(wl.uvw[k, 2], wl.w_max, wl.Nw)
-        exp.append((j0u | (j0v << 13) | ((S - 1) << 26), (p * Q * Q + ov * Q + ou) * S * S,
+        exp.append((j0u | (j0v << 16), (p * Q * Q + ov * Q + ou) * S * S,
                     np.float32(wl.vis[k, 0].real).view(np.uint32), np.float32(wl.vis[k, 0].imag).view(np.uint32)))
     exp = sorted(exp)
-    for order in (1, 2):
-        ctx.set_option("order", order)
+    for kb in (0, 12):
+        ctx.set_option("key_bits", kb)
         ws, info, stats = ctx.bin(*d, ks)
-        assert info["n_records"] == 20000 and info["order"] == order and info["tile"] == 7
+        assert info["n_records"] == 20000 and info["n_classes"] == 1 and info["record_bytes"] == 16
+        ush = info["u_shift"]
+        assert ush == (0 if kb == 0 else 4) and info["keys_per_class"] == N * ((N + (1 << ush) - 1) >> ush)
         raw = ws.cpu().numpy()
         rec = raw[info["off_records"]:info["off_records"] + 16 * 20000].view(np.uint32).reshape(-1, 4)
         got = sorted((int(r[2]), int(r[3]), int(r[0]), int(r[1])) for r in rec)
         assert got == [tuple(int(x) for x in e) for e in exp]
-        # records are grouped by key: bucket_start is monotone and ends at n_records; items cover every record once
+        # records are ordered by key = j0v * ceil(N / 2^ush) + (j0u >> ush); bucket_start matches that order
+        ju = (rec[:, 2] & 0xFFFF).astype(np.int64); jv = (rec[:, 2] >> 16).astype(np.int64)
+        key = jv * info["keys_per_class"] // N + (ju >> ush)
+        assert np.all(np.diff(key) >= 0)
         bs = raw[info["off_bucket_start"]:info["off_bucket_start"] + 4 * (info["n_keys"] + 1)].view(np.uint32)
-        assert bs[0] == 0 and bs[-1] == 20000 and np.all(np.diff(bs.astype(np.int64)) >= 0)
-        items = raw[info["off_items"]:info["off_items"] + 16 * info["n_items"]].view(np.uint32).reshape(-1, 4)
-        cover = np.zeros(20000, np.int32)
-        for b, c, org, s_ in items:
-            cover[b:b + c] += 1
-            u0, v0 = int(org) & 0xFFFF, int(org) >> 16
-            ju = rec[b:b + c, 2] & 0x1FFF; jv = (rec[b:b + c, 2] >> 13) & 0x1FFF
-            assert s_ == 7 and np.all((ju >= u0) & (ju < u0 + 7) & (jv >= v0) & (jv < v0 + 7))
-        assert np.all(cover == 1)
-    ctx.set_option("order", 0)
+        assert bs[0] == 0 and bs[-1] == 20000
+        assert np.array_equal(bs.astype(np.int64), np.searchsorted(key, np.arange(info["n_keys"] + 1)))
+    ctx.set_option("key_bits", 0)
 
 
 # ------------------------------------------------------------------ edge cases
