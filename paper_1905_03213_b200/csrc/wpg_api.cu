@@ -148,6 +148,7 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     ws->off_counters = o; o += align_up(sizeof(Counters));
     ws->off_hist = o;     o += align_up((size_t)(nkeys + 4) * 4);
     ws->off_blocksum = o; o += align_up((size_t)ws->nblocks_scan * 4 + 8);
+    ws->off_fscale = o;   o += align_up((size_t)nchan * 8);
     ws->off_key = o;      o += align_up((size_t)nvis * 4);
     ws->off_rank = o;     o += align_up((size_t)nvis * 4);
     ws->off_pre = o;      o += align_up((size_t)nvis * 8);

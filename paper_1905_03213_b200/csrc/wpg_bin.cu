@@ -17,37 +17,58 @@ __device__ __forceinline__ void warp_count(unsigned long long *dst, unsigned v) 
     if ((threadIdx.x & 31) == 0 && s) atomicAdd(dst, (unsigned long long)s);
 }
 
+// Pass 0: f[ch] = freq[ch] / c0 (G1), once per channel instead of once per visibility.  Same IEEE
+// division as G1 states, so the products u = uvw * f are bit-identical.
+__global__ void chan_scale_kernel(const double *__restrict__ freq, int nchan, double *__restrict__ fscale) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < nchan) fscale[c] = __ddiv_rn(freq[c], WPG_C0);
+}
+
+constexpr int kVpt = 4;            // visibilities per thread: four histogram atomics in flight per thread
+
 // Pass 1: position math (fp64, G1-G3), validity (G4, R9), key, rank inside the key's bucket.
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weight,
-                 const double *__restrict__ freq, const __grid_constant__ PlaneTab T,
+                 const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
                  const __grid_constant__ BinParams P, Counters *__restrict__ ctr,
                  unsigned *__restrict__ hist, unsigned *__restrict__ key_out,
                  unsigned *__restrict__ rank_out, uint2 *__restrict__ pre_out) {
-    long long nvis = P.nrow * P.nchan;
-    long long base = (long long)blockIdx.x * blockDim.x;
-    long long i = base + threadIdx.x;
+    const long long nvis = P.nrow * P.nchan;
+    const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
     unsigned c_grid = 0, c_oob = 0, c_zero = 0, c_clamp = 0, c_upd = 0;
-    if (i < nvis) {
-        long long row = i / P.nchan;
-        int ch = (int)(i - row * P.nchan);
-        unsigned key = WPG_NO_KEY;
-        if (weight[i] == 0.0f) {
-            c_zero = 1;
-        } else {
-            double f = __ddiv_rn(freq[ch], WPG_C0);
-            VisPos r = wpg_locate(uvw[3 * row], uvw[3 * row + 1], uvw[3 * row + 2], f, P, T);
-            if (!r.inside) {
-                c_oob = 1;
+    unsigned key[kVpt], rank[kVpt];
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) {
+        const long long i = base + j * 256;
+        key[j] = WPG_NO_KEY;
+        if (i < nvis) {
+            long long row = i; int ch = 0;
+            if (P.nchan > 1) { row = i / P.nchan; ch = (int)(i - row * P.nchan); }
+            if (__ldg(weight + i) == 0.0f) {
+                c_zero += 1;
             } else {
-                c_grid = 1; c_clamp = r.clamped; c_upd = r.S * r.S;
-                key = (unsigned)T.cls[r.p] * P.keys_per_class + (unsigned)r.j0v * (unsigned)P.nug +
-                      ((unsigned)r.j0u >> P.ushift);
-                rank_out[i] = atomicAdd(&hist[key], 1u);
-                pre_out[i] = make_uint2((unsigned)r.j0u | ((unsigned)r.j0v << 16), wpg_koff(r, P, T));
+                VisPos r = wpg_locate(__ldg(uvw + 3 * row), __ldg(uvw + 3 * row + 1), __ldg(uvw + 3 * row + 2),
+                                      __ldg(fscale + ch), P, T);
+                if (!r.inside) {
+                    c_oob += 1;
+                } else {
+                    c_grid += 1; c_clamp += r.clamped; c_upd += r.S * r.S;
+                    key[j] = (unsigned)T.cls[r.p] * P.keys_per_class + (unsigned)r.j0v * (unsigned)P.nug +
+                             ((unsigned)r.j0u >> P.ushift);
+                    pre_out[i] = make_uint2((unsigned)r.j0u | ((unsigned)r.j0v << 16), wpg_koff(r, P, T));
+                }
             }
         }
-        key_out[i] = key;
+    }
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) rank[j] = key[j] != WPG_NO_KEY ? atomicAdd(&hist[key[j]], 1u) : 0u;
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) {
+        const long long i = base + j * 256;
+        if (i < nvis) {
+            key_out[i] = key[j];
+            if (key[j] != WPG_NO_KEY) rank_out[i] = rank[j];
+        }
     }
     warp_count(&ctr->n_gridded, c_grid);
     warp_count(&ctr->n_skipped_oob, c_oob);
@@ -137,6 +158,15 @@ scan_apply_kernel(unsigned *__restrict__ hist, unsigned nkeys, const unsigned *_
     }
 }
 
+// One 16-byte store per fp32 record; 8 + 8 + 8 for the 24-byte fp64 record.
+__device__ __forceinline__ void store_rec(Rec<float> *dst, float re, float im, uint2 p) {
+    *reinterpret_cast<uint4 *>(dst) = make_uint4(__float_as_uint(re), __float_as_uint(im), p.x, p.y);
+}
+__device__ __forceinline__ void store_rec(Rec<double> *dst, double re, double im, uint2 p) {
+    dst->re = re; dst->im = im;
+    *reinterpret_cast<uint2 *>(&dst->pos) = p;
+}
+
 // Pass 3: scatter into key order.  The record carries weight*vis (R9, natural weighting).
 template <typename TT>
 __global__ void __launch_bounds__(256)
@@ -144,17 +174,27 @@ scatter_kernel(const float2 *__restrict__ vis, const float *__restrict__ weight,
                const unsigned *__restrict__ key, const unsigned *__restrict__ rank,
                const uint2 *__restrict__ pre, const unsigned *__restrict__ bucket_start,
                long long nvis, Rec<TT> *__restrict__ rec) {
-    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nvis) return;
-    unsigned k = key[i];
-    if (k == WPG_NO_KEY) return;
-    unsigned dst = bucket_start[k] + rank[i];
-    float2 v = vis[i];
-    TT w = (TT)weight[i];
-    uint2 p = pre[i];
-    Rec<TT> r;
-    r.re = w * (TT)v.x; r.im = w * (TT)v.y; r.pos = p.x; r.koff = p.y;
-    rec[dst] = r;
+    const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
+    unsigned k[kVpt], dst[kVpt];
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) {
+        const long long i = base + j * 256;
+        k[j] = i < nvis ? __ldg(key + i) : WPG_NO_KEY;
+    }
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) {
+        const long long i = base + j * 256;
+        dst[j] = k[j] != WPG_NO_KEY ? __ldg(bucket_start + k[j]) + __ldg(rank + i) : 0u;
+    }
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) {
+        const long long i = base + j * 256;
+        if (k[j] == WPG_NO_KEY) continue;
+        float2 v = __ldg(vis + i);
+        TT w = (TT)__ldg(weight + i);
+        uint2 p = __ldg(pre + i);
+        store_rec(rec + dst[j], w * (TT)v.x, w * (TT)v.y, p);
+    }
 }
 
 }  // namespace
@@ -169,8 +209,10 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
     unsigned *key = (unsigned *)(w + ws.off_key), *rank = (unsigned *)(w + ws.off_rank);
     uint2 *pre = (uint2 *)(w + ws.off_pre);
     cudaStream_t s = ctx->stream;
-    unsigned nb = (unsigned)((nvis + 255) / 256);
-    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, d_freq, tab, bp, ctr, hist, key, rank, pre);
+    double *fscale = (double *)(w + ws.off_fscale);
+    unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
+    chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale);
+    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist, key, rank, pre);
     scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
     scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
@@ -182,7 +224,7 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
             scatter_kernel<double><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_weight, key, rank, pre, hist, nvis,
                                                        (Rec<double> *)(w + ws.off_records));
     }
-    ctx->n_launches += nb ? 5 : 3;
+    ctx->n_launches += nb ? 6 : 4;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }

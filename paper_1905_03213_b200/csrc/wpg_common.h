@@ -51,7 +51,7 @@ struct Counters {
 };
 
 struct WorkspaceLayout {
-    size_t off_counters, off_key, off_rank, off_pre, off_records, off_hist, off_blocksum;
+    size_t off_counters, off_key, off_rank, off_pre, off_records, off_hist, off_blocksum, off_fscale;
     size_t total;
     uint32_t nkeys, nblocks_scan;
 };

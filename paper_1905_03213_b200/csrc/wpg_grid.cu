@@ -14,6 +14,8 @@
 //    run of visibilities costs one coefficient load and two packed FMAs per update; when the window
 //    moves, only the lanes whose cell changed flush (red.global.add.v2.f32 / .f64).
 //    Coefficients are read through L1 from the L2-resident stack, one record ahead of their use.
+#include <type_traits>
+
 #include "wpg_common.h"
 
 namespace {
@@ -92,35 +94,41 @@ grid_naive_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw
 }
 
 // ------------------------------------------------------------------------------------ runs
-// One lane's copy of a batch of 32 sorted records, handed out one by one with shuffles.
-template <typename T> struct RecBatch;
-template <> struct RecBatch<float> {
-    uint4 q;
-    __device__ __forceinline__ void load(const Rec<float> *p, bool ok) {
-        q = ok ? __ldg(reinterpret_cast<const uint4 *>(p)) : make_uint4(0, 0, 0, 0);
-    }
-    __device__ __forceinline__ void get(int j, float &re, float &im, unsigned &pos, unsigned &koff) const {
-        re = __uint_as_float(__shfl_sync(0xffffffffu, q.x, j));
-        im = __uint_as_float(__shfl_sync(0xffffffffu, q.y, j));
-        pos = __shfl_sync(0xffffffffu, q.z, j);
-        koff = __shfl_sync(0xffffffffu, q.w, j);
-    }
-};
-template <> struct RecBatch<double> {
-    double re_, im_; uint2 t;                                     // 24-byte records: 8-byte aligned only
-    __device__ __forceinline__ void load(const Rec<double> *p, bool ok) {
-        re_ = ok ? __ldg(&p->re) : 0.0; im_ = ok ? __ldg(&p->im) : 0.0;
-        t = ok ? __ldg(reinterpret_cast<const uint2 *>(&p->pos)) : make_uint2(0, 0);
-    }
-    __device__ __forceinline__ void get(int j, double &re, double &im, unsigned &pos, unsigned &koff) const {
-        re = __shfl_sync(0xffffffffu, re_, j);
-        im = __shfl_sync(0xffffffffu, im_, j);
-        pos = __shfl_sync(0xffffffffu, t.x, j);
-        koff = __shfl_sync(0xffffffffu, t.y, j);
-    }
-};
-
+// Per-warp ring of sorted records in shared memory, filled with cp.async (LDGSTS) two chunks ahead
+// of their use; a record is then one broadcast LDS away from every lane.
 constexpr int kRunThreads = 256;
+constexpr int kChunk = 16;                       // records per chunk
+constexpr int kRing = 4;                         // chunks in the ring
+constexpr unsigned kRingMask = kChunk * kRing - 1;
+
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// Copy chunk c of the item [i0, i1) into its ring slot (only the records that exist).
+__device__ __forceinline__ void ring_fill(Rec<float> *ring, const Rec<float> *rec, unsigned i0, unsigned i1, unsigned c, int lane) {
+    const unsigned i = i0 + c * kChunk + lane;
+    if (lane < kChunk && i < i1)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(ring + ((c * kChunk + lane) & kRingMask))), "l"(rec + i) : "memory");
+}
+__device__ __forceinline__ void ring_fill(Rec<double> *ring, const Rec<double> *rec, unsigned i0, unsigned i1, unsigned c, int lane) {
+    // 24-byte records are 8-byte aligned only: three 8-byte pieces per record
+    const unsigned long long *g = reinterpret_cast<const unsigned long long *>(rec + i0 + c * kChunk);
+    unsigned long long *sm = reinterpret_cast<unsigned long long *>(ring + ((c * kChunk) & kRingMask));
+    const unsigned first = i0 + c * kChunk;
+    const unsigned npiece = first < i1 ? 3u * min((unsigned)kChunk, i1 - first) : 0u;
+    for (unsigned q = lane; q < npiece; q += 32)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(sm + q)), "l"(g + q) : "memory");
+}
+__device__ __forceinline__ void ring_get(const Rec<float> *ring, unsigned slot, float &re, float &im, unsigned &pos, unsigned &koff) {
+    const uint4 q = *reinterpret_cast<const uint4 *>(ring + slot);
+    re = __uint_as_float(q.x); im = __uint_as_float(q.y); pos = q.z; koff = q.w;
+}
+__device__ __forceinline__ void ring_get(const Rec<double> *ring, unsigned slot, double &re, double &im, unsigned &pos, unsigned &koff) {
+    re = ring[slot].re; im = ring[slot].im;
+    const uint2 t = *reinterpret_cast<const uint2 *>(&ring[slot].pos);
+    pos = t.x; koff = t.y;
+}
 
 // SCT: compile-time support (a power of two) or 0 = S_rt.  NSLOT >= ceil(S^2 / 32).
 template <typename T, int SCT, int NSLOT, int MINB>
@@ -130,12 +138,16 @@ grid_runs_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bu
                  const typename Cplx<T>::type *__restrict__ K, typename Cplx<T>::type *__restrict__ grid,
                  int N, unsigned seg) {
     using C = typename Cplx<T>::type;
-    constexpr bool PIPE = NSLOT <= 8;         // coefficients of record i+1 are fetched while record i is added
+    constexpr bool PIPE = NSLOT <= 8;          // coefficients of record i+1 are requested before record i is added
+    constexpr bool FULL = SCT * SCT == NSLOT * 32;   // every lane-slot owns a cell
     const int S = SCT ? SCT : S_rt;
     const int S2 = S * S;
     const int lane = threadIdx.x & 31;
     const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
     const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
+
+    __shared__ __align__(16) Rec<T> ring_all[kRunThreads / 32][kChunk * kRing];
+    Rec<T> *ring = ring_all[threadIdx.x >> 5];
 
     int ra[NSLOT], rb[NSLOT];                  // this lane-slot's residue (b, a); rb = -1: idle slot
 #pragma unroll
@@ -152,99 +164,100 @@ grid_runs_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bu
         if (item >= nitems) break;
         const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
 
+        __syncwarp();                          // the previous item's ring reads are done
+#pragma unroll
+        for (unsigned c = 0; c < 3; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
+
         C acc[NSLOT];
-        int cell[NSLOT], coff[NSLOT];
-        C cnext[PIPE ? NSLOT : 1];
+        unsigned cell[NSLOT], coff[NSLOT];
 #pragma unroll
         for (int k = 0; k < NSLOT; ++k) { acc[k].x = acc[k].y = (T)0; cell[k] = 0; coff[k] = 0; }
+        unsigned pos_cur = 0;
 
-        RecBatch<T> batch;
-        T re, im; unsigned pos, koff;
-        batch.load(rec + i0 + lane, i0 + lane < i1);
-        batch.get(0, re, im, pos, koff);
-        // place every lane-slot on its cell of the first window
-        {
+        // the window moves to `pos`: lane-slots whose cell changes write their sum out (FLUSH) and
+        // every lane-slot gets the offset of its cell inside the S x S coefficient slice
+        auto place = [&](unsigned pos, auto flush_tag) {
+            constexpr bool FLUSH = decltype(flush_tag)::value;
             const int j0u = (int)(pos & 0xFFFFu), j0v = (int)(pos >> 16);
             const int ju = SCT ? (j0u & (S - 1)) : j0u % S, jv = SCT ? (j0v & (S - 1)) : j0v % S;
 #pragma unroll
             for (int k = 0; k < NSLOT; ++k) {
                 int iu = ra[k] - ju; iu += iu < 0 ? S : 0;
                 int iv = rb[k] - jv; iv += iv < 0 ? S : 0;
-                coff[k] = iv * S + iu;
-                cell[k] = (j0v + iv) * N + j0u + iu;
-                if (PIPE && rb[k] >= 0) cnext[k] = __ldg(K + koff + coff[k]);
-            }
-        }
-        for (unsigned i = i0; i < i1; ++i) {
-            const T cre = re, cim = im;
-            const unsigned cpos = pos, ckoff = koff;
-            C ccur[PIPE ? NSLOT : 1];
-            if (PIPE) {
-#pragma unroll
-                for (int k = 0; k < NSLOT; ++k) ccur[k] = cnext[k];
-            }
-            const bool has_next = i + 1 < i1;
-            bool moved = false;
-            int ncell[PIPE ? NSLOT : 1];
-            if (has_next) {
-                const unsigned j = (i + 1 - i0) & 31u;
-                if (j == 0) batch.load(rec + i + 1 + lane, i + 1 + lane < i1);
-                batch.get((int)j, re, im, pos, koff);
-                moved = pos != cpos;                                   // warp-uniform
-                if (PIPE && moved) {
-                    const int j0u = (int)(pos & 0xFFFFu), j0v = (int)(pos >> 16);
-                    const int ju = SCT ? (j0u & (S - 1)) : j0u % S, jv = SCT ? (j0v & (S - 1)) : j0v % S;
-#pragma unroll
-                    for (int k = 0; k < NSLOT; ++k) {
-                        int iu = ra[k] - ju; iu += iu < 0 ? S : 0;
-                        int iv = rb[k] - jv; iv += iv < 0 ? S : 0;
-                        coff[k] = iv * S + iu;                         // (the current record's loads are already out)
-                        ncell[k] = (j0v + iv) * N + j0u + iu;
-                    }
-                }
-                if (PIPE) {
-#pragma unroll
-                    for (int k = 0; k < NSLOT; ++k)
-                        if (rb[k] >= 0) cnext[k] = __ldg(K + koff + coff[k]);
-                }
-            }
-            // the current record
-            if (PIPE) {
-#pragma unroll
-                for (int k = 0; k < NSLOT; ++k)
-                    if (rb[k] >= 0) cmac(acc[k], cre, cim, ccur[k]);
-            } else {
-                // large supports: no lookahead; offsets of the CURRENT window are still in coff[]
-#pragma unroll
-                for (int k = 0; k < NSLOT; ++k)
-                    if (rb[k] >= 0) cmac(acc[k], cre, cim, __ldg(K + ckoff + coff[k]));
-            }
-            // the window moves: lanes whose cell changes write their sum out
-            if (moved) {
-                const int j0u = (int)(pos & 0xFFFFu), j0v = (int)(pos >> 16);
-                const int ju = SCT ? (j0u & (S - 1)) : j0u % S, jv = SCT ? (j0v & (S - 1)) : j0v % S;
-#pragma unroll
-                for (int k = 0; k < NSLOT; ++k) {
-                    int nc;
-                    if (PIPE) {
-                        nc = ncell[k];
-                    } else {
-                        int iu = ra[k] - ju; iu += iu < 0 ? S : 0;
-                        int iv = rb[k] - jv; iv += iv < 0 ? S : 0;
-                        coff[k] = iv * S + iu;
-                        nc = (j0v + iv) * N + j0u + iu;
-                    }
-                    if (rb[k] >= 0 && nc != cell[k]) {
-                        if (acc[k].x != (T)0 || acc[k].y != (T)0) red_add(grid + cell[k], acc[k]);
+                coff[k] = (unsigned)(iv * S + iu);
+                const unsigned nc = (unsigned)((j0v + iv) * N + j0u + iu);
+                if (FLUSH) {
+                    if ((FULL || rb[k] >= 0) && nc != cell[k]) {
+                        red_add(grid + cell[k], acc[k]);
                         acc[k].x = acc[k].y = (T)0;
-                        cell[k] = nc;
                     }
                 }
+                cell[k] = nc;
+            }
+            pos_cur = pos;
+        };
+        auto fetch = [&](C(&c)[NSLOT], unsigned koff, bool pred) {
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k)
+                if (pred && (FULL || rb[k] >= 0)) c[k] = __ldg(K + (koff + coff[k]));     // 32-bit index, one widening multiply-add
+        };
+        auto add = [&](T re, T im, const C(&c)[NSLOT]) {
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k)
+                if (FULL || rb[k] >= 0) cmac(acc[k], re, im, c[k]);
+        };
+        // entering chunk c: request chunk c + 3 (its slot held chunk c - 1), make chunks <= c + 1 visible
+        auto enter_chunk = [&](unsigned c) {
+            __syncwarp();
+            ring_fill(ring, rec, i0, i1, c + 3, lane);
+            cp_async_commit();
+            cp_async_wait<2>();
+            __syncwarp();
+        };
+
+        T reA, imA, reB, imB; unsigned posA, koffA, posB, koffB;
+        C cA[NSLOT], cB[PIPE ? NSLOT : 1];
+        enter_chunk(0);
+        ring_get(ring, 0, reA, imA, posA, koffA);
+        place(posA, std::false_type());
+        if (PIPE) fetch(cA, koffA, true);
+
+        // one record: `cur` is added, `nxt` is looked at (and its coefficients requested) first.
+        // Returns false after the last record of the item.
+        auto half = [&](unsigned i, T re, T im, unsigned koff, C(&cc)[NSLOT], T &nre, T &nim, unsigned &npos,
+                        unsigned &nkoff, C(&cn)[PIPE ? NSLOT : 1]) -> bool {
+            const bool has_next = i + 1 < i1;
+            ring_get(ring, (i + 1 - i0) & kRingMask, nre, nim, npos, nkoff);
+            const bool same = has_next && npos == pos_cur;
+            if (PIPE) {
+                fetch(reinterpret_cast<C(&)[NSLOT]>(cn), nkoff, same);
+            } else {
+                fetch(cc, koff, true);
+            }
+            add(re, im, cc);
+            if (!has_next) return false;
+            if (!same) {
+                place(npos, std::true_type());
+                if (PIPE) fetch(reinterpret_cast<C(&)[NSLOT]>(cn), nkoff, true);
+            }
+            return true;
+        };
+
+        for (unsigned i = i0;; i += 2) {
+            if (i != i0 && ((i - i0) & (kChunk - 1)) == 0) enter_chunk((i - i0) / kChunk);
+            if (PIPE) {
+                if (!half(i, reA, imA, koffA, cA, reB, imB, posB, koffB, cB)) break;
+                if (!half(i + 1, reB, imB, koffB, reinterpret_cast<C(&)[NSLOT]>(cB), reA, imA, posA, koffA,
+                          reinterpret_cast<C(&)[PIPE ? NSLOT : 1]>(cA))) break;
+            } else {
+                if (!half(i, reA, imA, koffA, cA, reB, imB, posB, koffB, cB)) break;
+                if (!half(i + 1, reB, imB, koffB, cA, reA, imA, posA, koffA, cB)) break;
             }
         }
 #pragma unroll
         for (int k = 0; k < NSLOT; ++k)
-            if (rb[k] >= 0 && (acc[k].x != (T)0 || acc[k].y != (T)0)) red_add(grid + cell[k], acc[k]);
+            if (FULL || rb[k] >= 0) red_add(grid + cell[k], acc[k]);
+        cp_async_wait<0>();
     }
 }
 
