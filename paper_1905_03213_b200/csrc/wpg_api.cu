@@ -62,6 +62,7 @@ extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
     else if (!strcmp(name, "ctas_per_sm")) { if (value < 0 || value > 32) return wpg_fail(ctx, WPG_EINVAL, "ctas_per_sm must be 0..32"); ctx->opt_ctas_per_sm = (int)value; }
     else if (!strcmp(name, "key_bits")) { if (value != 0 && (value < 8 || value > 28)) return wpg_fail(ctx, WPG_EINVAL, "key_bits must be 0 or 8..28"); ctx->opt_key_bits = (int)value; }
     else if (!strcmp(name, "timing")) { ctx->opt_timing = value != 0; }
+    else if (!strcmp(name, "no_pairs")) { ctx->opt_no_pairs = value != 0; }
     else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
     return WPG_OK;
 }
@@ -129,12 +130,16 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     bp->du = 1.0 / fov;
     bp->halfN = (double)(d->grid_N / 2);
     bp->ncls = (int)distinct.size();
-    // sort key = (class, j0v, j0u >> ushift): full resolution unless the key space would exceed 2^key_bits
+    // sort key = (class, j0v, j0u & 1, (j0u >> 1) >> ushift): a grid row is swept twice, even window starts
+    // first, then odd ones (the pair gridder keeps column ownership fixed within a parity); full resolution
+    // unless the key space would exceed 2^key_bits
     const int64_t cap = (int64_t)1 << (ctx->opt_key_bits ? ctx->opt_key_bits : 26);
+    const int64_t halfcols = (d->grid_N + 1) / 2;
     int ushift = 0;
-    while ((int64_t)bp->ncls * d->grid_N * (((int64_t)d->grid_N + (1 << ushift) - 1) >> ushift) > cap && ushift < 13) ++ushift;
+    while ((int64_t)bp->ncls * d->grid_N * 2 * ((halfcols + (1 << ushift) - 1) >> ushift) > cap && ushift < 13) ++ushift;
     bp->ushift = ushift;
-    bp->nug = (d->grid_N + (1 << ushift) - 1) >> ushift;
+    bp->nuh = (int)((halfcols + (1 << ushift) - 1) >> ushift);
+    bp->nug = 2 * bp->nuh;
     bp->keys_per_class = (uint32_t)((int64_t)d->grid_N * bp->nug);
     int64_t nkeys = (int64_t)bp->ncls * bp->keys_per_class;
     if (nkeys > ((int64_t)1 << 30)) return wpg_fail(ctx, WPG_EINVAL, "sort key space %lld too large", (long long)nkeys);

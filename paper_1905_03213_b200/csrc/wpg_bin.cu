@@ -3,9 +3,10 @@
 //
 // The paper's analogue is the re-order of PAPER.md:62-78: count array C, exclusive prefix sum
 // Eq. (2), scatter — keyed there by baseline (Eq. 1) so that consecutive samples of a baseline hit
-// the same grid point.  Here the key is (support class, window start j0v, j0u), i.e.
-// the visibilities are ordered by the grid point they hit, whatever baseline they came from: runs
-// of equal window start are what the gridder (wpg_grid.cu) accumulates in registers.
+// the same grid point.  Here the key is (support class, window start j0v, parity of
+// j0u, j0u >> 1), i.e. the visibilities are ordered by the grid point they hit, whatever baseline
+// they came from: runs of equal window start are what the gridder (wpg_grid.cu) accumulates in
+// registers, and within a (row, parity) sweep the window start moves by even steps.
 #include "wpg_common.h"
 
 namespace {
@@ -54,7 +55,7 @@ bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weigh
                 } else {
                     c_grid += 1; c_clamp += r.clamped; c_upd += r.S * r.S;
                     key[j] = (unsigned)T.cls[r.p] * P.keys_per_class + (unsigned)r.j0v * (unsigned)P.nug +
-                             ((unsigned)r.j0u >> P.ushift);
+                             ((unsigned)r.j0u & 1u) * (unsigned)P.nuh + (((unsigned)r.j0u >> 1) >> P.ushift);
                     pre_out[i] = make_uint2((unsigned)r.j0u | ((unsigned)r.j0v << 16), wpg_koff(r, P, T));
                 }
             }

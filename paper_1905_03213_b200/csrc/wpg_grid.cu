@@ -261,6 +261,203 @@ grid_runs_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bu
     }
 }
 
+// ------------------------------------------------------------------------------------ pairs
+// fp32, even support.  A lane-slot owns a PAIR of horizontally adjacent cells: the cells of the window
+// whose row is congruent to rb and whose columns are congruent to (ra2 + par, ra2 + par + 1) modulo S,
+// par = parity of the window start j0u (the records come sorted by (row, parity, column), so within a
+// sweep the ownership never changes).  The two coefficients of a pair are adjacent and 16-byte aligned
+// in K[p][ov][ou][iv][:], so one LDG.128 feeds two updates.
+//
+// v*c = re*c + i*(im*c): the lane keeps A = sum re*c and B = sum im*c per cell (two packed FMAs per
+// update, the coefficient pair used as loaded, (re,re) and (im,im) formed once per record) and
+// combines them when it writes the cell out: grid += (A.x - B.y, A.y + B.x).
+//
+// The coefficient loads run DEPTH records ahead of their use in a register ring (statically indexed,
+// the record loop is unrolled by DEPTH): the slice of a record is picked at random from a stack that
+// is several times the L1, so most loads are L2 hits (~300 cycles).  The look-ahead is "stateless":
+// the lane's offset inside the slice, (iv, iu0), is computed from the record's window start alone.
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void fma2(unsigned long long &acc, unsigned long long a, unsigned long long b) {
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ float2 unpack2(unsigned long long v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+__device__ __forceinline__ void ldg128(const float2 *p, unsigned long long &c0, unsigned long long &c1) {
+    asm volatile("ld.global.nc.v2.b64 {%0, %1}, [%2];" : "=l"(c0), "=l"(c1) : "l"(p));
+}
+
+template <int SCT, int NSLOT, int DEPTH, int MINB>
+__global__ void __launch_bounds__(kRunThreads, MINB)
+grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
+                  unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
+                  const float2 *__restrict__ K, float2 *__restrict__ grid, int N, unsigned seg) {
+    static_assert(kChunk % DEPTH == 0, "the look-ahead depth divides the chunk");
+    using U64 = unsigned long long;
+    const int S = SCT ? SCT : S_rt;
+    const int H = S >> 1;                                // pairs per window row
+    const int NP = S * H;                                // pairs per window
+    const int lane = threadIdx.x & 31;
+    const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
+    const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
+
+    __shared__ __align__(16) Rec<float> ring_all[kRunThreads / 32][kChunk * kRing];
+    Rec<float> *ring = ring_all[threadIdx.x >> 5];
+
+    // lane-slot constants.  Power-of-two S: RG packs (ra2 + 1, rb) with a guard bit so that
+    // (RG - pos) & M is (iu0 | iv << 16) in two instructions: iu0 = (ra2 + par - j0u) mod S equals
+    // ((ra2 + 1 - j0u) mod S) & ~1 because S and ra2 are even.
+    unsigned RG[NSLOT];
+    int ra2p1[NSLOT], rb[NSLOT];
+    bool act[NSLOT];
+#pragma unroll
+    for (int k = 0; k < NSLOT; ++k) {
+        int r = k * 32 + lane;
+        act[k] = r < NP;
+        r = act[k] ? r : 0;
+        rb[k] = r / H;
+        ra2p1[k] = 2 * (r - rb[k] * H) + 1;
+        RG[k] = (0x8000u + (unsigned)ra2p1[k]) | ((0x8000u + (unsigned)rb[k]) << 16);
+    }
+    constexpr unsigned M = SCT ? ((unsigned)(SCT - 2) | ((unsigned)(SCT - 1) << 16)) : 0u;
+
+    // (iu0 | iv << 16) of this lane-slot for a window starting at pos = j0u | j0v << 16
+    auto offset_in_window = [&](unsigned pos, int k) -> unsigned {
+        if (SCT) return (RG[k] - pos) & M;
+        const unsigned j0u = pos & 0xFFFFu, j0v = pos >> 16;
+        const int ju = (int)(j0u - ((j0u * magicS) >> 20) * (unsigned)S);     // j0u mod S
+        const int jv = (int)(j0v - ((j0v * magicS) >> 20) * (unsigned)S);
+        int x = ra2p1[k] - ju; x += x < 0 ? S : 0;
+        int y = rb[k] - jv;    y += y < 0 ? S : 0;
+        return (unsigned)(x & ~1) | ((unsigned)y << 16);
+    };
+
+    for (;;) {
+        unsigned item = 0;
+        if (lane == 0) item = atomicAdd(cursor, 1u);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= nitems) break;
+        const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
+        const unsigned cnt = i1 - i0;
+
+        __syncwarp();                          // the previous item's ring reads are done
+#pragma unroll
+        for (unsigned c = 0; c < 3; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
+
+        U64 A0[NSLOT], B0[NSLOT], A1[NSLOT], B1[NSLOT];     // accumulators of the pair's two cells
+        unsigned qcur[NSLOT];                               // (column | row << 16) of the pair's first cell
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) A0[k] = B0[k] = A1[k] = B1[k] = 0ull;
+
+        // look-ahead ring (registers)
+        U64 c0[DEPTH][NSLOT], c1[DEPTH][NSLOT];
+        unsigned qn[DEPTH][NSLOT];
+        float re[DEPTH], im[DEPTH];
+
+        auto flush = [&](int k) {
+            const unsigned q = qcur[k];
+            float2 *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
+            const float2 a0 = unpack2(A0[k]), b0 = unpack2(B0[k]), a1 = unpack2(A1[k]), b1 = unpack2(B1[k]);
+            red_add(g, make_float2(a0.x - b0.y, a0.y + b0.x));
+            red_add(g + 1, make_float2(a1.x - b1.y, a1.y + b1.x));
+        };
+        // stage s <- record at ring slot `slot`: window offset, cell, coefficient loads
+        auto produce = [&](int s, unsigned slot) {
+            float r_, i_; unsigned pos, koff;
+            ring_get(ring, slot, r_, i_, pos, koff);
+            re[s] = r_; im[s] = i_;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) {
+                const unsigned d = offset_in_window(pos, k);
+                qn[s][k] = act[k] ? pos + d : 0xFFFFFFFFu;
+                const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
+                ldg128(K + (koff + (act[k] ? coff : 0u)), c0[s][k], c1[s][k]);
+            }
+        };
+        auto consume = [&](int s) {
+            bool any = false;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) any |= qn[s][k] != qcur[k];
+            if (__any_sync(0xffffffffu, any)) {
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    if (qn[s][k] != qcur[k]) {
+                        flush(k);
+                        A0[k] = B0[k] = A1[k] = B1[k] = 0ull;
+                    }
+                    qcur[k] = qn[s][k];
+                }
+            }
+            const U64 rr = pack2(re[s], re[s]), ii = pack2(im[s], im[s]);
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) {
+                fma2(A0[k], c0[s][k], rr); fma2(B0[k], c0[s][k], ii);
+                fma2(A1[k], c1[s][k], rr); fma2(B1[k], c1[s][k], ii);
+            }
+        };
+        // entering chunk c of the PRODUCER: request chunk c + 2 (its slot held chunk c - 2, whose records
+        // are in registers or done), make chunks <= c visible
+        auto enter_chunk = [&](unsigned c) {
+            __syncwarp();
+            ring_fill(ring, rec, i0, i1, c + 3, lane);
+            cp_async_commit();
+            cp_async_wait<3>();
+            __syncwarp();
+        };
+
+        // prologue: records 0 .. DEPTH-1 into the look-ahead ring; the first window costs no write-out
+        enter_chunk(0);
+#pragma unroll
+        for (int s = 0; s < DEPTH; ++s)
+            if ((unsigned)s < cnt) produce(s, (unsigned)s);
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) qcur[k] = qn[0][k];
+
+        for (unsigned j = 0; j < cnt; j += DEPTH) {
+            // the producer is at record j + DEPTH .. j + 2 DEPTH - 1: all in one chunk (DEPTH divides kChunk)
+            const unsigned jp = j + DEPTH;
+            if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
+            if (jp + DEPTH <= cnt) {
+#pragma unroll
+                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, (jp + s) & kRingMask); }
+            } else {
+#pragma unroll
+                for (int s = 0; s < DEPTH; ++s) {
+                    if (j + s < cnt) consume(s);
+                    if (jp + s < cnt) produce(s, (jp + s) & kRingMask);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k)
+            if (act[k]) flush(k);
+        cp_async_wait<0>();
+    }
+}
+
+template <int SCT, int NSLOT, int DEPTH, int MINB>
+int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+                 int cls, int S) {
+    int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
+    int blocks = ctx->sm_count * per_sm;
+    unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
+    Counters *ctr = (Counters *)(w + ws.off_counters);
+    unsigned magicS = (1u << 20) / (unsigned)S + 1u;         // (x * magicS) >> 20 == x / S for x < 2^13, S <= 32
+    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB><<<blocks, kRunThreads, 0, ctx->stream>>>(
+        (const Rec<float> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
+        (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
+        (const float2 *)K, (float2 *)grid, bp.N, seg);
+    ctx->n_launches += 1;
+    WPG_CUDA(ctx, cudaGetLastError());
+    return WPG_OK;
+}
+
 template <typename T, int SCT, int NSLOT, int MINB>
 int launch_runs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                 int cls, int S) {
@@ -282,6 +479,19 @@ template <typename T>
 int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                  int cls, int S) {
     constexpr bool F = sizeof(T) == 4;
+    if (F && S % 2 == 0 && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
+        // fp32, even support: the pair gridder (S*S/2 pairs over 32 lanes)
+        const int np = S * S / 2, nslot = (np + 31) / 32;
+        if (S == 8) return launch_pairs<8, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 16) return launch_pairs<16, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 4) return launch_pairs<4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 1) return launch_pairs<0, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 2) return launch_pairs<0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 3) return launch_pairs<0, 3, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 4) return launch_pairs<0, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 6) return launch_pairs<0, 6, 1, 2>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 8) return launch_pairs<0, 8, 1, 1>(ctx, bp, ws, K, grid, w, cls, S);
+    }
     if (S == 8) return launch_runs<T, 8, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
     if (S == 16) return launch_runs<T, 16, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
     if (S == 4) return launch_runs<T, 4, 1, F ? 6 : 4>(ctx, bp, ws, K, grid, w, cls, S);
