@@ -65,8 +65,8 @@ int  wpg_version(void);
 
 /* Tuning knobs (all have defaults, 0 = default): "segment" = records per gridder work item;
  * "ctas_per_sm" = gridder CTAs per SM; "key_bits" = log2 cap of the binning sort-key space
- * (default 26: the key is (support class, j0v, parity of j0u, j0u >> 1) at full resolution unless that
- * exceeds the cap, then low bits of j0u >> 1 are dropped); "timing" 0/1 (see wpg_phase_ms).
+ * (default 26: the key is (support class, j0u, j0v) at full resolution unless that exceeds the cap,
+ * then low bits of j0v are dropped); "timing" 0/1 (see wpg_phase_ms).
  * Unknown name -> WPG_EINVAL. */
 int  wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value);
 
@@ -130,9 +130,8 @@ int  wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uvw, const f
 typedef struct {
     int64_t n_records;       /* valid visibilities = sorted records */
     int64_t n_keys;          /* number of sort keys = n_classes * keys_per_class */
-    int32_t n_classes;       /* distinct supports; with nuh = ceil(ceil(N/2) / 2^u_shift):
-                                key = (class * N + j0v) * 2 nuh + (j0u & 1) * nuh + ((j0u >> 1) >> u_shift) */
-    int32_t u_shift;
+    int32_t n_classes;       /* distinct supports; key = (class * N + j0u) * ceil(N / 2^key_shift) + (j0v >> key_shift) */
+    int32_t key_shift;
     int32_t record_bytes;    /* 16 (fp32) or 24 (fp64) */
     int32_t keys_per_class;
     int64_t off_records;     /* records sorted by key: {re, im, pos = j0u | j0v << 16, koff} */

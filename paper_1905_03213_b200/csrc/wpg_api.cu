@@ -63,6 +63,7 @@ extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
     else if (!strcmp(name, "key_bits")) { if (value != 0 && (value < 8 || value > 28)) return wpg_fail(ctx, WPG_EINVAL, "key_bits must be 0 or 8..28"); ctx->opt_key_bits = (int)value; }
     else if (!strcmp(name, "timing")) { ctx->opt_timing = value != 0; }
     else if (!strcmp(name, "no_pairs")) { ctx->opt_no_pairs = value != 0; }
+    else if (!strcmp(name, "variant")) { ctx->opt_variant = (int)value; }
     else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
     return WPG_OK;
 }
@@ -130,17 +131,16 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     bp->du = 1.0 / fov;
     bp->halfN = (double)(d->grid_N / 2);
     bp->ncls = (int)distinct.size();
-    // sort key = (class, j0v, j0u & 1, (j0u >> 1) >> ushift): a grid row is swept twice, even window starts
-    // first, then odd ones (the pair gridder keeps column ownership fixed within a parity); full resolution
-    // unless the key space would exceed 2^key_bits
+    // sort key = (class, j0u, j0v >> kshift): the visibilities are swept column by column of window starts,
+    // down the v axis, so a window that moves on leaves whole grid-row segments behind (contiguous write-outs)
+    // and keeps its column ownership (the parity of j0u is fixed within a sweep); full resolution unless the
+    // key space would exceed 2^key_bits
     const int64_t cap = (int64_t)1 << (ctx->opt_key_bits ? ctx->opt_key_bits : 26);
-    const int64_t halfcols = (d->grid_N + 1) / 2;
-    int ushift = 0;
-    while ((int64_t)bp->ncls * d->grid_N * 2 * ((halfcols + (1 << ushift) - 1) >> ushift) > cap && ushift < 13) ++ushift;
-    bp->ushift = ushift;
-    bp->nuh = (int)((halfcols + (1 << ushift) - 1) >> ushift);
-    bp->nug = 2 * bp->nuh;
-    bp->keys_per_class = (uint32_t)((int64_t)d->grid_N * bp->nug);
+    int kshift = 0;
+    while ((int64_t)bp->ncls * d->grid_N * (((int64_t)d->grid_N + (1 << kshift) - 1) >> kshift) > cap && kshift < 13) ++kshift;
+    bp->kshift = kshift;
+    bp->nkg = (d->grid_N + (1 << kshift) - 1) >> kshift;
+    bp->keys_per_class = (uint32_t)((int64_t)d->grid_N * bp->nkg);
     int64_t nkeys = (int64_t)bp->ncls * bp->keys_per_class;
     if (nkeys > ((int64_t)1 << 30)) return wpg_fail(ctx, WPG_EINVAL, "sort key space %lld too large", (long long)nkeys);
     bp->nkeys = (uint32_t)nkeys;
@@ -151,12 +151,9 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     size_t rec = prec == WPG_F32 ? sizeof(Rec<float>) : sizeof(Rec<double>);
     size_t o = 0;
     ws->off_counters = o; o += align_up(sizeof(Counters));
-    ws->off_hist = o;     o += align_up((size_t)(nkeys + 4) * 4);
+    ws->off_hist = o + 12; o += align_up((size_t)(nkeys + 8) * 4);    // bucket_start[0..nkeys]; [1..] is 16-byte aligned
     ws->off_blocksum = o; o += align_up((size_t)ws->nblocks_scan * 4 + 8);
     ws->off_fscale = o;   o += align_up((size_t)nchan * 8);
-    ws->off_key = o;      o += align_up((size_t)nvis * 4);
-    ws->off_rank = o;     o += align_up((size_t)nvis * 4);
-    ws->off_pre = o;      o += align_up((size_t)nvis * 8);
     ws->off_records = o;  o += align_up((size_t)nvis * rec);
     ws->total = o;
     return WPG_OK;
@@ -252,7 +249,7 @@ extern "C" int wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, con
     if (rc) return rc;
     if (info) {
         info->n_records = h.n_records; info->n_keys = ws.nkeys;
-        info->n_classes = bp.ncls; info->u_shift = bp.ushift;
+        info->n_classes = bp.ncls; info->key_shift = bp.kshift;
         info->record_bytes = prec == WPG_F32 ? 16 : 24; info->keys_per_class = (int32_t)bp.keys_per_class;
         info->off_records = (int64_t)ws.off_records; info->off_bucket_start = (int64_t)ws.off_hist;
     }

@@ -3,10 +3,10 @@
 //
 // The paper's analogue is the re-order of PAPER.md:62-78: count array C, exclusive prefix sum
 // Eq. (2), scatter — keyed there by baseline (Eq. 1) so that consecutive samples of a baseline hit
-// the same grid point.  Here the key is (support class, window start j0v, parity of
-// j0u, j0u >> 1), i.e. the visibilities are ordered by the grid point they hit, whatever baseline
-// they came from: runs of equal window start are what the gridder (wpg_grid.cu) accumulates in
-// registers, and within a (row, parity) sweep the window start moves by even steps.
+// the same grid point.  Here the key is (support class, window start j0u, j0v), i.e.
+// the visibilities are ordered by the grid point they hit, whatever baseline they came from: runs
+// of equal window start are what the gridder (wpg_grid.cu) accumulates in registers, and between
+// runs the window slides down the v axis at a fixed column.
 #include "wpg_common.h"
 
 namespace {
@@ -25,50 +25,52 @@ __global__ void chan_scale_kernel(const double *__restrict__ freq, int nchan, do
     if (c < nchan) fscale[c] = __ddiv_rn(freq[c], WPG_C0);
 }
 
-constexpr int kVpt = 4;            // visibilities per thread: four histogram atomics in flight per thread
+constexpr int kVpt = 4;            // visibilities per thread: four independent atomics in flight per thread
 
-// Pass 1: position math (fp64, G1-G3), validity (G4, R9), key, rank inside the key's bucket.
+// Position math (fp64, G1-G3) and validity (G4, R9) of visibility i; returns the sort key or WPG_NO_KEY.
+// The two passes below both evaluate it: recomputing is cheaper than a round trip of (key, position,
+// coefficient offset) through HBM, and the workspace holds nothing per visibility but the records.
+struct Located { unsigned key, pos, koff; int S; bool clamped, zero_weight; };
+__device__ __forceinline__ Located locate_vis(long long i, const double *__restrict__ uvw, const float *__restrict__ weight,
+                                              const double *__restrict__ fscale, const PlaneTab &T, const BinParams &P,
+                                              float *wt_out) {
+    Located L; L.key = WPG_NO_KEY; L.pos = L.koff = 0; L.S = 0; L.clamped = false;
+    long long row = i; int ch = 0;
+    if (P.nchan > 1) { row = i / P.nchan; ch = (int)(i - row * P.nchan); }
+    const float wt = __ldg(weight + i);
+    *wt_out = wt;
+    L.zero_weight = wt == 0.0f;
+    if (L.zero_weight) return L;
+    VisPos r = wpg_locate(__ldg(uvw + 3 * row), __ldg(uvw + 3 * row + 1), __ldg(uvw + 3 * row + 2),
+                          __ldg(fscale + ch), P, T);
+    if (!r.inside) return L;
+    L.S = r.S; L.clamped = r.clamped;
+    L.key = (unsigned)T.cls[r.p] * P.keys_per_class + (unsigned)r.j0u * (unsigned)P.nkg + ((unsigned)r.j0v >> P.kshift);
+    L.pos = (unsigned)r.j0u | ((unsigned)r.j0v << 16);
+    L.koff = wpg_koff(r, P, T);
+    return L;
+}
+
+// Pass 1: histogram of the keys (reductions without return value) and the wpg_stats counters.
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weight,
                  const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
-                 const __grid_constant__ BinParams P, Counters *__restrict__ ctr,
-                 unsigned *__restrict__ hist, unsigned *__restrict__ key_out,
-                 unsigned *__restrict__ rank_out, uint2 *__restrict__ pre_out) {
+                 const __grid_constant__ BinParams P, Counters *__restrict__ ctr, unsigned *__restrict__ hist) {
     const long long nvis = P.nrow * P.nchan;
     const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
     unsigned c_grid = 0, c_oob = 0, c_zero = 0, c_clamp = 0, c_upd = 0;
-    unsigned key[kVpt], rank[kVpt];
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
         const long long i = base + j * 256;
-        key[j] = WPG_NO_KEY;
         if (i < nvis) {
-            long long row = i; int ch = 0;
-            if (P.nchan > 1) { row = i / P.nchan; ch = (int)(i - row * P.nchan); }
-            if (__ldg(weight + i) == 0.0f) {
-                c_zero += 1;
-            } else {
-                VisPos r = wpg_locate(__ldg(uvw + 3 * row), __ldg(uvw + 3 * row + 1), __ldg(uvw + 3 * row + 2),
-                                      __ldg(fscale + ch), P, T);
-                if (!r.inside) {
-                    c_oob += 1;
-                } else {
-                    c_grid += 1; c_clamp += r.clamped; c_upd += r.S * r.S;
-                    key[j] = (unsigned)T.cls[r.p] * P.keys_per_class + (unsigned)r.j0v * (unsigned)P.nug +
-                             ((unsigned)r.j0u & 1u) * (unsigned)P.nuh + (((unsigned)r.j0u >> 1) >> P.ushift);
-                    pre_out[i] = make_uint2((unsigned)r.j0u | ((unsigned)r.j0v << 16), wpg_koff(r, P, T));
-                }
+            float wt;
+            const Located L = locate_vis(i, uvw, weight, fscale, T, P, &wt);
+            if (L.zero_weight) c_zero += 1;
+            else if (L.key == WPG_NO_KEY) c_oob += 1;
+            else {
+                c_grid += 1; c_clamp += L.clamped; c_upd += L.S * L.S;
+                asm volatile("red.global.add.u32 [%0], 1;" ::"l"(hist + L.key) : "memory");
             }
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) rank[j] = key[j] != WPG_NO_KEY ? atomicAdd(&hist[key[j]], 1u) : 0u;
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) {
-        const long long i = base + j * 256;
-        if (i < nvis) {
-            key_out[i] = key[j];
-            if (key[j] != WPG_NO_KEY) rank_out[i] = rank[j];
         }
     }
     warp_count(&ctr->n_gridded, c_grid);
@@ -168,33 +170,39 @@ __device__ __forceinline__ void store_rec(Rec<double> *dst, double re, double im
     *reinterpret_cast<uint2 *>(&dst->pos) = p;
 }
 
-// Pass 3: scatter into key order.  The record carries weight*vis (R9, natural weighting).
+// Pass 3: scatter into key order.  The slot of a visibility is the running cursor of its bucket
+// (bucket_start[key], advanced atomically: after this pass bucket_start[key] is the END of bucket key,
+// i.e. the array read one element earlier is the start array again — see wpg_launch_bin).  The record
+// carries weight*vis (R9, natural weighting).
 template <typename TT>
 __global__ void __launch_bounds__(256)
-scatter_kernel(const float2 *__restrict__ vis, const float *__restrict__ weight,
-               const unsigned *__restrict__ key, const unsigned *__restrict__ rank,
-               const uint2 *__restrict__ pre, const unsigned *__restrict__ bucket_start,
-               long long nvis, Rec<TT> *__restrict__ rec) {
+scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, const float *__restrict__ weight,
+               const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
+               const __grid_constant__ BinParams P, unsigned *__restrict__ cursor, Rec<TT> *__restrict__ rec) {
+    const long long nvis = P.nrow * P.nchan;
     const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
-    unsigned k[kVpt], dst[kVpt];
+    Located L[kVpt];
+    float wt[kVpt];
+    unsigned dst[kVpt];
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
         const long long i = base + j * 256;
-        k[j] = i < nvis ? __ldg(key + i) : WPG_NO_KEY;
+        L[j].key = WPG_NO_KEY; wt[j] = 0.f;
+        if (i < nvis) L[j] = locate_vis(i, uvw, weight, fscale, T, P, &wt[j]);
+    }
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) dst[j] = L[j].key != WPG_NO_KEY ? atomicAdd(cursor + L[j].key, 1u) : 0u;
+    float2 v[kVpt];
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) {
+        const long long i = base + j * 256;
+        v[j] = L[j].key != WPG_NO_KEY ? __ldg(vis + i) : make_float2(0.f, 0.f);
     }
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
-        const long long i = base + j * 256;
-        dst[j] = k[j] != WPG_NO_KEY ? __ldg(bucket_start + k[j]) + __ldg(rank + i) : 0u;
-    }
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) {
-        const long long i = base + j * 256;
-        if (k[j] == WPG_NO_KEY) continue;
-        float2 v = __ldg(vis + i);
-        TT w = (TT)__ldg(weight + i);
-        uint2 p = __ldg(pre + i);
-        store_rec(rec + dst[j], w * (TT)v.x, w * (TT)v.y, p);
+        if (L[j].key == WPG_NO_KEY) continue;
+        const TT w = (TT)wt[j];
+        store_rec(rec + dst[j], w * (TT)v[j].x, w * (TT)v[j].y, make_uint2(L[j].pos, L[j].koff));
     }
 }
 
@@ -205,24 +213,27 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
                    const WorkspaceLayout &ws, wpg_prec prec, char *w) {
     long long nvis = bp.nrow * bp.nchan;
     Counters *ctr = (Counters *)(w + ws.off_counters);
-    unsigned *hist = (unsigned *)(w + ws.off_hist);
+    // bucket_start[0 .. nkeys] lives at off_hist; the counts of key k are accumulated one element
+    // further on, at bucket_start[k + 1] (16-byte aligned for the scan: off_hist is 256-aligned + 12).
+    // The exclusive scan then leaves start[k] there, the scatter advances it to end[k] = start[k + 1],
+    // and bucket_start[0] stays 0: the array ends up as the start offsets of all nkeys + 1 buckets.
+    unsigned *bucket_start = (unsigned *)(w + ws.off_hist);
+    unsigned *hist = bucket_start + 1;
     unsigned *blocksum = (unsigned *)(w + ws.off_blocksum);
-    unsigned *key = (unsigned *)(w + ws.off_key), *rank = (unsigned *)(w + ws.off_rank);
-    uint2 *pre = (uint2 *)(w + ws.off_pre);
     cudaStream_t s = ctx->stream;
     double *fscale = (double *)(w + ws.off_fscale);
     unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
     chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale);
-    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist, key, rank, pre);
+    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
     scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
     scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     if (nb) {
         if (prec == WPG_F32)
-            scatter_kernel<float><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_weight, key, rank, pre, hist, nvis,
+            scatter_kernel<float><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, hist,
                                                       (Rec<float> *)(w + ws.off_records));
         else
-            scatter_kernel<double><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_weight, key, rank, pre, hist, nvis,
+            scatter_kernel<double><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, hist,
                                                        (Rec<double> *)(w + ws.off_records));
     }
     ctx->n_launches += nb ? 6 : 4;

@@ -30,11 +30,10 @@ struct BinParams {
     int nchan;
     int N, Q, Nw;
     double w_max, dw, du, halfN;   // dw = 2 w_max / Nw, du = 1/(N cell), halfN = N/2
-    int ushift;                    // the key drops this many low bits of j0u >> 1 (0 unless the key space is capped)
-    int nuh;                       // ceil(ceil(N/2) / 2^ushift): key columns per (grid row, parity of j0u)
-    int nug;                       // 2 * nuh: key columns per grid row
+    int kshift;                    // the key drops this many low bits of j0v (0 unless the key space is capped)
+    int nkg;                       // ceil(N / 2^kshift): keys per grid column
     int ncls;                      // number of sort classes (distinct supports)
-    uint32_t keys_per_class;       // N * nug; key = (cls * N + j0v) * nug + (j0u & 1) * nuh + ((j0u >> 1) >> ushift)
+    uint32_t keys_per_class;       // N * nkg; key = (cls * N + j0u) * nkg + (j0v >> kshift)
     uint32_t nkeys;                // ncls * keys_per_class
 };
 
@@ -52,7 +51,7 @@ struct Counters {
 };
 
 struct WorkspaceLayout {
-    size_t off_counters, off_key, off_rank, off_pre, off_records, off_hist, off_blocksum, off_fscale;
+    size_t off_counters, off_records, off_hist, off_blocksum, off_fscale;
     size_t total;
     uint32_t nkeys, nblocks_scan;
 };
@@ -67,6 +66,7 @@ struct wpg_ctx {
     int opt_ctas_per_sm = 0;  // gridder CTAs per SM, 0 = default
     int opt_key_bits = 0;     // cap of the sort key space (log2), 0 = default 26
     int opt_timing = 0;       // 1: wpg_grid brackets its phases with CUDA events
+    int opt_variant = 0;      // experimental kernel variant selector
     int opt_no_pairs = 0;     // 1: fp32 even supports also go through the run gridder (A/B comparison)
     // instrumentation
     int64_t n_launches = 0;   // kernels of this library launched so far

@@ -27,6 +27,10 @@ template <> struct Cplx<double> { using type = double2; };
 __device__ __forceinline__ void red_add(float2 *addr, float2 v) {
     asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(v.x), "f"(v.y) : "memory");
 }
+// two adjacent cells at once; addr must be 16-byte aligned
+__device__ __forceinline__ void red_add4(float2 *addr, float2 a, float2 b) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y) : "memory");
+}
 __device__ __forceinline__ void red_add(double2 *addr, double2 v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&addr->x), "d"(v.x) : "memory");
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&addr->y), "d"(v.y) : "memory");
@@ -264,8 +268,9 @@ grid_runs_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bu
 // ------------------------------------------------------------------------------------ pairs
 // fp32, even support.  A lane-slot owns a PAIR of horizontally adjacent cells: the cells of the window
 // whose row is congruent to rb and whose columns are congruent to (ra2 + par, ra2 + par + 1) modulo S,
-// par = parity of the window start j0u (the records come sorted by (row, parity, column), so within a
-// sweep the ownership never changes).  The two coefficients of a pair are adjacent and 16-byte aligned
+// par = parity of the window start j0u (the records come sorted by (column j0u, row j0v), so within a
+// sweep down the v axis the ownership never changes, and the cells a window leaves behind are whole
+// row segments: one contiguous 16-byte reduction per lane, 8 S bytes per row).  The two coefficients of a pair are adjacent and 16-byte aligned
 // in K[p][ov][ou][iv][:], so one LDG.128 feeds two updates.
 //
 // v*c = re*c + i*(im*c): the lane keeps A = sum re*c and B = sum im*c per cell (two packed FMAs per
@@ -364,8 +369,13 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
             const unsigned q = qcur[k];
             float2 *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
             const float2 a0 = unpack2(A0[k]), b0 = unpack2(B0[k]), a1 = unpack2(A1[k]), b1 = unpack2(B1[k]);
-            red_add(g, make_float2(a0.x - b0.y, a0.y + b0.x));
-            red_add(g + 1, make_float2(a1.x - b1.y, a1.y + b1.x));
+            const float2 o0 = make_float2(a0.x - b0.y, a0.y + b0.x), o1 = make_float2(a1.x - b1.y, a1.y + b1.x);
+            if ((reinterpret_cast<uintptr_t>(g) & 15) == 0) {
+                red_add4(g, o0, o1);
+            } else {
+                red_add(g, o0);
+                red_add(g + 1, o1);
+            }
         };
         // stage s <- record at ring slot `slot`: window offset, cell, coefficient loads
         auto produce = [&](int s, unsigned slot) {
@@ -482,7 +492,16 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     if (F && S % 2 == 0 && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp32, even support: the pair gridder (S*S/2 pairs over 32 lanes)
         const int np = S * S / 2, nslot = (np + 31) / 32;
-        if (S == 8) return launch_pairs<8, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 8) {
+            switch (ctx->opt_variant) {
+                case 1: return launch_pairs<8, 1, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
+                case 2: return launch_pairs<8, 1, 2, 4>(ctx, bp, ws, K, grid, w, cls, S);
+                case 3: return launch_pairs<8, 1, 8, 3>(ctx, bp, ws, K, grid, w, cls, S);
+                case 4: return launch_pairs<8, 1, 2, 6>(ctx, bp, ws, K, grid, w, cls, S);
+                case 5: return launch_pairs<8, 1, 4, 2>(ctx, bp, ws, K, grid, w, cls, S);
+                default: return launch_pairs<8, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+            }
+        }
         if (S == 16) return launch_pairs<16, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
         if (S == 4) return launch_pairs<4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 1) return launch_pairs<0, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);

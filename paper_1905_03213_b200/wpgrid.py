@@ -46,7 +46,7 @@ class Stats(ctypes.Structure):
 
 class BinInfo(ctypes.Structure):
     _fields_ = [("n_records", ctypes.c_int64), ("n_keys", ctypes.c_int64), ("n_classes", ctypes.c_int32),
-                ("u_shift", ctypes.c_int32), ("record_bytes", ctypes.c_int32), ("keys_per_class", ctypes.c_int32),
+                ("key_shift", ctypes.c_int32), ("record_bytes", ctypes.c_int32), ("keys_per_class", ctypes.c_int32),
                 ("off_records", ctypes.c_int64), ("off_bucket_start", ctypes.c_int64)]
 
     def as_dict(self):

@@ -134,16 +134,16 @@ def test_binning_records_match_oracle_index_map(ctx):
         ctx.set_option("key_bits", kb)
         ws, info, stats = ctx.bin(*d, ks)
         assert info["n_records"] == 20000 and info["n_classes"] == 1 and info["record_bytes"] == 16
-        ush = info["u_shift"]
-        nuh = (N // 2 + (1 << ush) - 1) >> ush
-        assert ush == (0 if kb == 0 else 4) and info["keys_per_class"] == N * 2 * nuh
+        ksh = info["key_shift"]
+        nkg = (N + (1 << ksh) - 1) >> ksh
+        assert ksh == (0 if kb == 0 else 4) and info["keys_per_class"] == N * nkg
         raw = ws.cpu().numpy()
         rec = raw[info["off_records"]:info["off_records"] + 16 * 20000].view(np.uint32).reshape(-1, 4)
         got = sorted((int(r[2]), int(r[3]), int(r[0]), int(r[1])) for r in rec)
         assert got == [tuple(int(x) for x in e) for e in exp]
-        # records are ordered by key = j0v * 2 nuh + (j0u & 1) * nuh + ((j0u >> 1) >> ush); bucket_start matches
+        # records are ordered by key = j0u * ceil(N / 2^ksh) + (j0v >> ksh); bucket_start matches that order
         ju = (rec[:, 2] & 0xFFFF).astype(np.int64); jv = (rec[:, 2] >> 16).astype(np.int64)
-        key = jv * 2 * nuh + (ju & 1) * nuh + ((ju >> 1) >> ush)
+        key = ju * nkg + (jv >> ksh)
         assert np.all(np.diff(key) >= 0)
         bs = raw[info["off_bucket_start"]:info["off_bucket_start"] + 4 * (info["n_keys"] + 1)].view(np.uint32)
         assert bs[0] == 0 and bs[-1] == 20000

@@ -67,7 +67,7 @@ def test_no_cpu_fallback_without_device(lib):
 def test_workspace_planning_is_host_logic(lib):
     d, sup, off, uni = wpgrid.make_desc(32, 4700.0, 8, 8, 2048, 8.3e-5)
     n = lib.wpg_grid_workspace_bytes(None, 10_000_000, 1, ctypes.byref(d), wpgrid.F32)
-    assert 10_000_000 * 32 < n < 10_000_000 * 40     # key 4 + rank 4 + pos,koff 8 + record 16 B per visibility (+ 16 MB of keys)
+    assert 10_000_000 * 16 < n < 10_000_000 * 19     # one 16 B record per visibility + 16.8 MB of bucket offsets
     # bad descriptors are refused (0 bytes)
     bad, *_ = wpgrid.make_desc(32, 4700.0, 7, 3, 2048, 8.3e-5)      # S*Q odd
     assert lib.wpg_grid_workspace_bytes(None, 1000, 1, ctypes.byref(bad), wpgrid.F32) == 0
