@@ -130,6 +130,11 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     double fov = (double)d->grid_N * d->cell;
     bp->du = 1.0 / fov;
     bp->halfN = (double)(d->grid_N / 2);
+    bp->rdu = 1.0 / bp->du;
+    bp->rdw = bp->dw > 0.0 ? 1.0 / bp->dw : 0.0;
+    bp->invQ = 1.0 / (double)d->oversample;
+    bp->qshift = -1;
+    for (int sft = 0; sft < 7; ++sft) if ((1 << sft) == d->oversample) bp->qshift = sft;
     bp->ncls = (int)distinct.size();
     // sort key = (class, j0u, j0v >> kshift): the visibilities are swept column by column of window starts,
     // down the v axis, so a window that moves on leaves whole grid-row segments behind (contiguous write-outs)
@@ -173,9 +178,12 @@ static int read_stats(wpg_ctx *ctx, const Counters *d_c, wpg_stats *out, Counter
     WPG_CUDA(ctx, cudaMemcpyAsync(&h, d_c, sizeof h, cudaMemcpyDeviceToHost, ctx->stream));
     WPG_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (out) {
-        out->n_gridded = (int64_t)h.n_gridded; out->n_skipped_oob = (int64_t)h.n_skipped_oob;
-        out->n_skipped_zero_weight = (int64_t)h.n_skipped_zero_weight;
-        out->n_clamped_w = (int64_t)h.n_clamped_w; out->n_updates = (int64_t)h.n_updates;
+        memset(out, 0, sizeof *out);
+        for (int s = 0; s < kStatSlots; ++s) {
+            out->n_gridded += (int64_t)h.n_gridded[s]; out->n_skipped_oob += (int64_t)h.n_skipped_oob[s];
+            out->n_skipped_zero_weight += (int64_t)h.n_skipped_zero_weight[s];
+            out->n_clamped_w += (int64_t)h.n_clamped_w[s]; out->n_updates += (int64_t)h.n_updates[s];
+        }
     }
     if (h_opt) *h_opt = h;
     return WPG_OK;

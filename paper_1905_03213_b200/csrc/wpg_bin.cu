@@ -13,9 +13,25 @@ namespace {
 
 constexpr int kScanBlock = 4096;   // keys per scan block (1024 threads x 4)
 
-__device__ __forceinline__ void warp_count(unsigned long long *dst, unsigned v) {
-    unsigned s = __reduce_add_sync(0xffffffffu, v);
-    if ((threadIdx.x & 31) == 0 && s) atomicAdd(dst, (unsigned long long)s);
+// Block totals of the five wpg_stats counters: warp sums, shared memory, one reduction per counter and block.
+__device__ __forceinline__ void block_count(Counters *ctr, unsigned c_grid, unsigned c_oob, unsigned c_zero,
+                                            unsigned c_clamp, unsigned c_upd) {
+    __shared__ unsigned s_cnt[5];
+    if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    unsigned v[5] = {c_grid, c_oob, c_zero, c_clamp, c_upd};
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+        const unsigned t = __reduce_add_sync(0xffffffffu, v[k]);
+        if ((threadIdx.x & 31) == 0 && t) atomicAdd(&s_cnt[k], t);
+    }
+    __syncthreads();
+    if (threadIdx.x < 5 && s_cnt[threadIdx.x]) {
+        unsigned long long *dst = threadIdx.x == 0 ? ctr->n_gridded : threadIdx.x == 1 ? ctr->n_skipped_oob
+                                : threadIdx.x == 2 ? ctr->n_skipped_zero_weight : threadIdx.x == 3 ? ctr->n_clamped_w
+                                : ctr->n_updates;
+        atomicAdd(dst + blockIdx.x % kStatSlots, (unsigned long long)s_cnt[threadIdx.x]);
+    }
 }
 
 // Pass 0: f[ch] = freq[ch] / c0 (G1), once per channel instead of once per visibility.  Same IEEE
@@ -31,21 +47,40 @@ constexpr int kVpt = 4;            // visibilities per thread: four independent 
 // The two passes below both evaluate it: recomputing is cheaper than a round trip of (key, position,
 // coefficient offset) through HBM, and the workspace holds nothing per visibility but the records.
 struct Located { unsigned key, pos, koff; int S; bool clamped, zero_weight; };
-__device__ __forceinline__ Located locate_vis(long long i, const double *__restrict__ uvw, const float *__restrict__ weight,
-                                              const double *__restrict__ fscale, const PlaneTab &T, const BinParams &P,
-                                              float *wt_out) {
+struct RawVis { double um, vm, wm, f; float wt; bool valid; };
+
+// All global loads of one visibility, issued before any arithmetic so that a thread has the inputs of
+// its kVpt visibilities in flight at once (the passes are latency-bound otherwise).
+__device__ __forceinline__ RawVis load_vis(long long i, long long nvis, const double *__restrict__ uvw,
+                                           const float *__restrict__ weight, const double *__restrict__ fscale,
+                                           const BinParams &P) {
+    RawVis r; r.valid = i < nvis; r.um = r.vm = r.wm = 0.0; r.f = 0.0; r.wt = 0.f;
+    if (r.valid) {
+        long long row = i; int ch = 0;
+        if (P.nchan > 1) {             // nrow * nchan < 2^32 (wpg_make_plan): 32-bit division
+            const unsigned r32 = (unsigned)i / (unsigned)P.nchan;
+            row = r32; ch = (int)((unsigned)i - r32 * (unsigned)P.nchan);
+        }
+        r.wt = __ldg(weight + i);
+        r.um = __ldg(uvw + 3 * row); r.vm = __ldg(uvw + 3 * row + 1); r.wm = __ldg(uvw + 3 * row + 2);
+        r.f = __ldg(fscale + ch);
+    }
+    return r;
+}
+// Keeps the compiler from consuming a loaded value (and so waiting for it) before the loads that
+// follow in program order have been issued.
+__device__ __forceinline__ void use_after_here(RawVis &r) {
+    asm volatile("" : "+f"(r.wt), "+d"(r.um), "+d"(r.vm), "+d"(r.wm));
+}
+
+__device__ __forceinline__ Located locate_vis(const RawVis &v, const SmemPlaneTab &T, const BinParams &P) {
     Located L; L.key = WPG_NO_KEY; L.pos = L.koff = 0; L.S = 0; L.clamped = false;
-    long long row = i; int ch = 0;
-    if (P.nchan > 1) { row = i / P.nchan; ch = (int)(i - row * P.nchan); }
-    const float wt = __ldg(weight + i);
-    *wt_out = wt;
-    L.zero_weight = wt == 0.0f;
-    if (L.zero_weight) return L;
-    VisPos r = wpg_locate(__ldg(uvw + 3 * row), __ldg(uvw + 3 * row + 1), __ldg(uvw + 3 * row + 2),
-                          __ldg(fscale + ch), P, T);
+    L.zero_weight = v.valid && v.wt == 0.0f;
+    if (!v.valid || L.zero_weight) return L;
+    VisPos r = wpg_locate(v.um, v.vm, v.wm, v.f, P, T);
     if (!r.inside) return L;
     L.S = r.S; L.clamped = r.clamped;
-    L.key = (unsigned)T.cls[r.p] * P.keys_per_class + (unsigned)r.j0u * (unsigned)P.nkg + ((unsigned)r.j0v >> P.kshift);
+    L.key = (unsigned)T.cls(r.p) * P.keys_per_class + (unsigned)r.j0u * (unsigned)P.nkg + ((unsigned)r.j0v >> P.kshift);
     L.pos = (unsigned)r.j0u | ((unsigned)r.j0v << 16);
     L.koff = wpg_koff(r, P, T);
     return L;
@@ -55,29 +90,33 @@ __device__ __forceinline__ Located locate_vis(long long i, const double *__restr
 __global__ void __launch_bounds__(256)
 bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weight,
                  const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
-                 const __grid_constant__ BinParams P, Counters *__restrict__ ctr, unsigned *__restrict__ hist) {
+                 const __grid_constant__ BinParams P, Counters *__restrict__ ctr, unsigned *__restrict__ hist, int dbg) {
     const long long nvis = P.nrow * P.nchan;
     const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
     unsigned c_grid = 0, c_oob = 0, c_zero = 0, c_clamp = 0, c_upd = 0;
+    __shared__ uint2 s_tab[WPG_MAX_NW];
+    const SmemPlaneTab ST{s_tab};
+    RawVis raw[kVpt];
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) raw[j] = load_vis(base + j * 256, nvis, uvw, weight, fscale, P);
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
+    wpg_stage_planetab(s_tab, T, P.Nw);
+    __syncthreads();
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
-        const long long i = base + j * 256;
-        if (i < nvis) {
-            float wt;
-            const Located L = locate_vis(i, uvw, weight, fscale, T, P, &wt);
-            if (L.zero_weight) c_zero += 1;
-            else if (L.key == WPG_NO_KEY) c_oob += 1;
-            else {
-                c_grid += 1; c_clamp += L.clamped; c_upd += L.S * L.S;
-                asm volatile("red.global.add.u32 [%0], 1;" ::"l"(hist + L.key) : "memory");
-            }
+        if (!raw[j].valid) continue;
+        Located L;
+        if (dbg & 32) { L.zero_weight = false; L.key = (unsigned)(__double_as_longlong(raw[j].um) >> 20) % P.nkeys; L.S = 8; L.clamped = false; }
+        else L = locate_vis(raw[j], ST, P);
+        if (L.zero_weight) c_zero += 1;
+        else if (L.key == WPG_NO_KEY) c_oob += 1;
+        else {
+            c_grid += 1; c_clamp += L.clamped; c_upd += L.S * L.S;
+            if (!(dbg & 16)) asm volatile("red.global.add.u32 [%0], 1;" ::"l"(hist + L.key) : "memory");
         }
     }
-    warp_count(&ctr->n_gridded, c_grid);
-    warp_count(&ctr->n_skipped_oob, c_oob);
-    warp_count(&ctr->n_skipped_zero_weight, c_zero);
-    warp_count(&ctr->n_clamped_w, c_clamp);
-    warp_count(&ctr->n_updates, c_upd);
+    block_count(ctr, c_grid, c_oob, c_zero, c_clamp, c_upd);
 }
 
 // Block-wide inclusive scan of one unsigned per thread (1024 threads); returns the inclusive
@@ -184,20 +223,26 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
     Located L[kVpt];
     float wt[kVpt];
     unsigned dst[kVpt];
+    float2 v[kVpt];
+    __shared__ uint2 s_tab[WPG_MAX_NW];
+    const SmemPlaneTab ST{s_tab};
+    {
+        RawVis raw[kVpt];
 #pragma unroll
-    for (int j = 0; j < kVpt; ++j) {
-        const long long i = base + j * 256;
-        L[j].key = WPG_NO_KEY; wt[j] = 0.f;
-        if (i < nvis) L[j] = locate_vis(i, uvw, weight, fscale, T, P, &wt[j]);
+        for (int j = 0; j < kVpt; ++j) {
+            const long long i = base + j * 256;
+            raw[j] = load_vis(i, nvis, uvw, weight, fscale, P);
+            v[j] = i < nvis ? __ldg(vis + i) : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
+        wpg_stage_planetab(s_tab, T, P.Nw);
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < kVpt; ++j) { L[j] = locate_vis(raw[j], ST, P); wt[j] = raw[j].wt; }
     }
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) dst[j] = L[j].key != WPG_NO_KEY ? atomicAdd(cursor + L[j].key, 1u) : 0u;
-    float2 v[kVpt];
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) {
-        const long long i = base + j * 256;
-        v[j] = L[j].key != WPG_NO_KEY ? __ldg(vis + i) : make_float2(0.f, 0.f);
-    }
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
         if (L[j].key == WPG_NO_KEY) continue;
@@ -224,7 +269,7 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
     double *fscale = (double *)(w + ws.off_fscale);
     unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
     chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale);
-    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
+    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist, ctx->opt_variant);
     scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
     scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);

@@ -30,6 +30,8 @@ struct BinParams {
     int nchan;
     int N, Q, Nw;
     double w_max, dw, du, halfN;   // dw = 2 w_max / Nw, du = 1/(N cell), halfN = N/2
+    double rdu, rdw, invQ;         // RN(1/du), RN(1/dw), 1/Q (wpg_div_const, floor division by Q)
+    int qshift;                    // log2 Q if Q is a power of two, else -1
     int kshift;                    // the key drops this many low bits of j0v (0 unless the key space is capped)
     int nkg;                       // ceil(N / 2^kshift): keys per grid column
     int ncls;                      // number of sort classes (distinct supports)
@@ -45,11 +47,14 @@ static_assert(sizeof(Rec<double>) == 24, "fp64 record is 24 B");
 
 // Device counters block at the head of the workspace.
 struct Counters {
-    unsigned long long n_gridded, n_skipped_oob, n_skipped_zero_weight, n_clamped_w, n_updates;
+    // wpg_stats counters, each spread over kStatSlots addresses (blocks add to slot blockIdx % kStatSlots:
+    // tens of thousands of reductions on ONE address serialise in L2); the host sums the slots
+    unsigned long long n_gridded[16], n_skipped_oob[16], n_skipped_zero_weight[16], n_clamped_w[16], n_updates[16];
     unsigned int n_records, pad0, pad1, pad2;
     unsigned int cursor[WPG_MAX_CLS];   // work-item cursors of the gridder launches (one per sort class)
 };
 
+constexpr int kStatSlots = 16;
 struct WorkspaceLayout {
     size_t off_counters, off_records, off_hist, off_blocksum, off_fscale;
     size_t total;
@@ -111,35 +116,88 @@ int wpg_launch_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const
 #ifdef __CUDACC__
 struct VisPos { int p, S, j0u, j0v, ou, ov; bool inside, clamped; };
 
-__device__ __forceinline__ void wpg_axis(double x_lambda, const BinParams &P, int S, int &j0, int &o) {
-    double x = __dadd_rn(__ddiv_rn(x_lambda, P.du), P.halfN);
-    long long X = (long long)floor(__dadd_rn(__dmul_rn(x, (double)P.Q), 0.5));
-    long long Y = X - (long long)((S - 2) * P.Q / 2);
-    long long q = Y / P.Q;
-    if ((Y % P.Q != 0) && (Y < 0)) q -= 1;           // floor division
-    j0 = (int)max(min(q, (long long)(1 << 20)), (long long)(-(1 << 20)));
-    o = (int)(Y - q * P.Q);
+// a / b for a divisor that is a launch constant, rb = RN(1 / b) computed on the host: the product, one exact
+// residual and one correction (Markstein's sequence) give the correctly rounded quotient, i.e. the value
+// of __ddiv_rn(a, b), in three instructions instead of the division's reciprocal iteration.  *t_guard: the
+// callers take floor() of a value derived from the quotient; if that value sits within a few ulps of an
+// integer they recompute with the IEEE division (never observed to differ; keeps G6 unconditional).
+__device__ __forceinline__ double wpg_div_const(double a, double b, double rb) {
+    const double q0 = __dmul_rn(a, rb);
+    const double rem = __fma_rn(-b, q0, a);
+    return __fma_rn(rem, rb, q0);
+}
+__device__ __forceinline__ bool wpg_near_integer(double t) {
+    const double fr = t - floor(t);
+    const double eps = fabs(t) * 1e-15 + 1e-300;
+    return fr < eps || 1.0 - fr < eps;
 }
 
+__device__ __forceinline__ void wpg_axis(double x_lambda, const BinParams &P, int S, int &j0, int &o) {
+    double x = __dadd_rn(wpg_div_const(x_lambda, P.du, P.rdu), P.halfN);
+    double t = __dadd_rn(__dmul_rn(x, (double)P.Q), 0.5);
+    if (wpg_near_integer(t)) {                                   // practically never
+        x = __dadd_rn(__ddiv_rn(x_lambda, P.du), P.halfN);
+        t = __dadd_rn(__dmul_rn(x, (double)P.Q), 0.5);
+    }
+    if (!(fabs(t) < 1073741824.0)) { j0 = -(1 << 20); o = 0; return; }      // far outside any grid (also NaN)
+    const int X = __double2int_rd(t);                            // floor
+    const int Y = X - (S - 2) * P.Q / 2;
+    int q;
+    if (P.qshift >= 0) {                                         // Q = 2^qshift: floor division is a shift
+        q = Y >> P.qshift;
+    } else {
+        q = __double2int_rd((double)Y * P.invQ);                 // within 1 of floor(Y / Q); fixed up below
+        int r = Y - q * P.Q;
+        q += r >= P.Q ? 1 : (r < 0 ? -1 : 0);
+    }
+    j0 = max(min(q, 1 << 20), -(1 << 20));
+    o = Y - q * P.Q;
+}
+
+// Plane lookup: `tab` is either the PlaneTab itself (kernel parameter, constant bank — fine when the
+// index is warp-uniform or rarely used) or its packed copy in shared memory (SmemPlaneTab: the binning
+// passes index it with a different plane in every lane, which the constant cache would serialise).
+struct SmemPlaneTab {
+    const uint2 *e;        // e[p] = {element offset of plane p, S_p | class << 8}
+    __device__ __forceinline__ int S(int p) const { return (int)(e[p].y & 0xFFu); }
+    __device__ __forceinline__ int cls(int p) const { return (int)(e[p].y >> 8); }
+    __device__ __forceinline__ int off(int p) const { return (int)e[p].x; }
+};
+struct ParamPlaneTab {
+    const PlaneTab &t;
+    __device__ __forceinline__ int S(int p) const { return t.S[p]; }
+    __device__ __forceinline__ int cls(int p) const { return t.cls[p]; }
+    __device__ __forceinline__ int off(int p) const { return t.off[p]; }
+};
+// fills the shared copy (call from every thread of the block, then __syncthreads)
+__device__ __forceinline__ void wpg_stage_planetab(uint2 *dst, const PlaneTab &T, int Nw) {
+    for (int p = threadIdx.x; p < Nw; p += blockDim.x) dst[p] = make_uint2((unsigned)T.off[p], (unsigned)T.S[p] | ((unsigned)T.cls[p] << 8));
+}
+
+template <typename Tab>
 __device__ __forceinline__ VisPos wpg_locate(double um, double vm, double wm, double f,
-                                             const BinParams &P, const PlaneTab &T) {
+                                             const BinParams &P, const Tab &T) {
     VisPos r;
     double u = __dmul_rn(um, f), v = __dmul_rn(vm, f), w = __dmul_rn(wm, f);     // G1
     r.clamped = fabs(w) > P.w_max;                                               // G2
     int p = 0;
     if (P.dw > 0.0) {
-        double fp = floor(__ddiv_rn(__dadd_rn(w, P.w_max), P.dw));
+        const double ws = __dadd_rn(w, P.w_max);
+        double qd = wpg_div_const(ws, P.dw, P.rdw);
+        if (wpg_near_integer(qd)) qd = __ddiv_rn(ws, P.dw);
+        double fp = floor(qd);
         p = fp < 0.0 ? 0 : (fp > (double)(P.Nw - 1) ? P.Nw - 1 : (int)fp);
     }
     r.p = p;
-    r.S = T.S[p];
+    r.S = T.S(p);
     wpg_axis(u, P, r.S, r.j0u, r.ou);                                            // G3
     wpg_axis(v, P, r.S, r.j0v, r.ov);
     r.inside = r.j0u >= 0 && r.j0v >= 0 && r.j0u + r.S <= P.N && r.j0v + r.S <= P.N;   // G4
     return r;
 }
 
-__device__ __forceinline__ uint32_t wpg_koff(const VisPos &r, const BinParams &P, const PlaneTab &T) {
-    return (uint32_t)(T.off[r.p] + (r.ov * P.Q + r.ou) * r.S * r.S);
+template <typename Tab>
+__device__ __forceinline__ uint32_t wpg_koff(const VisPos &r, const BinParams &P, const Tab &T) {
+    return (uint32_t)(T.off(r.p) + (r.ov * P.Q + r.ou) * r.S * r.S);
 }
 #endif

@@ -73,12 +73,13 @@ grid_naive_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw
         long long row = i / P.nchan;
         int ch = (int)(i - row * P.nchan);
         double f = __ddiv_rn(freq[ch], WPG_C0);
-        VisPos r = wpg_locate(uvw[3 * row], uvw[3 * row + 1], uvw[3 * row + 2], f, P, Tb);
+        const ParamPlaneTab PT{Tb};
+        VisPos r = wpg_locate(uvw[3 * row], uvw[3 * row + 1], uvw[3 * row + 2], f, P, PT);
         if (!r.inside) { c_oob++; continue; }
         c_grid++; c_clamp += r.clamped; c_upd += r.S * r.S;
         float2 v = vis[i];
         T re = (T)wt * (T)v.x, im = (T)wt * (T)v.y;
-        const C *Ks = K + wpg_koff(r, P, Tb);
+        const C *Ks = K + wpg_koff(r, P, PT);
         int S = r.S, S2 = S * S;
         for (int c = lane; c < S2; c += 32) {
             int iv = c / S, iu = c - iv * S;
@@ -89,11 +90,11 @@ grid_naive_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw
         }
     }
     if (lane == 0) {
-        if (c_grid) atomicAdd(&ctr->n_gridded, c_grid);
-        if (c_oob) atomicAdd(&ctr->n_skipped_oob, c_oob);
-        if (c_zero) atomicAdd(&ctr->n_skipped_zero_weight, c_zero);
-        if (c_clamp) atomicAdd(&ctr->n_clamped_w, c_clamp);
-        if (c_upd) atomicAdd(&ctr->n_updates, c_upd);
+        if (c_grid) atomicAdd(&ctr->n_gridded[blockIdx.x % kStatSlots], c_grid);
+        if (c_oob) atomicAdd(&ctr->n_skipped_oob[blockIdx.x % kStatSlots], c_oob);
+        if (c_zero) atomicAdd(&ctr->n_skipped_zero_weight[blockIdx.x % kStatSlots], c_zero);
+        if (c_clamp) atomicAdd(&ctr->n_clamped_w[blockIdx.x % kStatSlots], c_clamp);
+        if (c_upd) atomicAdd(&ctr->n_updates[blockIdx.x % kStatSlots], c_upd);
     }
 }
 
