@@ -87,10 +87,10 @@ __device__ __forceinline__ Located locate_vis(const RawVis &v, const SmemPlaneTa
 }
 
 // Pass 1: histogram of the keys (reductions without return value) and the wpg_stats counters.
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weight,
                  const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
-                 const __grid_constant__ BinParams P, Counters *__restrict__ ctr, unsigned *__restrict__ hist, int dbg) {
+                 const __grid_constant__ BinParams P, Counters *__restrict__ ctr, unsigned *__restrict__ hist) {
     const long long nvis = P.nrow * P.nchan;
     const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
     unsigned c_grid = 0, c_oob = 0, c_zero = 0, c_clamp = 0, c_upd = 0;
@@ -106,14 +106,12 @@ bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weigh
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
         if (!raw[j].valid) continue;
-        Located L;
-        if (dbg & 32) { L.zero_weight = false; L.key = (unsigned)(__double_as_longlong(raw[j].um) >> 20) % P.nkeys; L.S = 8; L.clamped = false; }
-        else L = locate_vis(raw[j], ST, P);
+        const Located L = locate_vis(raw[j], ST, P);
         if (L.zero_weight) c_zero += 1;
         else if (L.key == WPG_NO_KEY) c_oob += 1;
         else {
             c_grid += 1; c_clamp += L.clamped; c_upd += L.S * L.S;
-            if (!(dbg & 16)) asm volatile("red.global.add.u32 [%0], 1;" ::"l"(hist + L.key) : "memory");
+            asm volatile("red.global.add.u32 [%0], 1;" ::"l"(hist + L.key) : "memory");
         }
     }
     block_count(ctr, c_grid, c_oob, c_zero, c_clamp, c_upd);
@@ -214,7 +212,7 @@ __device__ __forceinline__ void store_rec(Rec<double> *dst, double re, double im
 // i.e. the array read one element earlier is the start array again — see wpg_launch_bin).  The record
 // carries weight*vis (R9, natural weighting).
 template <typename TT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 4)
 scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, const float *__restrict__ weight,
                const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
                const __grid_constant__ BinParams P, unsigned *__restrict__ cursor, Rec<TT> *__restrict__ rec) {
@@ -269,7 +267,7 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
     double *fscale = (double *)(w + ws.off_fscale);
     unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
     chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale);
-    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist, ctx->opt_variant);
+    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
     scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
     scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);

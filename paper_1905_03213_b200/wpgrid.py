@@ -11,7 +11,7 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libwpgrid.so")
+LIB_PATH = os.environ.get("WPGRID_LIB") or os.path.join(_HERE, "libwpgrid.so")   # override: an alternative build
 
 F32, F64 = 0, 1
 OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
