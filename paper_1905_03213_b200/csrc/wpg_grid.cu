@@ -274,9 +274,9 @@ grid_runs_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bu
 // row segments: one contiguous 16-byte reduction per lane, 8 S bytes per row).  The two coefficients of a pair are adjacent and 16-byte aligned
 // in K[p][ov][ou][iv][:], so one LDG.128 feeds two updates.
 //
-// v*c = re*c + i*(im*c): the lane keeps A = sum re*c and B = sum im*c per cell (two packed FMAs per
-// update, the coefficient pair used as loaded, (re,re) and (im,im) formed once per record) and
-// combines them when it writes the cell out: grid += (A.x - B.y, A.y + B.x).
+// v*c = (re, im)*c.x + (-im, re)*c.y: two packed FMAs per update; (re, im) and (-im, re) are formed once per
+// record and the coefficient components enter as broadcast scalars, so the accumulators are the cell
+// sums themselves and a pair is written out as one 16-byte reduction.
 //
 // The coefficient loads run DEPTH records ahead of their use in a register ring (statically indexed,
 // the record loop is unrolled by DEPTH): the slice of a record is picked at random from a stack that
@@ -354,100 +354,118 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
 
         __syncwarp();                          // the previous item's ring reads are done
 #pragma unroll
-        for (unsigned c = 0; c < 3; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
+        for (unsigned c = 0; c < 2; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
 
-        U64 A0[NSLOT], B0[NSLOT], A1[NSLOT], B1[NSLOT];     // accumulators of the pair's two cells
+        U64 acc0[NSLOT], acc1[NSLOT];                       // (re, im) sums of the pair's two cells
         unsigned qcur[NSLOT];                               // (column | row << 16) of the pair's first cell
 #pragma unroll
-        for (int k = 0; k < NSLOT; ++k) A0[k] = B0[k] = A1[k] = B1[k] = 0ull;
+        for (int k = 0; k < NSLOT; ++k) { acc0[k] = acc1[k] = 0ull; qcur[k] = 0xFFFFFFFFu; }
 
-        // look-ahead ring (registers)
+        // look-ahead ring (registers): coefficients, visibility, window start and "first record of a
+        // window" flag of the DEPTH records in flight
         U64 c0[DEPTH][NSLOT], c1[DEPTH][NSLOT];
-        unsigned qn[DEPTH][NSLOT];
-        float re[DEPTH], im[DEPTH];
+        U64 vis[DEPTH];
+        bool nw[DEPTH];
+        // producer state: the window of the record loaded last and the lane-slot's coefficient pointer in it
+        unsigned posP = 0xFFFFFFFFu;
+        const float2 *KcP[NSLOT];
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) KcP[k] = K;
 
+        // Write the pair out and clear its sums.  One asm statement with the accumulators as read-write
+        // operands: the cleared value then lives in the SAME register as the sum (a separate "acc = 0"
+        // makes the compiler keep two copies alive and pay moves for it on every record).
         auto flush = [&](int k) {
             const unsigned q = qcur[k];
             float2 *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
-            const float2 a0 = unpack2(A0[k]), b0 = unpack2(B0[k]), a1 = unpack2(A1[k]), b1 = unpack2(B1[k]);
-            const float2 o0 = make_float2(a0.x - b0.y, a0.y + b0.x), o1 = make_float2(a1.x - b1.y, a1.y + b1.x);
-            if ((reinterpret_cast<uintptr_t>(g) & 15) == 0) {
-                red_add4(g, o0, o1);
-            } else {
-                red_add(g, o0);
-                red_add(g + 1, o1);
-            }
+            // (two 8-byte reductions rather than one 16-byte red.v4: the latter wants both sums in one aligned
+            // register quad, which costs register moves on every record)
+            asm volatile("{ .reg .f32 a, b, c, d;\n\t"
+                         "mov.b64 {a, b}, %0; mov.b64 {c, d}, %1;\n\t"
+                         "red.global.add.v2.f32 [%2], {a, b};\n\t"
+                         "red.global.add.v2.f32 [%2 + 8], {c, d};\n\t"
+                         "mov.b64 %0, 0; mov.b64 %1, 0; }"
+                         : "+l"(acc0[k]), "+l"(acc1[k]) : "l"(g) : "memory");
         };
-        // stage s <- record at ring slot `slot`: window offset, cell, coefficient loads
-        auto produce = [&](int s, unsigned slot) {
-            float r_, i_; unsigned pos, koff;
-            ring_get(ring, slot, r_, i_, pos, koff);
-            re[s] = r_; im[s] = i_;
-#pragma unroll
-            for (int k = 0; k < NSLOT; ++k) {
-                const unsigned d = offset_in_window(pos, k);
-                qn[s][k] = act[k] ? pos + d : 0xFFFFFFFFu;
-                const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
-                ldg128(K + (koff + (act[k] ? coff : 0u)), c0[s][k], c1[s][k]);
-            }
-        };
-        auto consume = [&](int s) {
-            bool any = false;
-#pragma unroll
-            for (int k = 0; k < NSLOT; ++k) any |= qn[s][k] != qcur[k];
-            if (__any_sync(0xffffffffu, any)) {
+        // stage s <- record rp[0]: coefficient loads; the lane's offset inside the slice changes only
+        // with the window (warp-uniform branch, taken once per run of equal window starts)
+        auto produce = [&](int s, const Rec<float> *rp) {
+            // two 8-byte reads: (re, im) stays in its register pair until the record is consumed,
+            // (pos, koff) is used up at once (the consumer re-reads pos on the rare path)
+            vis[s] = *reinterpret_cast<const U64 *>(rp);
+            const uint2 pk = *reinterpret_cast<const uint2 *>(&rp->pos);
+            const unsigned pos = pk.x, koff = pk.y;
+            nw[s] = __any_sync(0xffffffffu, pos != posP);
+            if (__builtin_expect(nw[s], 0)) {
 #pragma unroll
                 for (int k = 0; k < NSLOT; ++k) {
-                    if (qn[s][k] != qcur[k]) {
-                        flush(k);
-                        A0[k] = B0[k] = A1[k] = B1[k] = 0ull;
+                    const unsigned d = offset_in_window(pos, k);
+                    const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
+                    KcP[k] = K + (act[k] ? coff : 0u);
+                }
+                posP = pos;
+            }
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) ldg128(KcP[k] + koff, c0[s][k], c1[s][k]);
+        };
+        auto consume = [&](int s, const Rec<float> *rc) {
+            if (__builtin_expect(nw[s], 0)) {  // the window moved: lane-slots whose cells changed write out
+                const unsigned pos = rc->pos;
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    const unsigned qn = act[k] ? pos + offset_in_window(pos, k) : 0xFFFFFFFFu;
+                    if (qn != qcur[k]) {
+                        if (qcur[k] != 0xFFFFFFFFu) flush(k);      // (the sums are zero before the first window)
+                        asm volatile("mov.b32 %0, %1;" : "+r"(qcur[k]) : "r"(qn));    // tied: no second copy of qcur
                     }
-                    qcur[k] = qn[s][k];
                 }
             }
-            const U64 rr = pack2(re[s], re[s]), ii = pack2(im[s], im[s]);
+            // acc += v * c = (re, im) * c.x + (-im, re) * c.y: the visibility pairs are formed once per record,
+            // the coefficient components enter as broadcast scalars
+            const float2 vv = unpack2(vis[s]);
+            const U64 v1 = vis[s], v2 = pack2(-vv.y, vv.x);
 #pragma unroll
             for (int k = 0; k < NSLOT; ++k) {
-                fma2(A0[k], c0[s][k], rr); fma2(B0[k], c0[s][k], ii);
-                fma2(A1[k], c1[s][k], rr); fma2(B1[k], c1[s][k], ii);
+                const float2 k0 = unpack2(c0[s][k]), k1 = unpack2(c1[s][k]);
+                fma2(acc0[k], v1, pack2(k0.x, k0.x)); fma2(acc0[k], v2, pack2(k0.y, k0.y));
+                fma2(acc1[k], v1, pack2(k1.x, k1.x)); fma2(acc1[k], v2, pack2(k1.y, k1.y));
             }
         };
-        // entering chunk c of the PRODUCER: request chunk c + 2 (its slot held chunk c - 2, whose records
-        // are in registers or done), make chunks <= c visible
+        // entering chunk c of the PRODUCER: request chunk c + 2 (its slot held chunk c - 2; the consumer, DEPTH
+        // records behind, may still re-read window starts of chunk c - 1), make chunks <= c visible
         auto enter_chunk = [&](unsigned c) {
             __syncwarp();
-            ring_fill(ring, rec, i0, i1, c + 3, lane);
+            ring_fill(ring, rec, i0, i1, c + 2, lane);
             cp_async_commit();
-            cp_async_wait<3>();
+            cp_async_wait<2>();
             __syncwarp();
         };
 
-        // prologue: records 0 .. DEPTH-1 into the look-ahead ring; the first window costs no write-out
+        // prologue: records 0 .. DEPTH-1 into the look-ahead ring
         enter_chunk(0);
 #pragma unroll
         for (int s = 0; s < DEPTH; ++s)
-            if ((unsigned)s < cnt) produce(s, (unsigned)s);
-#pragma unroll
-        for (int k = 0; k < NSLOT; ++k) qcur[k] = qn[0][k];
+            if ((unsigned)s < cnt) produce(s, ring + s);
 
         for (unsigned j = 0; j < cnt; j += DEPTH) {
-            // the producer is at record j + DEPTH .. j + 2 DEPTH - 1: all in one chunk (DEPTH divides kChunk)
+            // the producer is at records j + DEPTH .. j + 2 DEPTH - 1: all in one chunk (DEPTH divides kChunk)
             const unsigned jp = j + DEPTH;
             if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
+            const Rec<float> *rp = ring + (jp & kRingMask), *rc = ring + (j & kRingMask);
             if (jp + DEPTH <= cnt) {
 #pragma unroll
-                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, (jp + s) & kRingMask); }
+                for (int s = 0; s < DEPTH; ++s) { consume(s, rc + s); produce(s, rp + s); }
             } else {
 #pragma unroll
                 for (int s = 0; s < DEPTH; ++s) {
-                    if (j + s < cnt) consume(s);
-                    if (jp + s < cnt) produce(s, (jp + s) & kRingMask);
+                    if (j + s < cnt) consume(s, rc + s);
+                    if (jp + s < cnt) produce(s, rp + s);
                 }
             }
         }
 #pragma unroll
         for (int k = 0; k < NSLOT; ++k)
-            if (act[k]) flush(k);
+            if (act[k] && qcur[k] != 0xFFFFFFFFu) flush(k);
         cp_async_wait<0>();
     }
 }
