@@ -71,7 +71,6 @@ struct wpg_ctx {
     int opt_ctas_per_sm = 0;  // gridder CTAs per SM, 0 = default
     int opt_key_bits = 0;     // cap of the sort key space (log2), 0 = default 26
     int opt_timing = 0;       // 1: wpg_grid brackets its phases with CUDA events
-    int opt_variant = 0;      // experimental kernel variant selector
     int opt_no_pairs = 0;     // 1: fp32 even supports also go through the run gridder (A/B comparison)
     // instrumentation
     int64_t n_launches = 0;   // kernels of this library launched so far

@@ -361,16 +361,11 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
 #pragma unroll
         for (int k = 0; k < NSLOT; ++k) { acc0[k] = acc1[k] = 0ull; qcur[k] = 0xFFFFFFFFu; }
 
-        // look-ahead ring (registers): coefficients, visibility, window start and "first record of a
-        // window" flag of the DEPTH records in flight
+        // look-ahead ring (registers): coefficients, visibility and the lane-slot's cell of the DEPTH
+        // records in flight
         U64 c0[DEPTH][NSLOT], c1[DEPTH][NSLOT];
         U64 vis[DEPTH];
-        bool nw[DEPTH];
-        // producer state: the window of the record loaded last and the lane-slot's coefficient pointer in it
-        unsigned posP = 0xFFFFFFFFu;
-        const float2 *KcP[NSLOT];
-#pragma unroll
-        for (int k = 0; k < NSLOT; ++k) KcP[k] = K;
+        unsigned qn[DEPTH][NSLOT];
 
         // Write the pair out and clear its sums.  One asm statement with the accumulators as read-write
         // operands: the cleared value then lives in the SAME register as the sum (a separate "acc = 0"
@@ -391,32 +386,28 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         // with the window (warp-uniform branch, taken once per run of equal window starts)
         auto produce = [&](int s, const Rec<float> *rp) {
             // two 8-byte reads: (re, im) stays in its register pair until the record is consumed,
-            // (pos, koff) is used up at once (the consumer re-reads pos on the rare path)
+            // (pos, koff) is used up at once
             vis[s] = *reinterpret_cast<const U64 *>(rp);
             const uint2 pk = *reinterpret_cast<const uint2 *>(&rp->pos);
             const unsigned pos = pk.x, koff = pk.y;
-            nw[s] = __any_sync(0xffffffffu, pos != posP);
-            if (__builtin_expect(nw[s], 0)) {
 #pragma unroll
-                for (int k = 0; k < NSLOT; ++k) {
-                    const unsigned d = offset_in_window(pos, k);
-                    const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
-                    KcP[k] = K + (act[k] ? coff : 0u);
-                }
-                posP = pos;
+            for (int k = 0; k < NSLOT; ++k) {
+                const unsigned d = offset_in_window(pos, k);
+                qn[s][k] = act[k] ? pos + d : 0xFFFFFFFFu;
+                const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
+                ldg128(K + (koff + (act[k] ? coff : 0u)), c0[s][k], c1[s][k]);
             }
-#pragma unroll
-            for (int k = 0; k < NSLOT; ++k) ldg128(KcP[k] + koff, c0[s][k], c1[s][k]);
         };
-        auto consume = [&](int s, const Rec<float> *rc) {
-            if (__builtin_expect(nw[s], 0)) {  // the window moved: lane-slots whose cells changed write out
-                const unsigned pos = rc->pos;
+        auto consume = [&](int s) {
+            bool any = false;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) any |= qn[s][k] != qcur[k];
+            if (__any_sync(0xffffffffu, any)) {      // the window moved: lane-slots whose cells changed write out
 #pragma unroll
                 for (int k = 0; k < NSLOT; ++k) {
-                    const unsigned qn = act[k] ? pos + offset_in_window(pos, k) : 0xFFFFFFFFu;
-                    if (qn != qcur[k]) {
+                    if (qn[s][k] != qcur[k]) {
                         if (qcur[k] != 0xFFFFFFFFu) flush(k);      // (the sums are zero before the first window)
-                        asm volatile("mov.b32 %0, %1;" : "+r"(qcur[k]) : "r"(qn));    // tied: no second copy of qcur
+                        asm volatile("mov.b32 %0, %1;" : "+r"(qcur[k]) : "r"(qn[s][k]));    // tied: no second copy of qcur
                     }
                 }
             }
@@ -451,14 +442,14 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
             // the producer is at records j + DEPTH .. j + 2 DEPTH - 1: all in one chunk (DEPTH divides kChunk)
             const unsigned jp = j + DEPTH;
             if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
-            const Rec<float> *rp = ring + (jp & kRingMask), *rc = ring + (j & kRingMask);
+            const Rec<float> *rp = ring + (jp & kRingMask);
             if (jp + DEPTH <= cnt) {
 #pragma unroll
-                for (int s = 0; s < DEPTH; ++s) { consume(s, rc + s); produce(s, rp + s); }
+                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, rp + s); }
             } else {
 #pragma unroll
                 for (int s = 0; s < DEPTH; ++s) {
-                    if (j + s < cnt) consume(s, rc + s);
+                    if (j + s < cnt) consume(s);
                     if (jp + s < cnt) produce(s, rp + s);
                 }
             }
@@ -511,16 +502,7 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     if (F && S % 2 == 0 && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp32, even support: the pair gridder (S*S/2 pairs over 32 lanes)
         const int np = S * S / 2, nslot = (np + 31) / 32;
-        if (S == 8) {
-            switch (ctx->opt_variant) {
-                case 1: return launch_pairs<8, 1, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
-                case 2: return launch_pairs<8, 1, 2, 4>(ctx, bp, ws, K, grid, w, cls, S);
-                case 3: return launch_pairs<8, 1, 8, 3>(ctx, bp, ws, K, grid, w, cls, S);
-                case 4: return launch_pairs<8, 1, 2, 6>(ctx, bp, ws, K, grid, w, cls, S);
-                case 5: return launch_pairs<8, 1, 4, 2>(ctx, bp, ws, K, grid, w, cls, S);
-                default: return launch_pairs<8, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
-            }
-        }
+        if (S == 8) return launch_pairs<8, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
         if (S == 16) return launch_pairs<16, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
         if (S == 4) return launch_pairs<4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 1) return launch_pairs<0, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
