@@ -200,6 +200,22 @@ def run_reference(args):
         "gpu_launches": 0}))
 
 
+# --------------------------------------------------------------------------- multi-rank plumbing
+def max_over_ranks(value, dist, device):
+    """Max of a per-rank scalar over the process group (None = single process)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(n_updates_per_rank, world, ms_step_max):
+    """Whole-job throughput of `world` replicas that each process n_updates per step (weak scaling)."""
+    return world * n_updates_per_rank / (ms_step_max * 1e-3)
+
+
 # --------------------------------------------------------------------------- the CUDA arm
 def traffic_from_profiles(workload, prec):
     """dram bytes per gridder launch from the committed ncu --set full capture, if there is one."""
@@ -281,12 +297,9 @@ def run_b200(args):
     launches = ctx.launch_count() - launches0
     ms_total = e0.elapsed_time(e1)
     bin_ms, grid_ms = ctx.phase_ms()
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, dev)
     ms_step = ms_total / args.steps
-    value = world * n_updates / (ms_step * 1e-3)
+    value = aggregate_value(n_updates, world, ms_step)
 
     # ---- e2e: host buffers through wpg_grid_host, copies inside the timed region
     e2e = None
@@ -303,11 +316,8 @@ def run_b200(args):
         for _ in range(ksteps):
             ctx.grid_host(*h, stack, out=h_grid, image_out=h_img, weight_sum=wsum)   # synchronises
         dt = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([dt], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * n_updates * ksteps / dt, "unit": UNIT,
+        dt = max_over_ranks(dt, dist, dev)
+        e2e = {"value": aggregate_value(n_updates, world, 1e3 * dt / ksteps), "unit": UNIT,
                "h2d_bytes_per_step": int(sum(x.numel() * x.element_size() for x in h)),
                "d2h_bytes_per_step": int(h_grid.numel() * h_grid.element_size() + h_img.numel() * h_img.element_size()),
                "ms_per_step": 1e3 * dt / ksteps, "steps": ksteps,
@@ -328,7 +338,10 @@ def run_b200(args):
                                % ("" if prec == wpgrid.F32 else " / 2 for fp64"),
                 "gridder_ms": grid_ms, "binning_ms": bin_ms,
                 "gridder_updates_per_s": n_updates / (grid_ms * 1e-3),
-                "flop_per_update": FLOP_PER_UPDATE, "updates_per_launch": n_updates}
+                "flop_per_update": FLOP_PER_UPDATE, "updates_per_launch": n_updates,
+                # on-chip coefficient feed: 128 B/clk/SM of L1 / 8 B (c64) or 16 B (c128) per update
+                "l1_feed_frac": (n_updates / (grid_ms * 1e-3)) /
+                                (SM_COUNT * (16 if prec == wpgrid.F32 else 8) * SM_MAX_GHZ * 1e9)}
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
             hbm_gbs = json.load(f)["hbm_gbs"]; src = "measured"

@@ -255,3 +255,66 @@ def test_config5_scaled_both_precisions(ctx):
     st = oracle_stack(wl)
     ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
     check_all_paths(ctx, wl, st, ref, rstats)
+
+
+# ------------------------------------------------------------------ full size, bench.py's launch configuration
+def test_config2_full_size_as_benchmarked(ctx):
+    """BASELINE config 2 at its full 1e7 visibilities, in the configuration bench.py times (preallocated
+    workspace, default options, the library's own stack): the whole 2048^2 grid element by element against the
+    oracle (the C oracle with all host cores finishes 6.4e8 updates in about a second), the counters bit-exact,
+    and flux conservation (P11) on the GPU grid."""
+    import os
+    wl = synth.config2(device="cuda")
+    assert wl.nvis == 10_000_000
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=min(os.cpu_count() or 1, 32))
+    assert rstats["n_updates"] == 640_000_000
+    d = dev(wl)
+    ks = ctx.wkernel_build(wl.Nw, wl.w_max, wl.support, wl.oversample, wl.grid_N, wl.cell, wpgrid.F32)
+    ws = torch.empty(ctx.grid_workspace_bytes(wl.uvw.shape[0], 1, ks), dtype=torch.uint8, device="cuda")
+    grid = ctx.new_grid(ks)
+    for _ in range(2):                                  # twice: workspace reuse, as in the timed loop
+        grid.zero_()
+        g, s = ctx.grid(*d, ks, grid=grid, workspace=ws, stats=True)
+        assert s == rstats
+        gh = g.cpu().numpy()
+        assert relerr(gh, ref) <= TOL[wpgrid.F32]
+        assert abs(gh.sum(dtype=np.complex128) - ref.sum()) <= 1e-5 * abs(ref.sum())
+    # dirty image of the full grid
+    wsum = float(wl.weight.sum())
+    img = ctx.dirty_image(g, ks, wsum).cpu().numpy().astype(np.float64)
+    ref_img = oimage.dirty_image(ref, wl.cell, wsum)
+    assert np.max(np.abs(img - ref_img)) <= 2e-4 * np.max(np.abs(ref_img))
+
+
+def test_config5_1e7_both_precisions_full_grid(ctx):
+    """Config 5 (N = 4096, S = 16, 256-station tracks) on its first 1e7 visibilities through the full-size
+    grid, fp32 and fp64 from identical inputs, errors against the fp64 oracle (2.56e9 updates)."""
+    import os
+    wl = synth.config5(nvis=10_000_000, device="cuda")
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=min(os.cpu_count() or 1, 32))
+    d = dev(wl)
+    for prec in (wpgrid.F32, wpgrid.F64):
+        ks = upload(ctx, st, prec)
+        g, s = ctx.grid(*d, ks, stats=True)
+        assert s == rstats
+        e = relerr(g.cpu().numpy(), ref)
+        assert e <= TOL[prec], (prec, e)
+        del g
+
+
+def test_config3_large_grid_uniform(ctx):
+    """Config-3 sweep point in the regime the paper flags as slow (N = 8192 > 2048, S = 12 > 8), 4e6
+    visibilities through the full-size grid, fp32 and fp64."""
+    wl = synth.config3(N=8192, S=12, nvis=4_000_000)
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=8)
+    d = dev(wl)
+    for prec in (wpgrid.F32, wpgrid.F64):
+        ks = upload(ctx, st, prec)
+        g, s = ctx.grid(*d, ks, stats=True)
+        assert s == rstats
+        e = relerr(g.cpu().numpy(), ref)
+        assert e <= TOL[prec], (prec, e)
+        del g
