@@ -2,7 +2,7 @@
 """bench.py — throughput of the w-projection gridding hot path on B200 (BASELINE.json metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
-                    [--workload config2|config1|config3:N:S|config5] [--nvis n] [--prec f32|f64]
+                    [--workload config2|config1|config3:N:S|config4[:n_dump]|config5] [--nvis n] [--prec f32|f64]
 
 One "step" = one pass of the whole hot path over one batch of synthetic
 visibilities that is already resident in HBM: grid zero-fill -> binning (a1) -> gridder (a2) ->
@@ -64,6 +64,9 @@ def make_workload(spec, nvis, device):
         N = int(parts[1]) if len(parts) > 1 else 2048
         S = int(parts[2]) if len(parts) > 2 else 8
         return synth.config3(N=N, S=S, **kw)
+    if parts[0] == "config4":          # config4[:n_dump]; N(0,1) visibilities (same throughput, cheap to generate)
+        n_dump = int(parts[1]) if len(parts) > 1 else 360
+        return synth.config4(n_dump=n_dump, values="random")
     if parts[0] == "config5":
         return synth.config5(device=device, **kw)
     raise SystemExit("unknown workload %r" % spec)

@@ -65,7 +65,7 @@ int  wpg_version(void);
 
 /* Tuning knobs (all have defaults, 0 = default): "segment" = records per gridder work item;
  * "ctas_per_sm" = gridder CTAs per SM; "key_bits" = log2 cap of the binning sort-key space
- * (default 26: the key is (support class, j0u, j0v) at full resolution unless that exceeds the cap,
+ * (default 24 — a 64 MB offset table that stays in L2 — or 26 for ragged stacks: the key is (support class, j0u, j0v) at full resolution unless that exceeds the cap,
  * then low bits of j0v are dropped); "timing" 0/1 (see wpg_phase_ms); "no_pairs" 0/1 (1: fp32 even
  * supports go through the generic run gridder instead of the pair gridder — for A/B comparison).
  * Unknown name -> WPG_EINVAL. */

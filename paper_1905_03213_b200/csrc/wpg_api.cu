@@ -139,7 +139,9 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     // down the v axis, so a window that moves on leaves whole grid-row segments behind (contiguous write-outs)
     // and keeps its column ownership (the parity of j0u is fixed within a sweep); full resolution unless the
     // key space would exceed 2^key_bits
-    const int64_t cap = (int64_t)1 << (ctx->opt_key_bits ? ctx->opt_key_bits : 26);
+    // default cap: 2^24 keys (a 64 MB offset table stays in L2; at 2^26 the binning of N = 8192 takes twice as
+    // long); ragged stacks multiply the key space by the number of support classes and get 2^26
+    const int64_t cap = (int64_t)1 << (ctx->opt_key_bits ? ctx->opt_key_bits : (bp->ncls > 1 ? 26 : 24));
     int kshift = 0;
     while ((int64_t)bp->ncls * d->grid_N * (((int64_t)d->grid_N + (1 << kshift) - 1) >> kshift) > cap && kshift < 13) ++kshift;
     bp->kshift = kshift;

@@ -69,7 +69,7 @@ struct wpg_ctx {
     // options
     int opt_segment = 0;      // records per gridder work item, 0 = default
     int opt_ctas_per_sm = 0;  // gridder CTAs per SM, 0 = default
-    int opt_key_bits = 0;     // cap of the sort key space (log2), 0 = default 26
+    int opt_key_bits = 0;     // cap of the sort key space (log2), 0 = default 24
     int opt_timing = 0;       // 1: wpg_grid brackets its phases with CUDA events
     int opt_no_pairs = 0;     // 1: fp32 even supports also go through the run gridder (A/B comparison)
     // instrumentation
