@@ -1,31 +1,26 @@
 // Step a3 — dirty image: centre-origin inverse 2-D FFT of the grid, real part, / sum of weights,
 // / taper ("the master node performs an IFFT on the ... gridding result";
-// DESIGN.md O5, R11).  The fftshift/ifftshift pair is folded into (-1)^(i+j) sign checkerboards
-// before and after a plain cuFFT transform (N even), so no data is moved for the shift:
-//   img[n] = (-1)^(n1+n2) * IFFT_unnormalised[(-1)^(k1+k2) g[k]]   (the constant (-1)^N is 1).
+// DESIGN.md O5, R11).  The fftshift/ifftshift pair is (-1)^(i+j) sign checkerboards before and after a
+// plain transform (N even): img[n] = (-1)^(n1+n2) * IFFT_unnormalised[(-1)^(k1+k2) g[k]]  (the constant
+// (-1)^N is 1).  The transform is cuFFT, out of place from the caller's grid (which is not modified).
 #include "wpg_common.h"
 
 namespace {
 
 constexpr double kTaperFloor = 1e-3;
 
-template <typename C>
-__global__ void __launch_bounds__(256)
-checkerboard_copy(const C *__restrict__ g, C *__restrict__ out, int N) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
-    if (i >= N) return;
-    C v = g[(size_t)j * N + i];
-    if ((i + j) & 1) { v.x = -v.x; v.y = -v.y; }
-    out[(size_t)j * N + i] = v;
-}
-
+// f = plain (origin at index 0) unnormalised inverse FFT of the UNMODIFIED grid.  Modulating the input by
+// (-1)^(k1+k2) is a shift of the output by N/2 in both axes, so the input checkerboard is an index offset
+// here and costs no pass over the data; the output checkerboard is the sign below.
 template <typename C, typename T>
 __global__ void __launch_bounds__(256)
 correct_kernel(const C *__restrict__ f, T *__restrict__ img, const double *__restrict__ taper, int N, double inv_wsum) {
     int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
     if (i >= N) return;
+    const int h = N >> 1;
+    const int is = i < h ? i + h : i - h, js = j < h ? j + h : j - h;
     double t = taper[i] * taper[j];
-    double v = (double)f[(size_t)j * N + i].x;
+    double v = (double)f[(size_t)js * N + is].x;
     if ((i + j) & 1) v = -v;
     img[(size_t)j * N + i] = t >= kTaperFloor ? (T)(v * inv_wsum / t) : (T)0;
 }
@@ -85,17 +80,15 @@ extern "C" int wpg_dirty_image(wpg_ctx *ctx, const void *d_grid, const wpg_kdesc
     dim3 gr((N + 255) / 256, N);
     cudaStream_t s = ctx->stream;
     if (prec == WPG_F32) {
-        checkerboard_copy<float2><<<gr, 256, 0, s>>>((const float2 *)d_grid, (float2 *)d_workspace, N);
-        r = cufftExecC2C(ctx->plan, (cufftComplex *)d_workspace, (cufftComplex *)d_workspace, CUFFT_INVERSE);
+        r = cufftExecC2C(ctx->plan, (cufftComplex *)const_cast<void *>(d_grid), (cufftComplex *)d_workspace, CUFFT_INVERSE);
         if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftExecC2C: %s", cufft_str(r));
         correct_kernel<float2, float><<<gr, 256, 0, s>>>((const float2 *)d_workspace, (float *)d_image, ctx->d_taper, N, 1.0 / weight_sum);
     } else {
-        checkerboard_copy<double2><<<gr, 256, 0, s>>>((const double2 *)d_grid, (double2 *)d_workspace, N);
-        r = cufftExecZ2Z(ctx->plan, (cufftDoubleComplex *)d_workspace, (cufftDoubleComplex *)d_workspace, CUFFT_INVERSE);
+        r = cufftExecZ2Z(ctx->plan, (cufftDoubleComplex *)const_cast<void *>(d_grid), (cufftDoubleComplex *)d_workspace, CUFFT_INVERSE);
         if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftExecZ2Z: %s", cufft_str(r));
         correct_kernel<double2, double><<<gr, 256, 0, s>>>((const double2 *)d_workspace, (double *)d_image, ctx->d_taper, N, 1.0 / weight_sum);
     }
-    ctx->n_launches += 2;
+    ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }
