@@ -478,6 +478,162 @@ int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     return WPG_OK;
 }
 
+// ------------------------------------------------------------------------------------ cells (fp64)
+// The fp64 counterpart of the pair gridder: a c128 coefficient is 16 bytes, so a lane-slot owns ONE cell
+// (residue (rb, ra) of the window, any S) and one LDG.128 feeds one update of four DFMA.  Same structure
+// otherwise: cp.async record ring (24-byte records), stateless look-ahead DEPTH records deep, write-out
+// (two red.global.add.f64) as one asm with the sums as read-write operands.
+template <int SCT, int NSLOT, int DEPTH, int MINB>
+__global__ void __launch_bounds__(kRunThreads, MINB)
+grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
+                    unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
+                    const double2 *__restrict__ K, double2 *__restrict__ grid, int N, unsigned seg) {
+    static_assert(kChunk % DEPTH == 0, "the look-ahead depth divides the chunk");
+    const int S = SCT ? SCT : S_rt;
+    const int NC = S * S;
+    const int lane = threadIdx.x & 31;
+    const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
+    const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
+
+    __shared__ __align__(16) Rec<double> ring_all[kRunThreads / 32][kChunk * kRing];
+    Rec<double> *ring = ring_all[threadIdx.x >> 5];
+
+    unsigned RG[NSLOT];
+    int ra[NSLOT], rb[NSLOT];
+    bool act[NSLOT];
+#pragma unroll
+    for (int k = 0; k < NSLOT; ++k) {
+        int r = k * 32 + lane;
+        act[k] = r < NC;
+        r = act[k] ? r : 0;
+        rb[k] = r / S;
+        ra[k] = r - rb[k] * S;
+        RG[k] = (0x8000u + (unsigned)ra[k]) | ((0x8000u + (unsigned)rb[k]) << 16);
+    }
+    constexpr unsigned M = SCT ? ((unsigned)(SCT - 1) | ((unsigned)(SCT - 1) << 16)) : 0u;
+    // (iu | iv << 16) of this lane-slot's cell for a window starting at pos = j0u | j0v << 16
+    auto offset_in_window = [&](unsigned pos, int k) -> unsigned {
+        if (SCT) return (RG[k] - pos) & M;
+        const unsigned j0u = pos & 0xFFFFu, j0v = pos >> 16;
+        const int ju = (int)(j0u - ((j0u * magicS) >> 20) * (unsigned)S);
+        const int jv = (int)(j0v - ((j0v * magicS) >> 20) * (unsigned)S);
+        int x = ra[k] - ju; x += x < 0 ? S : 0;
+        int y = rb[k] - jv; y += y < 0 ? S : 0;
+        return (unsigned)x | ((unsigned)y << 16);
+    };
+
+    for (;;) {
+        unsigned item = 0;
+        if (lane == 0) item = atomicAdd(cursor, 1u);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= nitems) break;
+        const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
+        const unsigned cnt = i1 - i0;
+
+        __syncwarp();
+#pragma unroll
+        for (unsigned c = 0; c < 2; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
+
+        double accx[NSLOT], accy[NSLOT];
+        unsigned qcur[NSLOT];
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) { accx[k] = accy[k] = 0.0; qcur[k] = 0xFFFFFFFFu; }
+        double2 cf[DEPTH][NSLOT];
+        double vre[DEPTH], vim[DEPTH];
+        unsigned qn[DEPTH][NSLOT];
+
+        auto flush = [&](int k) {
+            const unsigned q = qcur[k];
+            double2 *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
+            asm volatile("red.global.add.f64 [%2], %0;\n\t"
+                         "red.global.add.f64 [%2 + 8], %1;\n\t"
+                         "mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;"
+                         : "+d"(accx[k]), "+d"(accy[k]) : "l"(g) : "memory");
+        };
+        auto produce = [&](int s, const Rec<double> *rp) {
+            vre[s] = rp->re; vim[s] = rp->im;
+            const uint2 pk = *reinterpret_cast<const uint2 *>(&rp->pos);
+            const unsigned pos = pk.x, koff = pk.y;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) {
+                const unsigned d = offset_in_window(pos, k);
+                qn[s][k] = act[k] ? pos + d : 0xFFFFFFFFu;
+                const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
+                cf[s][k] = __ldg(K + (koff + (act[k] ? coff : 0u)));
+            }
+        };
+        auto consume = [&](int s) {
+            bool any = false;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) any |= qn[s][k] != qcur[k];
+            if (__any_sync(0xffffffffu, any)) {
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    if (qn[s][k] != qcur[k]) {
+                        if (qcur[k] != 0xFFFFFFFFu) flush(k);
+                        asm volatile("mov.b32 %0, %1;" : "+r"(qcur[k]) : "r"(qn[s][k]));
+                    }
+                }
+            }
+            const double re = vre[s], im = vim[s];
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) {
+                accx[k] = fma(re, cf[s][k].x, accx[k]); accx[k] = fma(-im, cf[s][k].y, accx[k]);
+                accy[k] = fma(re, cf[s][k].y, accy[k]); accy[k] = fma(im, cf[s][k].x, accy[k]);
+            }
+        };
+        auto enter_chunk = [&](unsigned c) {
+            __syncwarp();
+            ring_fill(ring, rec, i0, i1, c + 2, lane);
+            cp_async_commit();
+            cp_async_wait<2>();
+            __syncwarp();
+        };
+
+        enter_chunk(0);
+#pragma unroll
+        for (int s = 0; s < DEPTH; ++s)
+            if ((unsigned)s < cnt) produce(s, ring + s);
+
+        for (unsigned j = 0; j < cnt; j += DEPTH) {
+            const unsigned jp = j + DEPTH;
+            if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
+            const Rec<double> *rp = ring + (jp & kRingMask);
+            if (jp + DEPTH <= cnt) {
+#pragma unroll
+                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, rp + s); }
+            } else {
+#pragma unroll
+                for (int s = 0; s < DEPTH; ++s) {
+                    if (j + s < cnt) consume(s);
+                    if (jp + s < cnt) produce(s, rp + s);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k)
+            if (act[k] && qcur[k] != 0xFFFFFFFFu) flush(k);
+        cp_async_wait<0>();
+    }
+}
+
+template <int SCT, int NSLOT, int DEPTH, int MINB>
+int launch_cells64(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+                   int cls, int S) {
+    int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
+    int blocks = ctx->sm_count * per_sm;
+    unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
+    Counters *ctr = (Counters *)(w + ws.off_counters);
+    unsigned magicS = (1u << 20) / (unsigned)S + 1u;
+    grid_cells64_kernel<SCT, NSLOT, DEPTH, MINB><<<blocks, kRunThreads, 0, ctx->stream>>>(
+        (const Rec<double> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
+        (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
+        (const double2 *)K, (double2 *)grid, bp.N, seg);
+    ctx->n_launches += 1;
+    WPG_CUDA(ctx, cudaGetLastError());
+    return WPG_OK;
+}
+
 template <typename T, int SCT, int NSLOT, int MINB>
 int launch_runs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                 int cls, int S) {
@@ -511,6 +667,16 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
         if (nslot <= 4) return launch_pairs<0, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 6) return launch_pairs<0, 6, 1, 2>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 8) return launch_pairs<0, 8, 1, 1>(ctx, bp, ws, K, grid, w, cls, S);
+    }
+    if (!F && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
+        // fp64: one cell per lane-slot, S*S cells over 32 lanes
+        const int nslot = (S * S + 31) / 32;
+        if (S == 8) return launch_cells64<8, 2, 4, 2>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 16) return launch_cells64<16, 8, 2, 1>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 4) return launch_cells64<4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 2) return launch_cells64<0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 5) return launch_cells64<0, 5, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 8) return launch_cells64<0, 8, 2, 1>(ctx, bp, ws, K, grid, w, cls, S);
     }
     if (S == 8) return launch_runs<T, 8, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
     if (S == 16) return launch_runs<T, 16, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
