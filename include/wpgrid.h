@@ -132,7 +132,8 @@ typedef struct {
     int64_t n_records;       /* valid visibilities = sorted records */
     int64_t n_keys;          /* number of sort keys = n_classes * keys_per_class */
     int32_t n_classes;       /* distinct supports; key = (class * N + j0u) * ceil(N / 2^key_shift) + (j0v >> key_shift) */
-    int32_t key_shift;
+    int32_t key_shift;       /* -1 for ragged stacks: each class gets its own shift, chosen on the device from a
+                                census of the classes so that the key budget (n_keys) goes where the visibilities are */
     int32_t record_bytes;    /* 16 (fp32) or 24 (fp64) */
     int32_t keys_per_class;
     int64_t off_records;     /* records sorted by key: {re, im, pos = j0u | j0v << 16, koff} */

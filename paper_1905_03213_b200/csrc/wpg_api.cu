@@ -148,6 +148,13 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     bp->nkg = (d->grid_N + (1 << kshift) - 1) >> kshift;
     bp->keys_per_class = (uint32_t)((int64_t)d->grid_N * bp->nkg);
     int64_t nkeys = (int64_t)bp->ncls * bp->keys_per_class;
+    // ragged stacks: the key space is a budget (2^25 keys unless key_bits is set) split among the classes on
+    // the device, after a census, so that the classes that hold the visibilities get the resolution
+    bp->dyn_keys = bp->ncls > 1;
+    if (bp->dyn_keys) {
+        nkeys = (int64_t)1 << (ctx->opt_key_bits ? ctx->opt_key_bits : 25);
+        if (nkeys < (int64_t)bp->ncls * d->grid_N) nkeys = (int64_t)bp->ncls * d->grid_N;
+    }
     if (nkeys > ((int64_t)1 << 30)) return wpg_fail(ctx, WPG_EINVAL, "sort key space %lld too large", (long long)nkeys);
     bp->nkeys = (uint32_t)nkeys;
 
@@ -258,7 +265,7 @@ extern "C" int wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, con
     if (rc) return rc;
     if (info) {
         info->n_records = h.n_records; info->n_keys = ws.nkeys;
-        info->n_classes = bp.ncls; info->key_shift = bp.kshift;
+        info->n_classes = bp.ncls; info->key_shift = bp.dyn_keys ? -1 : bp.kshift;
         info->record_bytes = prec == WPG_F32 ? 16 : 24; info->keys_per_class = (int32_t)bp.keys_per_class;
         info->off_records = (int64_t)ws.off_records; info->off_bucket_start = (int64_t)ws.off_hist;
     }

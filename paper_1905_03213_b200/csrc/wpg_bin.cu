@@ -35,10 +35,81 @@ __device__ __forceinline__ void block_count(Counters *ctr, unsigned c_grid, unsi
 }
 
 // Pass 0: f[ch] = freq[ch] / c0 (G1), once per channel instead of once per visibility.  Same IEEE
-// division as G1 states, so the products u = uvw * f are bit-identical.
-__global__ void chan_scale_kernel(const double *__restrict__ freq, int nchan, double *__restrict__ fscale) {
+// division as G1 states, so the products u = uvw * f are bit-identical.  For uniform stacks thread 0 also
+// writes the (static) key layout of the classes.
+__global__ void chan_scale_kernel(const double *__restrict__ freq, int nchan, double *__restrict__ fscale,
+                                  const __grid_constant__ BinParams P, Counters *__restrict__ ctr) {
     int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c < nchan) fscale[c] = __ddiv_rn(freq[c], WPG_C0);
+    if (c == 0 && !P.dyn_keys) {
+        for (int k = 0; k < P.ncls; ++k) {
+            ctr->key_base[k] = (unsigned)k * P.keys_per_class;
+            ctr->key_shift[k] = (unsigned)P.kshift;
+            ctr->key_nkg[k] = (unsigned)P.nkg;
+        }
+        ctr->key_base[P.ncls] = (unsigned)P.ncls * P.keys_per_class;
+    }
+}
+
+// Ragged stacks, pass 0b: census of the support classes (w -> plane -> class; weights and grid edges are
+// ignored — the census only steers the key resolution).  One thread per row, all channels.
+__global__ void __launch_bounds__(256)
+census_kernel(const double *__restrict__ uvw, const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
+              const __grid_constant__ BinParams P, Counters *__restrict__ ctr) {
+    __shared__ unsigned s_cnt[8][WPG_MAX_CLS];
+    __shared__ uint2 s_tab[WPG_MAX_NW];
+    for (int i = threadIdx.x; i < 8 * WPG_MAX_CLS; i += 256) (&s_cnt[0][0])[i] = 0;
+    wpg_stage_planetab(s_tab, T, P.Nw);
+    __syncthreads();
+    unsigned *mine = s_cnt[threadIdx.x >> 5];
+    for (long long row = (long long)blockIdx.x * 256 + threadIdx.x; row < P.nrow; row += (long long)gridDim.x * 256) {
+        const double wm = __ldg(uvw + 3 * row + 2);
+        for (int ch = 0; ch < P.nchan; ++ch) {
+            const double w = __dmul_rn(wm, __ldg(fscale + ch));
+            int p = 0;
+            if (P.dw > 0.0) {
+                const double fp = floor(wpg_div_const(__dadd_rn(w, P.w_max), P.dw, P.rdw));
+                p = fp < 0.0 ? 0 : (fp > (double)(P.Nw - 1) ? P.Nw - 1 : (int)fp);
+            }
+            atomicAdd(&mine[s_tab[p].y >> 8], 1u);
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < P.ncls) {
+        unsigned t = 0;
+        for (int wv = 0; wv < 8; ++wv) t += s_cnt[wv][threadIdx.x];
+        if (t) atomicAdd(&ctr->census[threadIdx.x], t);
+    }
+}
+
+// Ragged stacks, pass 0c (one thread): split the key budget among the classes.  Every class starts with one
+// key per grid column; the class with the most visibilities per key is refined (one more bit of j0v) as long
+// as the total stays within the budget.
+__global__ void plan_keys_kernel(Counters *__restrict__ ctr, int ncls, int N, unsigned budget) {
+    if (blockIdx.x || threadIdx.x) return;
+    unsigned sh[WPG_MAX_CLS];
+    unsigned long long total = 0;
+    auto keys = [&](unsigned s_) { return (unsigned long long)N * (unsigned)((N + (1 << s_) - 1) >> s_); };
+    for (int c = 0; c < ncls; ++c) { sh[c] = 13; total += keys(13); }
+    for (;;) {
+        int best = -1; double best_d = -1.0;
+        for (int c = 0; c < ncls; ++c) {
+            if (sh[c] == 0 || keys(sh[c] - 1) == keys(sh[c])) { if (sh[c] && keys(sh[c] - 1) == keys(sh[c])) { sh[c] -= 1; c -= 1; } continue; }
+            if (total - keys(sh[c]) + keys(sh[c] - 1) > budget) continue;
+            const double d = ((double)ctr->census[c] + 1.0) / (double)keys(sh[c]);
+            if (d > best_d) { best_d = d; best = c; }
+        }
+        if (best < 0) break;
+        total += keys(sh[best] - 1) - keys(sh[best]);
+        sh[best] -= 1;
+    }
+    unsigned base = 0;
+    for (int c = 0; c < ncls; ++c) {
+        ctr->key_base[c] = base; ctr->key_shift[c] = sh[c];
+        ctr->key_nkg[c] = (unsigned)((N + (1 << sh[c]) - 1) >> sh[c]);
+        base += (unsigned)keys(sh[c]);
+    }
+    ctr->key_base[ncls] = base;
 }
 
 constexpr int kVpt = 4;            // visibilities per thread: four independent atomics in flight per thread
@@ -80,7 +151,8 @@ __device__ __forceinline__ Located locate_vis(const RawVis &v, const SmemPlaneTa
     VisPos r = wpg_locate(v.um, v.vm, v.wm, v.f, P, T);
     if (!r.inside) return L;
     L.S = r.S; L.clamped = r.clamped;
-    L.key = (unsigned)T.cls(r.p) * P.keys_per_class + (unsigned)r.j0u * (unsigned)P.nkg + ((unsigned)r.j0v >> P.kshift);
+    const uint4 ck = T.ck[T.cls(r.p)];
+    L.key = ck.x + (unsigned)r.j0u * ck.y + ((unsigned)r.j0v >> ck.z);
     L.pos = (unsigned)r.j0u | ((unsigned)r.j0v << 16);
     L.koff = wpg_koff(r, P, T);
     return L;
@@ -95,13 +167,15 @@ bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weigh
     const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
     unsigned c_grid = 0, c_oob = 0, c_zero = 0, c_clamp = 0, c_upd = 0;
     __shared__ uint2 s_tab[WPG_MAX_NW];
-    const SmemPlaneTab ST{s_tab};
+    __shared__ uint4 s_ck[WPG_MAX_CLS];
+    const SmemPlaneTab ST{s_tab, s_ck};
     RawVis raw[kVpt];
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) raw[j] = load_vis(base + j * 256, nvis, uvw, weight, fscale, P);
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
     wpg_stage_planetab(s_tab, T, P.Nw);
+    wpg_stage_classkeys(s_ck, ctr, P.ncls);
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
@@ -215,7 +289,8 @@ template <typename TT>
 __global__ void __launch_bounds__(256, 4)
 scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, const float *__restrict__ weight,
                const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
-               const __grid_constant__ BinParams P, unsigned *__restrict__ cursor, Rec<TT> *__restrict__ rec) {
+               const __grid_constant__ BinParams P, const Counters *__restrict__ ctr, unsigned *__restrict__ cursor,
+               Rec<TT> *__restrict__ rec) {
     const long long nvis = P.nrow * P.nchan;
     const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
     Located L[kVpt];
@@ -223,7 +298,8 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
     unsigned dst[kVpt];
     float2 v[kVpt];
     __shared__ uint2 s_tab[WPG_MAX_NW];
-    const SmemPlaneTab ST{s_tab};
+    __shared__ uint4 s_ck[WPG_MAX_CLS];
+    const SmemPlaneTab ST{s_tab, s_ck};
     {
         RawVis raw[kVpt];
 #pragma unroll
@@ -235,6 +311,7 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
         wpg_stage_planetab(s_tab, T, P.Nw);
+        wpg_stage_classkeys(s_ck, ctr, P.ncls);
         __syncthreads();
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) { L[j] = locate_vis(raw[j], ST, P); wt[j] = raw[j].wt; }
@@ -266,17 +343,22 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
     cudaStream_t s = ctx->stream;
     double *fscale = (double *)(w + ws.off_fscale);
     unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
-    chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale);
+    chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale, bp, ctr);
+    if (bp.dyn_keys) {
+        census_kernel<<<ctx->sm_count * 8, 256, 0, s>>>(d_uvw, fscale, tab, bp, ctr);
+        plan_keys_kernel<<<1, 32, 0, s>>>(ctr, bp.ncls, bp.N, ws.nkeys);
+        ctx->n_launches += 2;
+    }
     if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
     scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
     scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     if (nb) {
         if (prec == WPG_F32)
-            scatter_kernel<float><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, hist,
+            scatter_kernel<float><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
                                                       (Rec<float> *)(w + ws.off_records));
         else
-            scatter_kernel<double><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, hist,
+            scatter_kernel<double><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
                                                        (Rec<double> *)(w + ws.off_records));
     }
     ctx->n_launches += nb ? 6 : 4;

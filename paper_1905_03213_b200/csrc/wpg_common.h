@@ -36,7 +36,8 @@ struct BinParams {
     int nkg;                       // ceil(N / 2^kshift): keys per grid column
     int ncls;                      // number of sort classes (distinct supports)
     uint32_t keys_per_class;       // N * nkg; key = (cls * N + j0u) * nkg + (j0v >> kshift)
-    uint32_t nkeys;                // ncls * keys_per_class
+    uint32_t nkeys;                // size of the key space (ncls * keys_per_class, or the key budget if dynamic)
+    int dyn_keys;                  // 1: per-class key layout chosen on the device (ragged stacks)
 };
 
 // Sorted record.  pos = j0u | j0v << 16 (window start, cells); koff = element offset
@@ -52,6 +53,10 @@ struct Counters {
     unsigned long long n_gridded[16], n_skipped_oob[16], n_skipped_zero_weight[16], n_clamped_w[16], n_updates[16];
     unsigned int n_records, pad0, pad1, pad2;
     unsigned int cursor[WPG_MAX_CLS];   // work-item cursors of the gridder launches (one per sort class)
+    // key layout of each sort class: key = key_base[cls] + j0u * key_nkg[cls] + (j0v >> key_shift[cls]).
+    // Uniform stacks: filled from the host plan.  Ragged stacks: chosen on the device from a census of the
+    // classes (the key budget goes to the classes that hold the visibilities).
+    unsigned int key_base[WPG_MAX_CLS + 1], key_shift[WPG_MAX_CLS], key_nkg[WPG_MAX_CLS], census[WPG_MAX_CLS];
 };
 
 constexpr int kStatSlots = 16;
@@ -158,6 +163,7 @@ __device__ __forceinline__ void wpg_axis(double x_lambda, const BinParams &P, in
 // passes index it with a different plane in every lane, which the constant cache would serialise).
 struct SmemPlaneTab {
     const uint2 *e;        // e[p] = {element offset of plane p, S_p | class << 8}
+    const uint4 *ck;       // ck[cls] = {key_base, key_nkg, key_shift, -}
     __device__ __forceinline__ int S(int p) const { return (int)(e[p].y & 0xFFu); }
     __device__ __forceinline__ int cls(int p) const { return (int)(e[p].y >> 8); }
     __device__ __forceinline__ int off(int p) const { return (int)e[p].x; }
@@ -171,6 +177,9 @@ struct ParamPlaneTab {
 // fills the shared copy (call from every thread of the block, then __syncthreads)
 __device__ __forceinline__ void wpg_stage_planetab(uint2 *dst, const PlaneTab &T, int Nw) {
     for (int p = threadIdx.x; p < Nw; p += blockDim.x) dst[p] = make_uint2((unsigned)T.off[p], (unsigned)T.S[p] | ((unsigned)T.cls[p] << 8));
+}
+__device__ __forceinline__ void wpg_stage_classkeys(uint4 *dst, const Counters *ctr, int ncls) {
+    for (int c = threadIdx.x; c < ncls; c += blockDim.x) dst[c] = make_uint4(ctr->key_base[c], ctr->key_nkg[c], ctr->key_shift[c], 0u);
 }
 
 template <typename Tab>
