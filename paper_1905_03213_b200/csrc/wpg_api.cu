@@ -46,6 +46,11 @@ extern "C" void wpg_destroy(wpg_ctx *ctx) {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     for (auto &e : ctx->ev) cudaEventDestroy(e);
+    for (int i = 0; i < 3; ++i) {
+        if (ctx->side[i]) cudaStreamDestroy(ctx->side[i]);
+        if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     if (ctx->plan) cufftDestroy(ctx->plan);
     if (ctx->d_taper) cudaFree(ctx->d_taper);
     if (ctx->d_host_scratch) cudaFree(ctx->d_host_scratch);

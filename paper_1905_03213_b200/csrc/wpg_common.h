@@ -81,6 +81,9 @@ struct wpg_ctx {
     int64_t n_launches = 0;   // kernels of this library launched so far
     std::vector<cudaEvent_t> ev;   // triplets: start, after binning, after gridder (pool, reused)
     size_t ev_used = 0;            // triplets recorded since the last wpg_phase_ms
+    // side streams for the gridder launches of ragged stacks (one launch per support class; created lazily)
+    cudaStream_t side[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
     // cuFFT plan cache
     cufftHandle plan = 0; int plan_N = 0; int plan_prec = -1;
     // taper table cache for dirty_image

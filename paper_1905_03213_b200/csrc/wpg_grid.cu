@@ -694,13 +694,36 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
 int wpg_launch_grid(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws,
                     wpg_prec prec, const void *K, void *grid, char *w) {
     if (bp.nrow == 0) return WPG_OK;
-    for (int cls = 0; cls < bp.ncls; ++cls) {
-        int S = tab.clsS[cls];
-        int rc = prec == WPG_F32 ? launch_class<float>(ctx, bp, ws, K, grid, w, cls, S)
-                                 : launch_class<double>(ctx, bp, ws, K, grid, w, cls, S);
-        if (rc) return rc;
+    if (bp.ncls == 1) {
+        return prec == WPG_F32 ? launch_class<float>(ctx, bp, ws, K, grid, w, 0, tab.clsS[0])
+                               : launch_class<double>(ctx, bp, ws, K, grid, w, 0, tab.clsS[0]);
     }
-    return WPG_OK;
+    // Ragged stack: one launch per support class, independent of each other (they only meet in the grid's
+    // reductions).  Most classes hold few visibilities and cannot fill the machine on their own, so the
+    // launches are spread over the context's stream and three side streams, large supports first.
+    cudaStream_t main_stream = ctx->stream;
+    if (!ctx->ev_fork) {
+        WPG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+        for (int i = 0; i < 3; ++i) {
+            WPG_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->side[i], cudaStreamNonBlocking));
+            WPG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming));
+        }
+    }
+    WPG_CUDA(ctx, cudaEventRecord(ctx->ev_fork, main_stream));
+    for (int i = 0; i < 3; ++i) WPG_CUDA(ctx, cudaStreamWaitEvent(ctx->side[i], ctx->ev_fork, 0));
+    int rc = WPG_OK;
+    for (int cls = bp.ncls - 1; cls >= 0 && rc == WPG_OK; --cls) {
+        const int S = tab.clsS[cls];
+        ctx->stream = cls % 4 == 0 ? main_stream : ctx->side[cls % 4 - 1];
+        rc = prec == WPG_F32 ? launch_class<float>(ctx, bp, ws, K, grid, w, cls, S)
+                             : launch_class<double>(ctx, bp, ws, K, grid, w, cls, S);
+    }
+    ctx->stream = main_stream;
+    for (int i = 0; i < 3; ++i) {
+        WPG_CUDA(ctx, cudaEventRecord(ctx->ev_join[i], ctx->side[i]));
+        WPG_CUDA(ctx, cudaStreamWaitEvent(main_stream, ctx->ev_join[i], 0));
+    }
+    return rc;
 }
 
 int wpg_launch_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
