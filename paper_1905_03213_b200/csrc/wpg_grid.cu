@@ -299,17 +299,23 @@ __device__ __forceinline__ void ldg128(const float2 *p, unsigned long long &c0, 
     asm volatile("ld.global.nc.v2.b64 {%0, %1}, [%2];" : "=l"(c0), "=l"(c1) : "l"(p));
 }
 
-template <int SCT, int NSLOT, int DEPTH, int MINB>
+// G > 1 (small supports: S*S/2 <= 32/G pairs, NSLOT = 1): the warp is split into G groups of 32/G lanes and
+// every group takes its own record, G records per step (record t*G + g goes to group g), so that a 4x4
+// support does not leave three quarters of the warp idle.
+template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1>
 __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
                   const unsigned *__restrict__ key_base, int cls, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
                   const float2 *__restrict__ K, float2 *__restrict__ grid, int N, unsigned seg) {
-    static_assert(kChunk % DEPTH == 0, "the look-ahead depth divides the chunk");
+    static_assert(kChunk % (DEPTH * G) == 0, "a look-ahead step divides the chunk");
+    static_assert(G == 1 || NSLOT == 1, "lane groups only for one-slot supports");
+    constexpr int LPG = 32 / G;                          // lanes per group
     using U64 = unsigned long long;
     const int S = SCT ? SCT : S_rt;
     const int H = S >> 1;                                // pairs per window row
     const int NP = S * H;                                // pairs per window
     const int lane = threadIdx.x & 31;
+    const int grp = G > 1 ? lane / LPG : 0;              // this lane's group: takes record t*G + grp of step t
     const unsigned r_begin = __ldg(bucket_start + __ldg(key_base + cls)), r_end = __ldg(bucket_start + __ldg(key_base + cls + 1));
     const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
 
@@ -324,7 +330,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     bool act[NSLOT];
 #pragma unroll
     for (int k = 0; k < NSLOT; ++k) {
-        int r = k * 32 + lane;
+        int r = k * 32 + (G > 1 ? lane % LPG : lane);
         act[k] = r < NP;
         r = act[k] ? r : 0;
         rb[k] = r / H;
@@ -384,16 +390,18 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         };
         // stage s <- record rp[0]: coefficient loads; the lane's offset inside the slice changes only
         // with the window (warp-uniform branch, taken once per run of equal window starts)
-        auto produce = [&](int s, const Rec<float> *rp) {
+        // `valid` (per lane, only ever false for G > 1 at the ragged end of an item): a lane without a record
+        // loads coefficient 0 of the stack, adds 0 * c and reports "no cell" (which writes its sums out early)
+        auto produce = [&](int s, const Rec<float> *rp, bool valid) {
             // two 8-byte reads: (re, im) stays in its register pair until the record is consumed,
             // (pos, koff) is used up at once
-            vis[s] = *reinterpret_cast<const U64 *>(rp);
-            const uint2 pk = *reinterpret_cast<const uint2 *>(&rp->pos);
+            vis[s] = valid ? *reinterpret_cast<const U64 *>(rp) : 0ull;
+            const uint2 pk = valid ? *reinterpret_cast<const uint2 *>(&rp->pos) : make_uint2(0u, 0u);
             const unsigned pos = pk.x, koff = pk.y;
 #pragma unroll
             for (int k = 0; k < NSLOT; ++k) {
                 const unsigned d = offset_in_window(pos, k);
-                qn[s][k] = act[k] ? pos + d : 0xFFFFFFFFu;
+                qn[s][k] = act[k] && valid ? pos + d : 0xFFFFFFFFu;
                 const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
                 ldg128(K + (koff + (act[k] ? coff : 0u)), c0[s][k], c1[s][k]);
             }
@@ -436,21 +444,22 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         enter_chunk(0);
 #pragma unroll
         for (int s = 0; s < DEPTH; ++s)
-            if ((unsigned)s < cnt) produce(s, ring + s);
+            if ((unsigned)(s * G) < cnt) produce(s, ring + s * G + grp, (unsigned)(s * G + grp) < cnt);
 
-        for (unsigned j = 0; j < cnt; j += DEPTH) {
-            // the producer is at records j + DEPTH .. j + 2 DEPTH - 1: all in one chunk (DEPTH divides kChunk)
-            const unsigned jp = j + DEPTH;
+        constexpr unsigned STEP = DEPTH * G;                 // records per trip of the loop
+        for (unsigned j = 0; j < cnt; j += STEP) {
+            // the producer is at records j + STEP .. j + 2 STEP - 1: all in one chunk (STEP divides kChunk)
+            const unsigned jp = j + STEP;
             if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
-            const Rec<float> *rp = ring + (jp & kRingMask);
-            if (jp + DEPTH <= cnt) {
+            const Rec<float> *rp = ring + (jp & kRingMask) + grp;
+            if (jp + STEP <= cnt) {
 #pragma unroll
-                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, rp + s); }
+                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, rp + s * G, true); }
             } else {
 #pragma unroll
                 for (int s = 0; s < DEPTH; ++s) {
-                    if (j + s < cnt) consume(s);
-                    if (jp + s < cnt) produce(s, rp + s);
+                    if (j + s * G < cnt) consume(s);
+                    if (jp + s * G < cnt) produce(s, rp + s * G, jp + s * G + grp < cnt);
                 }
             }
         }
@@ -461,7 +470,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     }
 }
 
-template <int SCT, int NSLOT, int DEPTH, int MINB>
+template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1>
 int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                  int cls, int S) {
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
@@ -469,7 +478,7 @@ int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;         // (x * magicS) >> 20 == x / S for x < 2^13, S <= 32
-    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB><<<blocks, kRunThreads, 0, ctx->stream>>>(
+    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB, G><<<blocks, kRunThreads, 0, ctx->stream>>>(
         (const Rec<float> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
         ctr->key_base, cls, S, magicS, &ctr->cursor[cls],
         (const float2 *)K, (float2 *)grid, bp.N, seg);
@@ -660,7 +669,7 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
         const int np = S * S / 2, nslot = (np + 31) / 32;
         if (S == 8) return launch_pairs<8, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
         if (S == 16) return launch_pairs<16, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
-        if (S == 4) return launch_pairs<4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 4) return launch_pairs<4, 1, 4, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);        // 8 pairs: 4 records per step
         if (nslot <= 1) return launch_pairs<0, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 2) return launch_pairs<0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 3) return launch_pairs<0, 3, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);
