@@ -175,7 +175,7 @@ bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weigh
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
     wpg_stage_planetab(s_tab, T, P.Nw);
-    wpg_stage_classkeys(s_ck, ctr, P.ncls);
+    wpg_stage_classkeys(s_ck, ctr, P);
     __syncthreads();
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
@@ -311,7 +311,7 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
         wpg_stage_planetab(s_tab, T, P.Nw);
-        wpg_stage_classkeys(s_ck, ctr, P.ncls);
+        wpg_stage_classkeys(s_ck, ctr, P);
         __syncthreads();
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) { L[j] = locate_vis(raw[j], ST, P); wt[j] = raw[j].wt; }

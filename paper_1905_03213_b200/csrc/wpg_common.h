@@ -181,8 +181,10 @@ struct ParamPlaneTab {
 __device__ __forceinline__ void wpg_stage_planetab(uint2 *dst, const PlaneTab &T, int Nw) {
     for (int p = threadIdx.x; p < Nw; p += blockDim.x) dst[p] = make_uint2((unsigned)T.off[p], (unsigned)T.S[p] | ((unsigned)T.cls[p] << 8));
 }
-__device__ __forceinline__ void wpg_stage_classkeys(uint4 *dst, const Counters *ctr, int ncls) {
-    for (int c = threadIdx.x; c < ncls; c += blockDim.x) dst[c] = make_uint4(ctr->key_base[c], ctr->key_nkg[c], ctr->key_shift[c], 0u);
+__device__ __forceinline__ void wpg_stage_classkeys(uint4 *dst, const Counters *ctr, const BinParams &P) {
+    for (int c = threadIdx.x; c < P.ncls; c += blockDim.x)
+        dst[c] = P.dyn_keys ? make_uint4(ctr->key_base[c], ctr->key_nkg[c], ctr->key_shift[c], 0u)
+                            : make_uint4((unsigned)c * P.keys_per_class, (unsigned)P.nkg, (unsigned)P.kshift, 0u);   // no load
 }
 
 template <typename Tab>

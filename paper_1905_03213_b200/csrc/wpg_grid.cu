@@ -139,7 +139,7 @@ __device__ __forceinline__ void ring_get(const Rec<double> *ring, unsigned slot,
 template <typename T, int SCT, int NSLOT, int MINB>
 __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_runs_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
-                 const unsigned *__restrict__ key_base, int cls, int S_rt, unsigned *__restrict__ cursor,
+                 const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned *__restrict__ cursor,
                  const typename Cplx<T>::type *__restrict__ K, typename Cplx<T>::type *__restrict__ grid,
                  int N, unsigned seg) {
     using C = typename Cplx<T>::type;
@@ -148,7 +148,9 @@ grid_runs_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bu
     const int S = SCT ? SCT : S_rt;
     const int S2 = S * S;
     const int lane = threadIdx.x & 31;
-    const unsigned r_begin = __ldg(bucket_start + __ldg(key_base + cls)), r_end = __ldg(bucket_start + __ldg(key_base + cls + 1));
+    // key range of this support class: from the device table (ragged stacks) or by value (key_base == nullptr)
+    if (key_base) { key_lo = __ldg(key_base + cls); key_hi = __ldg(key_base + cls + 1); }
+    const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
     const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
 
     __shared__ __align__(16) Rec<T> ring_all[kRunThreads / 32][kChunk * kRing];
@@ -305,7 +307,7 @@ __device__ __forceinline__ void ldg128(const float2 *p, unsigned long long &c0, 
 template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1>
 __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
-                  const unsigned *__restrict__ key_base, int cls, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
+                  const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
                   const float2 *__restrict__ K, float2 *__restrict__ grid, int N, unsigned seg) {
     static_assert(kChunk % (DEPTH * G) == 0, "a look-ahead step divides the chunk");
     static_assert(G == 1 || NSLOT == 1, "lane groups only for one-slot supports");
@@ -316,7 +318,9 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     const int NP = S * H;                                // pairs per window
     const int lane = threadIdx.x & 31;
     const int grp = G > 1 ? lane / LPG : 0;              // this lane's group: takes record t*G + grp of step t
-    const unsigned r_begin = __ldg(bucket_start + __ldg(key_base + cls)), r_end = __ldg(bucket_start + __ldg(key_base + cls + 1));
+    // key range of this support class: from the device table (ragged stacks) or by value (key_base == nullptr)
+    if (key_base) { key_lo = __ldg(key_base + cls); key_hi = __ldg(key_base + cls + 1); }
+    const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
     const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
 
     __shared__ __align__(16) Rec<float> ring_all[kRunThreads / 32][kChunk * kRing];
@@ -480,7 +484,7 @@ int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;         // (x * magicS) >> 20 == x / S for x < 2^13, S <= 32
     grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB, G><<<blocks, kRunThreads, 0, ctx->stream>>>(
         (const Rec<float> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
-        ctr->key_base, cls, S, magicS, &ctr->cursor[cls],
+        bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
         (const float2 *)K, (float2 *)grid, bp.N, seg);
     ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
@@ -495,13 +499,15 @@ int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
 template <int SCT, int NSLOT, int DEPTH, int MINB>
 __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
-                    const unsigned *__restrict__ key_base, int cls, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
+                    const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
                     const double2 *__restrict__ K, double2 *__restrict__ grid, int N, unsigned seg) {
     static_assert(kChunk % DEPTH == 0, "the look-ahead depth divides the chunk");
     const int S = SCT ? SCT : S_rt;
     const int NC = S * S;
     const int lane = threadIdx.x & 31;
-    const unsigned r_begin = __ldg(bucket_start + __ldg(key_base + cls)), r_end = __ldg(bucket_start + __ldg(key_base + cls + 1));
+    // key range of this support class: from the device table (ragged stacks) or by value (key_base == nullptr)
+    if (key_base) { key_lo = __ldg(key_base + cls); key_hi = __ldg(key_base + cls + 1); }
+    const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
     const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
 
     __shared__ __align__(16) Rec<double> ring_all[kRunThreads / 32][kChunk * kRing];
@@ -636,7 +642,7 @@ int launch_cells64(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws,
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;
     grid_cells64_kernel<SCT, NSLOT, DEPTH, MINB><<<blocks, kRunThreads, 0, ctx->stream>>>(
         (const Rec<double> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
-        ctr->key_base, cls, S, magicS, &ctr->cursor[cls],
+        bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
         (const double2 *)K, (double2 *)grid, bp.N, seg);
     ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
@@ -653,7 +659,7 @@ int launch_runs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, co
     Counters *ctr = (Counters *)(w + ws.off_counters);
     grid_runs_kernel<T, SCT, NSLOT, MINB><<<blocks, kRunThreads, 0, ctx->stream>>>(
         (const Rec<T> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
-        ctr->key_base, cls, S, &ctr->cursor[cls],
+        bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, &ctr->cursor[cls],
         (const C *)K, (C *)grid, bp.N, seg);
     ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
