@@ -318,3 +318,38 @@ def test_config3_large_grid_uniform(ctx):
         e = relerr(g.cpu().numpy(), ref)
         assert e <= TOL[prec], (prec, e)
         del g
+
+
+# ------------------------------------------------------------------ code paths added with the pair / cell gridders
+@pytest.mark.parametrize("S", [2, 4, 6, 8, 10, 16, 22, 24])
+def test_even_supports_segments_and_tails(ctx, S):
+    """Every instantiation of the pair gridder (lane groups at S = 4, power-of-two and generic supports, the
+    run-gridder fallback above S = 22) and of the fp64 cell gridder, with work-item lengths that leave ragged
+    tails in the look-ahead ring (1, 5, 17 records) and one item for everything."""
+    rng = np.random.default_rng(100 + S)
+    N, cell, Q, Nw, w_max, n = 128, 0.06 / 128, 4, 6, 80.0, 6000
+    du = 1.0 / 0.06
+    uvw = np.stack([rng.uniform(-40, 40, n) * du, rng.uniform(-40, 40, n) * du, rng.uniform(-90, 90, n)], 1)
+    uvw[: n // 3, :2] = np.round(uvw[: n // 3, :2] / du) * du          # long runs of equal windows as well
+    vis = (rng.standard_normal((n, 1)) + 1j * rng.standard_normal((n, 1))).astype(np.complex64)
+    wt = rng.uniform(0.5, 1.5, (n, 1)).astype(np.float32)
+    freq = np.array([synth.C0])
+    st = owk.build_stack(Nw, w_max, S, Q, N, cell)
+    ref, rstats = ogrid.grid(uvw, vis, wt, freq, st)
+    assert rstats["n_gridded"] > 5000
+    wl = synth.Workload("even%d" % S, uvw, freq, vis, wt, N, cell, Nw, w_max, S, Q)
+    check_all_paths(ctx, wl, st, ref, rstats, segments=(0, 1, 5, 17, 100000))
+    ctx.set_option("no_pairs", 1)                                       # the run gridder on the same input
+    check_all_paths(ctx, wl, st, ref, rstats)
+    ctx.set_option("no_pairs", 0)
+
+
+def test_ragged_stack_key_budgets_both_precisions(ctx):
+    """Ragged stack (per-class sort keys planned on the device from the class census): the result must not
+    depend on the key budget — from one key per grid column (key_bits = 8 is below the minimum and is raised
+    to it) to ample — in fp32 and fp64."""
+    wl = synth.config4(n_dump=1, nchan=2, values="random")
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    assert len(set(st.support.tolist())) >= 4
+    check_all_paths(ctx, wl, st, ref, rstats, key_bits=(0, 8, 20, 27))
