@@ -49,6 +49,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="library option name=value (tuning)")
+    ap.add_argument("--no-row-block", action="store_true",
+                    help="do not pass the rows-per-time-step hint of track-based workloads to the library")
     return ap.parse_args()
 
 
@@ -77,6 +79,7 @@ def workload_config(wl, prec):
             "Nw": wl.Nw, "support": wl.support if np.isscalar(wl.support) else list(wl.support),
             "oversample": wl.oversample, "precision": prec,
             "step": "grid zero-fill + binning (a1) + gridder (a2) + dirty_image (a3); wkernel_build (a0) untimed",
+            "row_block": int(wl.notes.get("row_block", 0)),
             "l2": "inputs (%.0f MB) larger than the 126 MB L2; no explicit flush" %
                   ((wl.uvw.nbytes + wl.vis.nbytes + wl.weight.nbytes) / 1e6)}
 
@@ -251,6 +254,8 @@ def run_b200(args):
     prec = wpgrid.F32 if args.prec == "f32" else wpgrid.F64
     wl = make_workload(args.workload, args.nvis, dev)
     ctx = wpgrid.Context(local)
+    row_block = 0 if args.no_row_block else int(wl.notes.get("row_block", 0))
+    ctx.set_option("row_block", row_block)     # rows are time-major, baseline-minor (Measurement Set order)
     for o in args.option:
         k, v = o.split("=")
         ctx.set_option(k, int(v))

@@ -67,7 +67,12 @@ int  wpg_version(void);
  * "ctas_per_sm" = gridder CTAs per SM; "key_bits" = log2 cap of the binning sort-key space
  * (default 24 — a 64 MB offset table that stays in L2 — or 26 for ragged stacks: the key is (support class, j0u, j0v) at full resolution unless that exceeds the cap,
  * then low bits of j0v are dropped); "timing" 0/1 (see wpg_phase_ms); "no_pairs" 0/1 (1: fp32 even
- * supports go through the generic run gridder instead of the pair gridder — for A/B comparison).
+ * supports go through the generic run gridder instead of the pair gridder — for A/B comparison);
+ * "row_block" = rows per time step when the rows come time-major, baseline-minor (the row order of a
+ * Measurement Set; 0 = unknown, the default): a binning thread then handles the same
+ * baseline at consecutive time steps, whose samples mostly hit the same grid point, and
+ * updates the bucket counter once per run instead of once per visibility.  A hint only: any value gives
+ * the same result.
  * Unknown name -> WPG_EINVAL. */
 int  wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value);
 

@@ -68,6 +68,7 @@ extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
     else if (!strcmp(name, "key_bits")) { if (value != 0 && (value < 8 || value > 28)) return wpg_fail(ctx, WPG_EINVAL, "key_bits must be 0 or 8..28"); ctx->opt_key_bits = (int)value; }
     else if (!strcmp(name, "timing")) { ctx->opt_timing = value != 0; }
     else if (!strcmp(name, "no_pairs")) { ctx->opt_no_pairs = value != 0; }
+    else if (!strcmp(name, "row_block")) { if (value < 0) return wpg_fail(ctx, WPG_EINVAL, "row_block must be >= 0"); ctx->opt_row_block = value; }
     else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
     return WPG_OK;
 }
@@ -128,6 +129,10 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
 
     memset(bp, 0, sizeof *bp);
     bp->nrow = nrow; bp->nchan = nchan;
+    // time-coherent thread mapping only if it is well formed and leaves enough parallelism
+    bp->vis_block = 0;
+    if (ctx->opt_row_block > 0 && ctx->opt_row_block * nchan < ((int64_t)1 << 31) && nvis >= 64 * ctx->opt_row_block * nchan)
+        bp->vis_block = (uint32_t)(ctx->opt_row_block * nchan);
     bp->N = d->grid_N; bp->Q = d->oversample; bp->Nw = d->Nw;
     bp->w_max = d->w_max;
     bp->dw = 2.0 * d->w_max / (double)d->Nw;

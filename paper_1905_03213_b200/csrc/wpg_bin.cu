@@ -114,6 +114,38 @@ __global__ void plan_keys_kernel(Counters *__restrict__ ctr, int ncls, int N, un
 
 constexpr int kVpt = 4;            // visibilities per thread: four independent atomics in flight per thread
 
+// The kVpt visibilities of a thread.  Default: a block takes 256 * kVpt consecutive visibilities, thread t the
+// ones at t, t + 256, ...  With the "row_block" hint (P.vis_block = visibilities per time step): thread
+// (dg, x) takes visibility x of the time steps dg * kVpt + j — the same baseline and channel at consecutive
+// times, whose window starts (and so sort keys) mostly coincide, so that the bucket counter is
+// touched once per run of equal keys.  Loads stay coalesced either way (consecutive lanes, consecutive x).
+__device__ __forceinline__ void vis_indices(const BinParams &P, unsigned (&idx)[kVpt]) {
+    const unsigned long long nvis = (unsigned long long)(P.nrow * P.nchan);     // < 2^32 - 1 (wpg_make_plan)
+    if (P.vis_block) {
+        const unsigned t = blockIdx.x * 256u + threadIdx.x;
+        const unsigned dg = t / P.vis_block, x = t - dg * P.vis_block;
+#pragma unroll
+        for (int j = 0; j < kVpt; ++j) {
+            const unsigned long long i = (unsigned long long)(dg * kVpt + j) * P.vis_block + x;
+            idx[j] = i < nvis ? (unsigned)i : 0xFFFFFFFFu;
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < kVpt; ++j) {
+            const unsigned long long i = (unsigned long long)blockIdx.x * (256 * kVpt) + j * 256 + threadIdx.x;
+            idx[j] = i < nvis ? (unsigned)i : 0xFFFFFFFFu;
+        }
+    }
+}
+// run structure of a thread's keys: head[j] = first of a run of equal valid keys, len[j] = length of the run from j
+__device__ __forceinline__ void key_runs(const unsigned (&key)[kVpt], bool (&head)[kVpt], unsigned (&len)[kVpt]) {
+#pragma unroll
+    for (int j = kVpt - 1; j >= 0; --j) {
+        len[j] = 1u + ((j + 1 < kVpt && key[j + 1] == key[j]) ? len[j + 1 < kVpt ? j + 1 : j] : 0u);
+        head[j] = key[j] != WPG_NO_KEY && (j == 0 || key[j] != key[j - 1]);
+    }
+}
+
 // Position math (fp64, G1-G3) and validity (G4, R9) of visibility i; returns the sort key or WPG_NO_KEY.
 // The two passes below both evaluate it: recomputing is cheaper than a round trip of (key, position,
 // coefficient offset) through HBM, and the workspace holds nothing per visibility but the records.
@@ -164,30 +196,35 @@ bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weigh
                  const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
                  const __grid_constant__ BinParams P, Counters *__restrict__ ctr, unsigned *__restrict__ hist) {
     const long long nvis = P.nrow * P.nchan;
-    const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
+    unsigned idx[kVpt];
+    vis_indices(P, idx);
     unsigned c_grid = 0, c_oob = 0, c_zero = 0, c_clamp = 0, c_upd = 0;
     __shared__ uint2 s_tab[WPG_MAX_NW];
     __shared__ uint4 s_ck[WPG_MAX_CLS];
     const SmemPlaneTab ST{s_tab, s_ck};
     RawVis raw[kVpt];
 #pragma unroll
-    for (int j = 0; j < kVpt; ++j) raw[j] = load_vis(base + j * 256, nvis, uvw, weight, fscale, P);
+    for (int j = 0; j < kVpt; ++j) raw[j] = load_vis(idx[j], nvis, uvw, weight, fscale, P);
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
     wpg_stage_planetab(s_tab, T, P.Nw);
     wpg_stage_classkeys(s_ck, ctr, P);
     __syncthreads();
+    unsigned key[kVpt], len[kVpt];
+    bool head[kVpt];
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
+        key[j] = WPG_NO_KEY;
         if (!raw[j].valid) continue;
         const Located L = locate_vis(raw[j], ST, P);
         if (L.zero_weight) c_zero += 1;
         else if (L.key == WPG_NO_KEY) c_oob += 1;
-        else {
-            c_grid += 1; c_clamp += L.clamped; c_upd += L.S * L.S;
-            asm volatile("red.global.add.u32 [%0], 1;" ::"l"(hist + L.key) : "memory");
-        }
+        else { c_grid += 1; c_clamp += L.clamped; c_upd += L.S * L.S; key[j] = L.key; }
     }
+    key_runs(key, head, len);
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j)
+        if (head[j]) asm volatile("red.global.add.u32 [%0], %1;" ::"l"(hist + key[j]), "r"(len[j]) : "memory");
     block_count(ctr, c_grid, c_oob, c_zero, c_clamp, c_upd);
 }
 
@@ -292,7 +329,8 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
                const __grid_constant__ BinParams P, const Counters *__restrict__ ctr, unsigned *__restrict__ cursor,
                Rec<TT> *__restrict__ rec) {
     const long long nvis = P.nrow * P.nchan;
-    const long long base = (long long)blockIdx.x * (256 * kVpt) + threadIdx.x;
+    unsigned idx[kVpt];
+    vis_indices(P, idx);
     Located L[kVpt];
     float wt[kVpt];
     unsigned dst[kVpt];
@@ -304,7 +342,7 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
         RawVis raw[kVpt];
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) {
-            const long long i = base + j * 256;
+            const long long i = idx[j];        // 0xFFFFFFFF = none (>= nvis)
             raw[j] = load_vis(i, nvis, uvw, weight, fscale, P);
             v[j] = i < nvis ? __ldg(vis + i) : make_float2(0.f, 0.f);
         }
@@ -316,8 +354,17 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) { L[j] = locate_vis(raw[j], ST, P); wt[j] = raw[j].wt; }
     }
+    // one returning atomic per run of equal keys (the slowest instruction of the pass: ~5 cycles per lane)
+    unsigned key[kVpt], len[kVpt];
+    bool head[kVpt];
 #pragma unroll
-    for (int j = 0; j < kVpt; ++j) dst[j] = L[j].key != WPG_NO_KEY ? atomicAdd(cursor + L[j].key, 1u) : 0u;
+    for (int j = 0; j < kVpt; ++j) key[j] = L[j].key;
+    key_runs(key, head, len);
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) dst[j] = head[j] ? atomicAdd(cursor + key[j], len[j]) : 0u;
+#pragma unroll
+    for (int j = 1; j < kVpt; ++j)
+        if (key[j] != WPG_NO_KEY && !head[j]) dst[j] = dst[j - 1] + 1u;
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
         if (L[j].key == WPG_NO_KEY) continue;
@@ -343,6 +390,10 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
     cudaStream_t s = ctx->stream;
     double *fscale = (double *)(w + ws.off_fscale);
     unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
+    if (bp.vis_block) {                // ceil(time steps / kVpt) * vis_block threads
+        const long long nd = (nvis + bp.vis_block - 1) / bp.vis_block;
+        nb = (unsigned)((((nd + kVpt - 1) / kVpt) * bp.vis_block + 255) / 256);
+    }
     chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale, bp, ctr);
     if (bp.dyn_keys) {
         census_kernel<<<ctx->sm_count * 8, 256, 0, s>>>(d_uvw, fscale, tab, bp, ctr);

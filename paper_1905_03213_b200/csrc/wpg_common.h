@@ -28,6 +28,8 @@ struct PlaneTab {
 struct BinParams {
     int64_t nrow;
     int nchan;
+    uint32_t vis_block;            // 0, or visibilities per time step (row_block * nchan): a binning thread then takes
+                                   // the SAME baseline/channel at consecutive time steps (see wpg_vis_index)
     int N, Q, Nw;
     double w_max, dw, du, halfN;   // dw = 2 w_max / Nw, du = 1/(N cell), halfN = N/2
     double rdu, rdw, invQ;         // RN(1/du), RN(1/dw), 1/Q (wpg_div_const, floor division by Q)
@@ -76,6 +78,7 @@ struct wpg_ctx {
     int opt_ctas_per_sm = 0;  // gridder CTAs per SM, 0 = default
     int opt_key_bits = 0;     // cap of the sort key space (log2), 0 = default 24
     int opt_timing = 0;       // 1: wpg_grid brackets its phases with CUDA events
+    int64_t opt_row_block = 0; // rows per time step (0 = unknown), see wpg_set_option
     int opt_no_pairs = 0;     // 1: fp32 even supports also go through the run gridder (A/B comparison)
     // instrumentation
     int64_t n_launches = 0;   // kernels of this library launched so far

@@ -35,7 +35,7 @@ class Workload:
     support: object        # int (uniform) or ("ragged", S_min, S_max): each side applies rule K6 itself
     oversample: int
     sources: dict = field(default_factory=dict)   # flux, l, m
-    notes: dict = field(default_factory=dict)
+    notes: dict = field(default_factory=dict)     # e.g. row_block: rows per time step (rows are dump-major)
 
     @property
     def nvis(self):
@@ -174,7 +174,7 @@ def config2(nvis=10_000_000, seed=SEED0 + 2, device=None, n_dump=4961, noise=Tru
     src = _sources(rng, 20, 0.3 * N * cell)
     vis = _fill_vis(rng, uvw, freq, src, device, noise)
     return Workload("config2", uvw, freq, vis, np.ones(vis.shape, np.float32),
-                    N, cell, 32, w_max, 8, 8, src)
+                    N, cell, 32, w_max, 8, 8, src, notes={"row_block": E.size * (E.size - 1) // 2})
 
 
 def config3(N=2048, S=8, nvis=50_000_000, seed=SEED0 + 3):
@@ -230,7 +230,7 @@ def config4(n_dump=360, nchan=8, seed=SEED0 + 4, device=None, max_rows=None, noi
         vis.real[...] = rng.standard_normal(vis.shape, dtype=np.float32)
         vis.imag[...] = rng.standard_normal(vis.shape, dtype=np.float32)
     return Workload("config4", uvw, freq, vis, np.ones(vis.shape, np.float32),
-                    N, cell, Nw, w_max, ("ragged", 8, 32), 8, src)
+                    N, cell, Nw, w_max, ("ragged", 8, 32), 8, src, notes={"row_block": E.size * (E.size - 1) // 2})
 
 
 def config5(nvis=100_000_000, seed=SEED0 + 5, device=None, n_dump=3064, noise=True):
@@ -245,7 +245,7 @@ def config5(nvis=100_000_000, seed=SEED0 + 5, device=None, n_dump=3064, noise=Tr
     src = _sources(rng, 20, 0.3 * N * cell)
     vis = _fill_vis(rng, uvw, freq, src, device, noise)
     return Workload("config5", uvw, freq, vis, np.ones(vis.shape, np.float32),
-                    N, cell, 64, w_max, 16, 8, src)
+                    N, cell, 64, w_max, 16, 8, src, notes={"row_block": E.size * (E.size - 1) // 2})
 
 
 def tiny_dft_case(seed=SEED0, N=64, fov=0.08, nvis=300, w_abs=60.0, nsrc=3, src_half=0.02,

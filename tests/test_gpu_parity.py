@@ -273,6 +273,7 @@ def test_config2_full_size_as_benchmarked(ctx):
     ks = ctx.wkernel_build(wl.Nw, wl.w_max, wl.support, wl.oversample, wl.grid_N, wl.cell, wpgrid.F32)
     ws = torch.empty(ctx.grid_workspace_bytes(wl.uvw.shape[0], 1, ks), dtype=torch.uint8, device="cuda")
     grid = ctx.new_grid(ks)
+    ctx.set_option("row_block", wl.notes["row_block"])  # as bench.py does for track-based workloads
     for _ in range(2):                                  # twice: workspace reuse, as in the timed loop
         grid.zero_()
         g, s = ctx.grid(*d, ks, grid=grid, workspace=ws, stats=True)
@@ -280,6 +281,7 @@ def test_config2_full_size_as_benchmarked(ctx):
         gh = g.cpu().numpy()
         assert relerr(gh, ref) <= TOL[wpgrid.F32]
         assert abs(gh.sum(dtype=np.complex128) - ref.sum()) <= 1e-5 * abs(ref.sum())
+    ctx.set_option("row_block", 0)
     # dirty image of the full grid
     wsum = float(wl.weight.sum())
     img = ctx.dirty_image(g, ks, wsum).cpu().numpy().astype(np.float64)
@@ -353,3 +355,33 @@ def test_ragged_stack_key_budgets_both_precisions(ctx):
     ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
     assert len(set(st.support.tolist())) >= 4
     check_all_paths(ctx, wl, st, ref, rstats, key_bits=(0, 8, 20, 27))
+
+
+def test_row_block_hint_changes_nothing_but_speed(ctx):
+    """The rows-per-time-step hint only re-maps binning threads to visibilities (same baseline at consecutive
+    times, one bucket-counter update per run of equal keys): counters bit-exact, grid within tolerance, for a
+    track-based workload, for a block size that does not divide the row count, and with several channels."""
+    wl = synth.config2(nvis=400_001)
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    for rb in (wl.notes["row_block"], 1, 777):
+        ctx.set_option("row_block", rb)
+        check_all_paths(ctx, wl, st, ref, rstats, precs=(wpgrid.F32,))
+    rng = np.random.default_rng(5)
+    N, cell, Q, S, Nw, w_max = 256, 0.1 / 256, 8, 8, 8, 100.0
+    nrow, nchan = 40_000, 2
+    # slowly drifting tracks: 123 "baselines", consecutive time steps move by a fraction of a cell
+    b = np.arange(nrow) % 123; t = np.arange(nrow) // 123
+    uvw = np.stack([(b - 60) * 9.0 + 0.7 * t, (b % 11 - 5) * 80.0 + 0.4 * t, rng.uniform(-90, 90, 123)[b]], 1)
+    freq = np.array([1.0, 1.02]) * synth.C0 / 0.5
+    vis = (rng.standard_normal((nrow, nchan)) + 1j * rng.standard_normal((nrow, nchan))).astype(np.complex64)
+    wt = rng.uniform(0.0, 2.0, (nrow, nchan)).astype(np.float32)
+    wt[rng.uniform(size=wt.shape) < 0.05] = 0.0
+    st = owk.build_stack(Nw, w_max, S, Q, N, cell)
+    ref, rstats = ogrid.grid(uvw, vis, wt, freq, st)
+    assert rstats["n_gridded"] > 50_000
+    wl2 = synth.Workload("tracks", uvw, freq, vis, wt, N, cell, Nw, w_max, S, Q)
+    for rb in (123, 0):
+        ctx.set_option("row_block", rb)
+        check_all_paths(ctx, wl2, st, ref, rstats)
+    ctx.set_option("row_block", 0)
