@@ -27,10 +27,6 @@ template <> struct Cplx<double> { using type = double2; };
 __device__ __forceinline__ void red_add(float2 *addr, float2 v) {
     asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(addr), "f"(v.x), "f"(v.y) : "memory");
 }
-// two adjacent cells at once; addr must be 16-byte aligned
-__device__ __forceinline__ void red_add4(float2 *addr, float2 a, float2 b) {
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y) : "memory");
-}
 __device__ __forceinline__ void red_add(double2 *addr, double2 v) {
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&addr->x), "d"(v.x) : "memory");
     asm volatile("red.global.add.f64 [%0], %1;" ::"l"(&addr->y), "d"(v.y) : "memory");
