@@ -300,13 +300,20 @@ __device__ __forceinline__ void ldg128(const float2 *p, unsigned long long &c0, 
 // G > 1 (small supports: S*S/2 <= 32/G pairs, NSLOT = 1): the warp is split into G groups of 32/G lanes and
 // every group takes its own record, G records per step (record t*G + g goes to group g), so that a 4x4
 // support does not leave three quarters of the warp idle.
-template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1>
+// RPS > 0: a slot holds RPS whole window rows (RPS * S/2 <= 32 lanes, the rest idle) instead of 32 consecutive
+// pairs: for S = 12 four rows are 384 bytes = three whole 128-byte lines of the slice, where 32 consecutive pairs
+// (5 1/3 rows) straddle five, and the coefficient loads are bound by the lines they touch.
+// ST: the producer keeps the lane-slots' offsets of the current window and re-derives them only when the window
+// start changes (supports that are not a power of two pay ~25 instructions per slot for the modulo arithmetic;
+// for powers of two the two-instruction stateless form is cheaper than the test).
+template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1, int RPS = 0, bool ST = false>
 __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
                   const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
                   const float2 *__restrict__ K, float2 *__restrict__ grid, int N, unsigned seg) {
     static_assert(kChunk % (DEPTH * G) == 0, "a look-ahead step divides the chunk");
     static_assert(G == 1 || NSLOT == 1, "lane groups only for one-slot supports");
+    static_assert(!ST || G == 1, "window tracking in the producer needs one window per warp");
     constexpr int LPG = 32 / G;                          // lanes per group
     using U64 = unsigned long long;
     const int S = SCT ? SCT : S_rt;
@@ -332,19 +339,26 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     for (int k = 0; k < NSLOT; ++k) {
         int r = k * 32 + (G > 1 ? lane % LPG : lane);
         act[k] = r < NP;
+        if (RPS) {                                       // RPS rows per slot
+            const int row = k * RPS + lane / H;
+            act[k] = lane < RPS * H && row < S;
+            r = row * H + lane % H;
+        }
         r = act[k] ? r : 0;
         rb[k] = r / H;
         ra2p1[k] = 2 * (r - rb[k] * H) + 1;
         RG[k] = (0x8000u + (unsigned)ra2p1[k]) | ((0x8000u + (unsigned)rb[k]) << 16);
     }
-    constexpr unsigned M = SCT ? ((unsigned)(SCT - 2) | ((unsigned)(SCT - 1) << 16)) : 0u;
+    constexpr bool POW2 = SCT > 0 && (SCT & (SCT - 1)) == 0;       // compile-time S that is not a power of two: generic formula, constant folded
+    constexpr unsigned M = POW2 ? ((unsigned)(SCT - 2) | ((unsigned)(SCT - 1) << 16)) : 0u;
 
     // (iu0 | iv << 16) of this lane-slot for a window starting at pos = j0u | j0v << 16
     auto offset_in_window = [&](unsigned pos, int k) -> unsigned {
-        if (SCT) return (RG[k] - pos) & M;
+        if (POW2) return (RG[k] - pos) & M;
         const unsigned j0u = pos & 0xFFFFu, j0v = pos >> 16;
-        const int ju = (int)(j0u - ((j0u * magicS) >> 20) * (unsigned)S);     // j0u mod S
-        const int jv = (int)(j0v - ((j0v * magicS) >> 20) * (unsigned)S);
+        const unsigned mg = SCT ? (1u << 20) / (unsigned)(SCT ? SCT : 1) + 1u : magicS;
+        const int ju = (int)(j0u - ((j0u * mg) >> 20) * (unsigned)S);     // j0u mod S
+        const int jv = (int)(j0v - ((j0v * mg) >> 20) * (unsigned)S);
         int x = ra2p1[k] - ju; x += x < 0 ? S : 0;
         int y = rb[k] - jv;    y += y < 0 ? S : 0;
         return (unsigned)(x & ~1) | ((unsigned)y << 16);
@@ -376,6 +390,9 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         // Write the pair out and clear its sums.  One asm statement with the accumulators as read-write
         // operands: the cleared value then lives in the SAME register as the sum (a separate "acc = 0"
         // makes the compiler keep two copies alive and pay moves for it on every record).
+        unsigned posP = 0xFFFFFFFFu, dP[NSLOT], cP[NSLOT];  // ST: window of the last record produced, offsets in it
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) dP[k] = cP[k] = 0;
         auto flush = [&](int k) {
             const unsigned q = qcur[k];
             float2 *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
@@ -398,6 +415,22 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
             vis[s] = valid ? *reinterpret_cast<const U64 *>(rp) : 0ull;
             const uint2 pk = valid ? *reinterpret_cast<const uint2 *>(&rp->pos) : make_uint2(0u, 0u);
             const unsigned pos = pk.x, koff = pk.y;
+            if (ST) {
+                if (__any_sync(0xffffffffu, pos != posP)) {
+#pragma unroll
+                    for (int k = 0; k < NSLOT; ++k) {
+                        dP[k] = offset_in_window(pos, k);
+                        cP[k] = act[k] ? (dP[k] >> 16) * (unsigned)S + (dP[k] & 0xFFFFu) : 0u;
+                    }
+                    posP = pos;
+                }
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    qn[s][k] = act[k] && valid ? pos + dP[k] : 0xFFFFFFFFu;
+                    ldg128(K + (koff + cP[k]), c0[s][k], c1[s][k]);
+                }
+                return;
+            }
 #pragma unroll
             for (int k = 0; k < NSLOT; ++k) {
                 const unsigned d = offset_in_window(pos, k);
@@ -470,7 +503,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     }
 }
 
-template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1>
+template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1, int RPS = 0, bool ST = false>
 int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                  int cls, int S) {
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
@@ -478,7 +511,7 @@ int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;         // (x * magicS) >> 20 == x / S for x < 2^13, S <= 32
-    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB, G><<<blocks, kRunThreads, 0, ctx->stream>>>(
+    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB, G, RPS, ST><<<blocks, kRunThreads, 0, ctx->stream>>>(
         (const Rec<float> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
         bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
         (const float2 *)K, (float2 *)grid, bp.N, seg);
@@ -672,12 +705,13 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
         if (S == 8) return launch_pairs<8, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
         if (S == 16) return launch_pairs<16, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
         if (S == 4) return launch_pairs<4, 1, 4, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);        // 8 pairs: 4 records per step
-        if (nslot <= 1) return launch_pairs<0, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 2) return launch_pairs<0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 3) return launch_pairs<0, 3, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 4) return launch_pairs<0, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 6) return launch_pairs<0, 6, 1, 2>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 8) return launch_pairs<0, 8, 1, 1>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 12) return launch_pairs<12, 3, 2, 3, 1, 4, true>(ctx, bp, ws, K, grid, w, cls, S);     // 4 rows per slot
+        if (nslot <= 1) return launch_pairs<0, 1, 4, 4, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 2) return launch_pairs<0, 2, 4, 3, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 3) return launch_pairs<0, 3, 2, 3, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 4) return launch_pairs<0, 4, 2, 2, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 6) return launch_pairs<0, 6, 1, 2, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 8) return launch_pairs<0, 8, 1, 1, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
     }
     if (!F && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp64: one cell per lane-slot, S*S cells over 32 lanes
