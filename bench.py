@@ -350,6 +350,21 @@ def run_b200(args):
                 # on-chip coefficient feed: 128 B/clk/SM of L1 / 8 B (c64) or 16 B (c128) per update
                 "l1_feed_frac": (n_updates / (grid_ms * 1e-3)) /
                                 (SM_COUNT * (16 if prec == wpgrid.F32 else 8) * SM_MAX_GHZ * 1e9)}
+    # atomic roofline (BASELINE metric: "% of HBM/atomic roofline"): the measured reduction rate into a buffer of
+    # the grid's size is the ceiling of a one-atomic-per-update design; the naive gridder is that design
+    red_per_s, _ = ctx.microbench(0, 1000, max(1 << 25, wl.grid_N * wl.grid_N * 8))
+    g_naive = ctx.new_grid(stack)
+    ctx.grid_naive(d_vis, d_uvw, d_wt, d_freq, stack, grid=g_naive)
+    n0, n1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0.record()
+    for _ in range(3):
+        ctx.grid_naive(d_vis, d_uvw, d_wt, d_freq, stack, grid=g_naive)
+    n1.record(); torch.cuda.synchronize()
+    naive_ms = n0.elapsed_time(n1) / 3
+    del g_naive
+    roofline["atomic"] = {"red_v2_f32_per_s": red_per_s, "naive_gridder_updates_per_s": n_updates / (naive_ms * 1e-3),
+                          "gridder_over_red_ceiling": (n_updates / (grid_ms * 1e-3)) / red_per_s,
+                          "note": "measured after the timed region; fp32 reduction rate also quoted for fp64 runs"}
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
             hbm_gbs = json.load(f)["hbm_gbs"]; src = "measured"

@@ -149,6 +149,15 @@ int  wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *
              void *d_workspace, size_t workspace_bytes, wpg_bin_info *h_info_out,
              wpg_stats *h_stats_or_null);
 
+/* Machine-limit microbenchmarks (instrumentation; SURVEY.md §8(d) wants fractions of MEASURED peaks).
+ * which: 0 = red.global.add.v2.f32, a warp per 256-byte row segment at a pseudo-random place of the buffer (the
+ *            naive gridder's pattern; "write access ... in an atomic manner");
+ *        1 = the same, every lane its own pseudo-random cell;   2 = L1-resident 16-byte loads;
+ *        3 = fma.rn.f32x2;   4 = fma.rn.f64.
+ * d_buf: device scratch, buf_bytes >= 1 MiB (the reductions use the largest power-of-two number of 8-byte cells
+ * that fits; its contents are overwritten).  h_out[0] = operations/s, h_out[1] = kernel ms.  Synchronises. */
+int  wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_bytes, double *h_out /*[2]*/);
+
 /* ---- a3: dirty image — PAPER.md:52, 88 (IFFT of the grid), R11 (grid correction) ---------- */
 size_t wpg_dirty_image_workspace_bytes(int grid_N, wpg_prec prec);
 /* image[jm][jl] = Re(centred inverse FFT of grid) * N^2-normalised / weight_sum / taper;

@@ -429,14 +429,14 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
                     qn[s][k] = act[k] && valid ? pos + dP[k] : 0xFFFFFFFFu;
                     ldg128(K + (koff + cP[k]), c0[s][k], c1[s][k]);
                 }
-                return;
-            }
+            } else {
 #pragma unroll
-            for (int k = 0; k < NSLOT; ++k) {
-                const unsigned d = offset_in_window(pos, k);
-                qn[s][k] = act[k] && valid ? pos + d : 0xFFFFFFFFu;
-                const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
-                ldg128(K + (koff + (act[k] ? coff : 0u)), c0[s][k], c1[s][k]);
+                for (int k = 0; k < NSLOT; ++k) {
+                    const unsigned d = offset_in_window(pos, k);
+                    qn[s][k] = act[k] && valid ? pos + d : 0xFFFFFFFFu;
+                    const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
+                    ldg128(K + (koff + (act[k] ? coff : 0u)), c0[s][k], c1[s][k]);
+                }
             }
         };
         auto consume = [&](int s) {

@@ -1,0 +1,114 @@
+// Microbenchmarks of the machine limits the gridder is read against ("fractions of
+// MEASURED peaks"): the global reduction rate (the ceiling of the naive one-atomic-per-update design and of the
+// paper's own kernel), the L1 coefficient feed (one LDG.128 per two fp32 updates), and the packed
+// FP32 / FP64 FMA issue rates.  Instrumentation only: nothing on the gridding path calls these.
+#include "wpg_common.h"
+
+namespace {
+
+// which = 0: red.global.add.v2.f32, consecutive lanes -> consecutive cells, every warp its own 256-byte segment
+//            picked pseudo-randomly in the buffer (the naive gridder's pattern: a window row per 8 lanes);
+// which = 1: the same instruction, every LANE its own pseudo-random cell (worst case);
+__global__ void __launch_bounds__(256)
+micro_red_kernel(float2 *__restrict__ buf, unsigned ncell_mask, int iters, int scattered) {
+    const unsigned gtid = blockIdx.x * 256u + threadIdx.x;
+    const unsigned lane = threadIdx.x & 31u, gwarp = gtid >> 5;
+    unsigned x = (scattered ? gtid : gwarp) * 2654435761u + 12345u;
+    for (int i = 0; i < iters; ++i) {
+        x = x * 1664525u + 1013904223u;
+        const unsigned cell = scattered ? ((x >> 4) & ncell_mask) : ((((x >> 4) & ncell_mask) & ~31u) + lane);
+        asm volatile("red.global.add.v2.f32 [%0], {%1, %2};" ::"l"(buf + cell), "f"(1.0f), "f"(0.5f) : "memory");
+    }
+}
+
+// which = 2: L1-resident LDG.128: every warp re-reads its own eight 512-byte slices (32 lanes x 16 B each; 4 KB per
+// warp, 16 warps per SM), 8 loads in flight; the slice order rotates with the trip count so that the read-only
+// loads can be neither merged nor hoisted
+__global__ void __launch_bounds__(256)
+micro_l1_kernel(const float4 *src, float *sink, int iters) {
+    const unsigned gwarp = (blockIdx.x * 256u + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
+    const float4 *p = src + (size_t)(gwarp & 4095u) * 256u + lane;
+    float acc = 0.f;
+    for (int i = 0; i < iters; ++i) {
+        float4 v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v[k].x), "=f"(v[k].y), "=f"(v[k].z), "=f"(v[k].w) : "l"(p + ((i + k) & 7) * 32));
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc += v[k].x + v[k].w;
+    }
+    if (acc == 123.456f) sink[0] = acc;
+}
+
+// which = 3: fma.rn.f32x2 issue rate, 8 independent accumulator pairs per thread
+__global__ void __launch_bounds__(256)
+micro_ffma2_kernel(float *__restrict__ sink, int iters, float seed) {
+    unsigned long long a[8], b, c;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b) : "f"(seed), "f"(seed + 1.f));
+    asm("mov.b64 %0, {%1, %1};" : "=l"(c) : "f"(0.999f));
+#pragma unroll
+    for (int k = 0; k < 8; ++k) asm("mov.b64 %0, {%1, %2};" : "=l"(a[k]) : "f"((float)k), "f"(seed));
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(a[k]) : "l"(b), "l"(c));
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(a[k])); s += x + y; }
+    if (s == 123.456f) sink[0] = s;
+}
+
+// which = 4: fma.rn.f64 issue rate, 8 independent accumulators per thread
+__global__ void __launch_bounds__(256)
+micro_dfma_kernel(double *__restrict__ sink, int iters, double seed) {
+    double a[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) a[k] = seed + k;
+    const double b = seed * 0.5, c = 0.999;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) a[k] = fma(a[k], c, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) s += a[k];
+    if (s == 123.456) sink[0] = s;
+}
+
+}  // namespace
+
+// h_out[0] = operations per second (reductions of one cell, 16-byte loads, packed FMAs = 2 FMA, FMAs),
+// h_out[1] = kernel milliseconds.  d_buf: device scratch of at least buf_bytes >= 1 MiB (power of two used).
+extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_bytes, double *h_out) {
+    if (!ctx || !h_out || !d_buf) return WPG_EINVAL;
+    if (which < 0 || which > 4 || iters < 1 || buf_bytes < ((size_t)1 << 20))
+        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which 0..4, iters >= 1, buffer >= 1 MiB");
+    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    size_t ncell = 1;
+    while (ncell * 2 * sizeof(float2) <= buf_bytes) ncell *= 2;
+    if (which == 2 && buf_bytes < ((size_t)16 << 20)) return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which = 2 needs a 16 MiB buffer");
+    const int blocks = ctx->sm_count * (which == 2 ? 2 : 8);
+    cudaEvent_t e0, e1;
+    WPG_CUDA(ctx, cudaEventCreate(&e0));
+    WPG_CUDA(ctx, cudaEventCreate(&e1));
+    cudaStream_t s = ctx->stream;
+    for (int rep = 0; rep < 2; ++rep) {            // the first repetition warms up
+        WPG_CUDA(ctx, cudaEventRecord(e0, s));
+        if (which <= 1) micro_red_kernel<<<blocks, 256, 0, s>>>((float2 *)d_buf, (unsigned)(ncell - 1), iters, which);
+        else if (which == 2) micro_l1_kernel<<<blocks, 256, 0, s>>>((const float4 *)d_buf, (float *)d_buf, iters);
+        else if (which == 3) micro_ffma2_kernel<<<blocks, 256, 0, s>>>((float *)d_buf, iters, 1.0f);
+        else micro_dfma_kernel<<<blocks, 256, 0, s>>>((double *)d_buf, iters, 1.0);
+        WPG_CUDA(ctx, cudaEventRecord(e1, s));
+        ctx->n_launches += 1;
+    }
+    WPG_CUDA(ctx, cudaEventSynchronize(e1));
+    float ms = 0.f;
+    WPG_CUDA(ctx, cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    WPG_CUDA(ctx, cudaGetLastError());
+    const double threads = (double)blocks * 256.0;
+    const double ops = threads * (double)iters * (which == 0 || which == 1 ? 1.0 : 8.0);
+    h_out[0] = ops / (ms * 1e-3);
+    h_out[1] = ms;
+    return WPG_OK;
+}

@@ -20,7 +20,7 @@ EXPORTS = (
     "wpg_create", "wpg_destroy", "wpg_last_error", "wpg_version", "wpg_set_option", "wpg_taper",
     "wpg_ragged_support", "wpg_wkernel_elems", "wpg_wkernel_build", "wpg_grid_workspace_bytes",
     "wpg_grid", "wpg_grid_naive", "wpg_grid_host", "wpg_bin", "wpg_dirty_image_workspace_bytes",
-    "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms",
+    "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms", "wpg_microbench",
 )
 
 
@@ -90,6 +90,7 @@ def load():
     lib.wpg_dirty_image.argtypes = [vp, vp, kd, dbl, cint, vp, vp, sz]; lib.wpg_dirty_image.restype = cint
     lib.wpg_launch_count.argtypes = [vp]; lib.wpg_launch_count.restype = i64
     lib.wpg_phase_ms.argtypes = [vp, ctypes.POINTER(dbl)]; lib.wpg_phase_ms.restype = cint
+    lib.wpg_microbench.argtypes = [vp, cint, cint, vp, sz, ctypes.POINTER(dbl)]; lib.wpg_microbench.restype = cint
     _lib = lib
     return lib
 
@@ -186,6 +187,14 @@ class Context:
         """(binning ms, gridder ms) of the last wpg_grid call made with option "timing" = 1."""
         out = (ctypes.c_double * 2)()
         self._check(self.lib.wpg_phase_ms(self.h, out))
+        return float(out[0]), float(out[1])
+
+    def microbench(self, which, iters=2000, buf_bytes=1 << 25):
+        """(operations/s, ms) of machine-limit microbenchmark `which` (see wpg_microbench in wpgrid.h)."""
+        t = self.torch
+        buf = t.zeros(buf_bytes, dtype=t.uint8, device=self.device)
+        out = (ctypes.c_double * 2)()
+        self._check(self.lib.wpg_microbench(self.h, int(which), int(iters), buf.data_ptr(), buf.numel(), out))
         return float(out[0]), float(out[1])
 
     # ---- a0
