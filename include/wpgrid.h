@@ -149,6 +149,27 @@ int  wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *
              void *d_workspace, size_t workspace_bytes, wpg_bin_info *h_info_out,
              wpg_stats *h_stats_or_null);
 
+/* ---- the paper's own data order: Eqs. (1)-(2), PAPER.md:62-84 -------------------------
+ * Baseline index I_B = (-S^2 + 2 S N_ant + S)/2 + |ant1 - ant2|, S = min(ant1, ant2)  (Eq. 1; autocorrelation
+ * slots included: N_ant (N_ant + 1) / 2 values), count array C, B_start_index = exclusive prefix sum of C (Eq. 2),
+ * rows re-ordered "grouped by baseline and then ordered by time" (time = input row order: a stable re-order).
+ *   d_ant1, d_ant2  int32 [nrow] antenna IDs in 0 .. n_ant - 1 (n_ant <= 4096); at most 8192 rows per baseline
+ *                   and call (WPG_EINVAL otherwise — chunk the input in time).
+ * wpg_baseline_reorder: the re-order alone (tests): d_bstart_out u32 [N_ant (N_ant + 1) / 2 + 1] = Eq. (2) with the
+ *   row count appended, d_perm_out u32 [nrow], perm[slot] = input row.  Synchronises.
+ * wpg_grid_baseline_order: grid += gridding of all visibilities as wpg_grid does (same arguments, uniform stacks
+ *   only), but with the records in baseline-then-time order and no position sort: the register accumulator
+ *   walks each baseline's time series and writes out when the grid point changes.  Same result
+ *   as wpg_grid up to summation order.  Synchronises once (after the re-order, to check the antenna IDs). */
+size_t wpg_baseline_workspace_bytes(int64_t nrow, int nchan, int n_ant, wpg_prec prec);
+int  wpg_baseline_reorder(wpg_ctx *ctx, const int *d_ant1, const int *d_ant2, int n_ant, int64_t nrow,
+                          unsigned *d_bstart_out, unsigned *d_perm_out, void *d_workspace, size_t workspace_bytes);
+int  wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                             const double *d_freq, const int *d_ant1, const int *d_ant2, int n_ant,
+                             int64_t nrow, int nchan, const void *d_kernels, const wpg_kdesc *desc,
+                             wpg_prec prec, void *d_grid, void *d_workspace, size_t workspace_bytes,
+                             wpg_stats *h_stats_or_null);
+
 /* Machine-limit microbenchmarks (instrumentation; SURVEY.md §8(d) wants fractions of MEASURED peaks).
  * which: 0 = red.global.add.v2.f32, a warp per 256-byte row segment at a pseudo-random place of the buffer (the
  *            naive gridder's pattern; "write access ... in an atomic manner");

@@ -375,6 +375,19 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
 
 }  // namespace
 
+// Exclusive prefix sum of hist[0 .. n-1] in place, hist[n] = total (also written to ctr->n_records);
+// blocksum: ceil((n + 1) / 4096) words of scratch.  Shared with the baseline re-order (wpg_baseline.cu, Eq. 2).
+int wpg_launch_exclusive_scan(wpg_ctx *ctx, unsigned *hist, unsigned n, unsigned *blocksum, Counters *ctr) {
+    const unsigned nblocks = (n + 1 + kScanBlock - 1) / kScanBlock;
+    cudaStream_t s = ctx->stream;
+    scan_reduce_kernel<<<nblocks, 1024, 0, s>>>(hist, n, blocksum);
+    scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, nblocks, ctr);
+    scan_apply_kernel<<<nblocks, 1024, 0, s>>>(hist, n, blocksum);
+    ctx->n_launches += 3;
+    WPG_CUDA(ctx, cudaGetLastError());
+    return WPG_OK;
+}
+
 int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
                    const double *d_freq, const PlaneTab &tab, const BinParams &bp,
                    const WorkspaceLayout &ws, wpg_prec prec, char *w) {

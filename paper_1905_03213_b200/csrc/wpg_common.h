@@ -111,6 +111,7 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
 void wpg_pswf_eval(const double *nu, int64_t n, double *out);     // wpg_pswf.cu (host)
 
 // launchers
+int wpg_launch_exclusive_scan(wpg_ctx *ctx, unsigned *hist, unsigned n, unsigned *blocksum, Counters *ctr);
 int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
                    const double *d_freq, const PlaneTab &tab, const BinParams &bp,
                    const WorkspaceLayout &ws, wpg_prec prec, char *d_ws);

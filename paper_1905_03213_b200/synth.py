@@ -122,6 +122,14 @@ def earth_rotation_uvw(E, N, n_dump, dt=10.0, dec_deg=DEC_DEG, lat_deg=LAT_DEG, 
     return np.ascontiguousarray(out)
 
 
+def track_antennas(n_ant, nrow):
+    """Antenna IDs (int32) of the rows earth_rotation_uvw produces: dump-major, baselines (i < j) in
+    np.triu_indices order within a dump."""
+    i, j = np.triu_indices(n_ant, k=1)
+    reps = -(-nrow // i.size)
+    return (np.tile(i, reps)[:nrow].astype(np.int32), np.tile(j, reps)[:nrow].astype(np.int32))
+
+
 def _disc_layout(rng, n, radius):
     r = radius * np.sqrt(rng.uniform(0, 1, n)); th = rng.uniform(0, 2 * math.pi, n)
     return r * np.cos(th), r * np.sin(th)
@@ -174,7 +182,7 @@ def config2(nvis=10_000_000, seed=SEED0 + 2, device=None, n_dump=4961, noise=Tru
     src = _sources(rng, 20, 0.3 * N * cell)
     vis = _fill_vis(rng, uvw, freq, src, device, noise)
     return Workload("config2", uvw, freq, vis, np.ones(vis.shape, np.float32),
-                    N, cell, 32, w_max, 8, 8, src, notes={"row_block": E.size * (E.size - 1) // 2})
+                    N, cell, 32, w_max, 8, 8, src, notes={"row_block": E.size * (E.size - 1) // 2, "n_ant": int(E.size)})
 
 
 def config3(N=2048, S=8, nvis=50_000_000, seed=SEED0 + 3):
@@ -230,7 +238,7 @@ def config4(n_dump=360, nchan=8, seed=SEED0 + 4, device=None, max_rows=None, noi
         vis.real[...] = rng.standard_normal(vis.shape, dtype=np.float32)
         vis.imag[...] = rng.standard_normal(vis.shape, dtype=np.float32)
     return Workload("config4", uvw, freq, vis, np.ones(vis.shape, np.float32),
-                    N, cell, Nw, w_max, ("ragged", 8, 32), 8, src, notes={"row_block": E.size * (E.size - 1) // 2})
+                    N, cell, Nw, w_max, ("ragged", 8, 32), 8, src, notes={"row_block": E.size * (E.size - 1) // 2, "n_ant": int(E.size)})
 
 
 def config5(nvis=100_000_000, seed=SEED0 + 5, device=None, n_dump=3064, noise=True):
@@ -245,7 +253,7 @@ def config5(nvis=100_000_000, seed=SEED0 + 5, device=None, n_dump=3064, noise=Tr
     src = _sources(rng, 20, 0.3 * N * cell)
     vis = _fill_vis(rng, uvw, freq, src, device, noise)
     return Workload("config5", uvw, freq, vis, np.ones(vis.shape, np.float32),
-                    N, cell, 64, w_max, 16, 8, src, notes={"row_block": E.size * (E.size - 1) // 2})
+                    N, cell, 64, w_max, 16, 8, src, notes={"row_block": E.size * (E.size - 1) // 2, "n_ant": int(E.size)})
 
 
 def tiny_dft_case(seed=SEED0, N=64, fov=0.08, nvis=300, w_abs=60.0, nsrc=3, src_half=0.02,

@@ -21,6 +21,7 @@ EXPORTS = (
     "wpg_ragged_support", "wpg_wkernel_elems", "wpg_wkernel_build", "wpg_grid_workspace_bytes",
     "wpg_grid", "wpg_grid_naive", "wpg_grid_host", "wpg_bin", "wpg_dirty_image_workspace_bytes",
     "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms", "wpg_microbench",
+    "wpg_baseline_workspace_bytes", "wpg_baseline_reorder", "wpg_grid_baseline_order",
 )
 
 
@@ -90,6 +91,10 @@ def load():
     lib.wpg_dirty_image.argtypes = [vp, vp, kd, dbl, cint, vp, vp, sz]; lib.wpg_dirty_image.restype = cint
     lib.wpg_launch_count.argtypes = [vp]; lib.wpg_launch_count.restype = i64
     lib.wpg_phase_ms.argtypes = [vp, ctypes.POINTER(dbl)]; lib.wpg_phase_ms.restype = cint
+    lib.wpg_baseline_workspace_bytes.argtypes = [i64, cint, cint, cint]; lib.wpg_baseline_workspace_bytes.restype = sz
+    lib.wpg_baseline_reorder.argtypes = [vp, vp, vp, cint, i64, vp, vp, vp, sz]; lib.wpg_baseline_reorder.restype = cint
+    lib.wpg_grid_baseline_order.argtypes = [vp, vp, vp, vp, vp, vp, vp, cint, i64, cint, vp, kd, cint, vp, vp, sz, stp]
+    lib.wpg_grid_baseline_order.restype = cint
     lib.wpg_microbench.argtypes = [vp, cint, cint, vp, sz, ctypes.POINTER(dbl)]; lib.wpg_microbench.restype = cint
     _lib = lib
     return lib
@@ -276,6 +281,38 @@ class Context:
                                            ptr(out), ctypes.byref(st) if stats else None,
                                            ptr(image_out) if image_out is not None else None, float(weight_sum)))
         return out, (st.as_dict() if stats else None)
+
+    # ---- the paper's baseline-then-time order (Eqs. 1-2)
+    def baseline_reorder(self, ant1, ant2, n_ant):
+        """(B_start_index [nb + 1], perm [nrow]) as torch int32-sized unsigned tensors (values < 2^31 here)."""
+        t = self.torch
+        assert ant1.dtype == t.int32 and ant2.dtype == t.int32 and ant1.is_cuda and ant2.is_cuda
+        nrow = ant1.numel()
+        nb = n_ant * (n_ant + 1) // 2
+        bstart = t.empty(nb + 1, dtype=t.int32, device=self.device)
+        perm = t.empty(max(nrow, 1), dtype=t.int32, device=self.device)
+        need = int(self.lib.wpg_baseline_workspace_bytes(nrow, 1, n_ant, F32))
+        ws = t.empty(need, dtype=t.uint8, device=self.device)
+        self._check(self.lib.wpg_baseline_reorder(self.h, ant1.data_ptr(), ant2.data_ptr(), n_ant, nrow,
+                                                  bstart.data_ptr(), perm.data_ptr(), ws.data_ptr(), ws.numel()))
+        return bstart, perm[:nrow]
+
+    def grid_baseline_order(self, vis, uvw, weight, freq, ant1, ant2, n_ant, stack, grid=None, workspace=None, stats=False):
+        """grid += gridding(vis) with the records in the paper's baseline-then-time order."""
+        t = self.torch
+        nrow, nchan = self._inputs(vis, uvw, weight, freq)
+        assert ant1.dtype == t.int32 and ant2.dtype == t.int32 and ant1.numel() == nrow and ant2.numel() == nrow
+        if grid is None:
+            grid = self.new_grid(stack)
+        if workspace is None:
+            need = int(self.lib.wpg_baseline_workspace_bytes(nrow, nchan, n_ant, stack.prec))
+            workspace = t.empty(need, dtype=t.uint8, device=self.device)
+        st = Stats()
+        self._check(self.lib.wpg_grid_baseline_order(
+            self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(), ant1.data_ptr(), ant2.data_ptr(),
+            n_ant, nrow, nchan, stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec, grid.data_ptr(),
+            workspace.data_ptr(), workspace.numel(), ctypes.byref(st) if stats else None))
+        return grid, (st.as_dict() if stats else None)
 
     def bin(self, vis, uvw, weight, freq, stack, workspace=None):
         """Step a1 alone.  Returns (workspace tensor, BinInfo dict, stats dict)."""
