@@ -49,6 +49,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--option", action="append", default=[], help="library option name=value (tuning)")
+    ap.add_argument("--order", default="position", choices=["position", "baseline"],
+                    help="position: wpg_grid (sort by window start); baseline: the paper's Eq. (1)-(2) order, "
+                         "wpg_grid_baseline_order (track-based workloads, uniform stacks)")
     ap.add_argument("--no-row-block", action="store_true",
                     help="do not pass the rows-per-time-step hint of track-based workloads to the library")
     return ap.parse_args()
@@ -74,12 +77,12 @@ def make_workload(spec, nvis, device):
     raise SystemExit("unknown workload %r" % spec)
 
 
-def workload_config(wl, prec):
+def workload_config(wl, prec, order="position"):
     return {"workload": wl.name, "grid_N": wl.grid_N, "nvis": int(wl.nvis), "nchan": int(wl.freq.size),
             "Nw": wl.Nw, "support": wl.support if np.isscalar(wl.support) else list(wl.support),
             "oversample": wl.oversample, "precision": prec,
             "step": "grid zero-fill + binning (a1) + gridder (a2) + dirty_image (a3); wkernel_build (a0) untimed",
-            "row_block": int(wl.notes.get("row_block", 0)),
+            "row_block": int(wl.notes.get("row_block", 0)), "order": order,
             "l2": "inputs (%.0f MB) larger than the 126 MB L2; no explicit flush" %
                   ((wl.uvw.nbytes + wl.vis.nbytes + wl.weight.nbytes) / 1e6)}
 
@@ -235,7 +238,7 @@ def traffic_from_profiles(workload, prec):
 
 def run_b200(args):
     import torch
-    from paper_1905_03213_b200 import wpgrid
+    from paper_1905_03213_b200 import synth, wpgrid
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -274,12 +277,24 @@ def run_b200(args):
     ws = torch.empty(ctx.grid_workspace_bytes(nrow, nchan, stack), dtype=torch.uint8, device=dev)
     iws = torch.empty(int(ctx.lib.wpg_dirty_image_workspace_bytes(wl.grid_N, prec)), dtype=torch.uint8, device=dev)
 
+    if args.order == "baseline":
+        n_ant = int(wl.notes["n_ant"])
+        a1, a2 = synth.track_antennas(n_ant, nrow)
+        d_a1, d_a2 = torch.from_numpy(a1).to(dev), torch.from_numpy(a2).to(dev)
+        ws = torch.empty(int(ctx.lib.wpg_baseline_workspace_bytes(nrow, nchan, n_ant, prec)), dtype=torch.uint8, device=dev)
+
+        def grid_call(g, stats=False):
+            return ctx.grid_baseline_order(d_vis, d_uvw, d_wt, d_freq, d_a1, d_a2, n_ant, stack, grid=g, workspace=ws, stats=stats)
+    else:
+        def grid_call(g, stats=False):
+            return ctx.grid(d_vis, d_uvw, d_wt, d_freq, stack, grid=g, workspace=ws, stats=stats)
+
     def step():
         grid.zero_()
-        ctx.grid(d_vis, d_uvw, d_wt, d_freq, stack, grid=grid, workspace=ws)
+        grid_call(grid)
         return ctx.dirty_image(grid, stack, wsum, workspace=iws)
 
-    _, stats = ctx.grid(d_vis, d_uvw, d_wt, d_freq, stack, grid=ctx.new_grid(stack), workspace=ws, stats=True)
+    _, stats = grid_call(ctx.new_grid(stack), stats=True)
     n_updates = stats["n_updates"]
     for _ in range(max(args.warmup, 3)):
         step()
@@ -375,7 +390,7 @@ def run_b200(args):
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": args.prec, "data": "synthetic", "config": workload_config(wl, args.prec),
+           "vs_baseline": None, "dtype": args.prec, "data": "synthetic", "config": workload_config(wl, args.prec, args.order),
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
            "stats": stats, "multi_gpu": "replicas only" if world > 1 else "single GPU"}
     if not args.no_cpu_baseline and world == 1:

@@ -233,7 +233,7 @@ extern "C" int wpg_phase_ms(wpg_ctx *ctx, double *out) {
 }
 
 // Event i (0 start, 1 after binning, 2 after gridder) of the current timed call.
-static int mark(wpg_ctx *ctx, int i) {
+int wpg_mark(wpg_ctx *ctx, int i) {
     if (!ctx->opt_timing) return WPG_OK;
     if (i == 0 && ctx->ev_used >= 4096) ctx->ev_used = 0;       // pool bound: start over
     size_t k = 3 * ctx->ev_used + (size_t)i;
@@ -257,7 +257,7 @@ static int bin_common(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, cons
     if (!d_workspace || workspace_bytes < ws->total)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, ws->total);
     WPG_CUDA(ctx, cudaSetDevice(ctx->device));
-    if ((rc = mark(ctx, 0))) return rc;
+    if ((rc = wpg_mark(ctx, 0))) return rc;
     char *w = (char *)d_workspace;
     // counters + histogram are contiguous at the head of the workspace
     WPG_CUDA(ctx, cudaMemsetAsync(w, 0, ws->off_blocksum, ctx->stream));
@@ -291,10 +291,10 @@ extern "C" int wpg_grid(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, co
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     int rc = bin_common(ctx, d_vis, d_uvw, d_weight, d_freq, nrow, nchan, desc, prec, d_workspace, workspace_bytes, &tab, &bp, &ws);
     if (rc) return rc;
-    if ((rc = mark(ctx, 1))) return rc;
+    if ((rc = wpg_mark(ctx, 1))) return rc;
     rc = wpg_launch_grid(ctx, tab, bp, ws, prec, d_kernels, d_grid, (char *)d_workspace);
     if (rc) return rc;
-    if ((rc = mark(ctx, 2))) return rc;
+    if ((rc = wpg_mark(ctx, 2))) return rc;
     if (h_stats) return read_stats(ctx, (const Counters *)((char *)d_workspace + ws.off_counters), h_stats, nullptr);
     return WPG_OK;
 }

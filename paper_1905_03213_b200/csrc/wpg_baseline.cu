@@ -225,6 +225,7 @@ extern "C" int wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const do
     WPG_CUDA(ctx, cudaSetDevice(ctx->device));
     char *w = (char *)d_workspace;
     cudaStream_t s = ctx->stream;
+    if ((rc = wpg_mark(ctx, 0))) return rc;
     rc = bl_reorder(ctx, d_ant1, d_ant2, n_ant, nrow, w, L);             // Eqs. (1)-(2), baseline-then-time order
     if (rc) return rc;
     const long long nvis = (long long)nrow * nchan;
@@ -242,6 +243,7 @@ extern "C" int wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const do
     }
     ctx->n_launches += nbk ? 2 : 1;
     WPG_CUDA(ctx, cudaGetLastError());
+    if ((rc = wpg_mark(ctx, 1))) return rc;
     if (nvis) {
         // the gridder of wpg_grid.cu walks the records in this order: one class, key range [0, 1) = all records
         WorkspaceLayout ws{};
@@ -250,6 +252,7 @@ extern "C" int wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const do
         rc = wpg_launch_grid(ctx, tab, bp, ws, prec, d_kernels, d_grid, w);
         if (rc) return rc;
     }
+    if ((rc = wpg_mark(ctx, 2))) return rc;
     if (h_stats) {
         Counters h;
         WPG_CUDA(ctx, cudaMemcpyAsync(&h, ctr, sizeof h, cudaMemcpyDeviceToHost, s));

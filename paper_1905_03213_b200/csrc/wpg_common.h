@@ -110,6 +110,7 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
                   PlaneTab *tab, BinParams *bp, WorkspaceLayout *ws);
 void wpg_pswf_eval(const double *nu, int64_t n, double *out);     // wpg_pswf.cu (host)
 
+int wpg_mark(wpg_ctx *ctx, int i);      // timing event i (0 start, 1 after binning / re-order, 2 after gridder) if option "timing"
 // launchers
 int wpg_launch_exclusive_scan(wpg_ctx *ctx, unsigned *hist, unsigned n, unsigned *blocksum, Counters *ctr);
 int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
