@@ -20,6 +20,8 @@ gridder    O4  G1-G7 convolutional gridding (data model
                row x channel PAPER.md:56), plain C loops in grid_oracle.c
 image      O5  dirty image = centred inverse FFT / taper
            O6  brute-force direct 3-D DFT image (pin for the whole chain)
+baseline_  Eqs. (1)-(2): baseline index from antenna IDs, count array C, exclusive
+order      prefix sum, stable baseline-then-time re-order
 =========  ==================================================================
 
 Parity pins (tests/ -m "not gpu"): P1 taper vs independent Legendre recipe and
@@ -27,5 +29,7 @@ printed values, P2 direct double sum vs zero-padded FFT route, P3 symmetries,
 P4 w=0 separability, P5 slice sums ~ 1, P6/P7 worked index/plane examples
 (tests/golden/), P8 stored kernel values (tests/golden/), P9 gridded dirty
 image vs direct 3-D DFT, P10 single-visibility footprint, P11 flux
-conservation, P12 linearity/chunking.  No function here is "parity unpinned".
+conservation, P12 linearity/chunking; Eqs. (1)-(2): worked example, bijection onto the antenna
+triangle, closed-form row starts, numpy cumsum / stable argsort
+(tests/test_oracle_baseline_order.py).  No function here is "parity unpinned".
 """
