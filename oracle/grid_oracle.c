@@ -166,6 +166,49 @@ int oracle_grid(const double *uvw, const float *vis, const float *weight, const 
     return 0;
 }
 
+/* Degridding, the adjoint of oracle_grid with unit weights (PAPER.md:36 names it as
+ * the companion operation of gridding):
+ *   vis[r][c] = sum_{iv,iu} grid[j0v+iv][j0u+iu] * conj(K[p][ov][ou][iv][iu])
+ * with plane, window and sub-cell offsets exactly as in G1-G4; a visibility whose window is not fully inside the
+ * grid is predicted as 0 (counted).  vis_out: complex128 pairs [nrow][nchan].  counts_out: {n_predicted, n_outside}. */
+int oracle_degrid(const double *uvw, const double *freq, int64_t nrow, int nchan, const double *K,
+                  const int *support, const int64_t *plane_offset, int Nw, int Q, int N, double cell,
+                  double w_max, const double *grid, double *vis_out, int64_t *counts_out) {
+    int64_t n_pred = 0, n_out = 0;
+    for (int64_t r = 0; r < nrow; ++r) {
+        for (int c = 0; c < nchan; ++c) {
+            double f = freq[c] / C0;
+            double u = uvw[3 * r + 0] * f, v = uvw[3 * r + 1] * f, w = uvw[3 * r + 2] * f;
+            int clamped;
+            int p = oracle_plane(w, w_max, Nw, &clamped);
+            int S = support[p];
+            int64_t j0u, j0v; int ou, ov;
+            oracle_index_map(u, N, cell, S, Q, &j0u, &ou);
+            oracle_index_map(v, N, cell, S, Q, &j0v, &ov);
+            double sr = 0.0, si = 0.0;
+            if (j0u < 0 || j0v < 0 || j0u + S > N || j0v + S > N) {
+                n_out++;
+            } else {
+                const double *Ks = K + 2 * (plane_offset[p] + ((int64_t)ov * Q + ou) * S * S);
+                for (int iv = 0; iv < S; ++iv) {
+                    const double *g = grid + 2 * ((j0v + iv) * (int64_t)N + j0u);
+                    const double *k = Ks + 2 * (int64_t)iv * S;
+                    for (int iu = 0; iu < S; ++iu) {
+                        double gr = g[2 * iu], gi = g[2 * iu + 1], kr = k[2 * iu], ki = k[2 * iu + 1];
+                        sr += gr * kr + gi * ki;          /* g * conj(k) */
+                        si += gi * kr - gr * ki;
+                    }
+                }
+                n_pred++;
+            }
+            vis_out[2 * (r * nchan + c)] = sr;
+            vis_out[2 * (r * nchan + c) + 1] = si;
+        }
+    }
+    counts_out[0] = n_pred; counts_out[1] = n_out;
+    return 0;
+}
+
 int oracle_max_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -41,6 +41,8 @@ def _load():
         lib.oracle_grid.argtypes = [vp, vp, vp, vp, i64, cint, vp, vp, vp, cint, cint, cint,
                                     dbl, dbl, vp, vp, cint]
         lib.oracle_grid.restype = cint
+        lib.oracle_degrid.argtypes = [vp, vp, i64, cint, vp, vp, vp, cint, cint, cint, dbl, dbl, vp, vp, vp]
+        lib.oracle_degrid.restype = cint
         lib.oracle_max_threads.restype = cint
         _lib = lib
     return _lib
@@ -92,3 +94,25 @@ def grid(uvw, vis, weight, freq, stack, grid=None, threads=1):
     if rc != 0:
         raise RuntimeError("oracle_grid failed rc=%d" % rc)
     return grid, dict(zip(STAT_NAMES, (int(x) for x in st)))
+
+
+def degrid(uvw, freq, stack, grid):
+    """Adjoint of :func:`grid` with unit weights (oracle_degrid in grid_oracle.c):
+    vis[r][c] = sum over the window of grid * conj(K slice); 0 where the window leaves the grid.
+    Returns (vis [nrow][nchan] complex128, {"n_predicted", "n_outside"})."""
+    uvw = np.ascontiguousarray(uvw, dtype=np.float64)
+    freq = np.ascontiguousarray(freq, dtype=np.float64)
+    grid = np.ascontiguousarray(grid, dtype=np.complex128)
+    nrow, nchan, N = uvw.shape[0], freq.shape[0], stack.grid_N
+    assert grid.shape == (N, N)
+    K = np.ascontiguousarray(stack.data, dtype=np.complex128)
+    sup = np.ascontiguousarray(stack.support, dtype=np.int32)
+    off = np.ascontiguousarray(stack.plane_offset, dtype=np.int64)
+    out = np.zeros((nrow, nchan), dtype=np.complex128)
+    cnt = np.zeros(2, dtype=np.int64)
+    rc = _load().oracle_degrid(uvw.ctypes.data, freq.ctypes.data, nrow, nchan, K.ctypes.data, sup.ctypes.data,
+                               off.ctypes.data, stack.Nw, stack.oversample, N, stack.cell, stack.w_max,
+                               grid.ctypes.data, out.ctypes.data, cnt.ctypes.data)
+    if rc != 0:
+        raise RuntimeError("oracle_degrid failed rc=%d" % rc)
+    return out, {"n_predicted": int(cnt[0]), "n_outside": int(cnt[1])}
