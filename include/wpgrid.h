@@ -170,6 +170,18 @@ int  wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const double *d_uv
                              wpg_prec prec, void *d_grid, void *d_workspace, size_t workspace_bytes,
                              wpg_stats *h_stats_or_null);
 
+/* ---- degridding: the adjoint of wpg_grid with unit weights ---------------
+ *   vis_out[r][c] = sum over the S x S window of grid[j0v+iv][j0u+iu] * conj(K[p][ov][ou][iv][iu]),
+ * plane, window and sub-cell offsets exactly as in wpg_grid (G1-G4); a visibility whose window is not fully inside
+ * the grid is predicted as 0.  With grid = centred FFT of (model image / taper) this predicts the visibilities of
+ * the model (measurement model O1).
+ *   d_grid  c64 | c128 [N][N] (not modified)      d_vis_out  c64 | c128 [nrow][nchan] (overwritten)
+ *   h_counts2_or_null: {predicted, outside}; if non-NULL the call synchronises. */
+size_t wpg_degrid_workspace_bytes(int nchan);
+int  wpg_degrid(wpg_ctx *ctx, const void *d_grid, const double *d_uvw, const double *d_freq, int64_t nrow, int nchan,
+                const void *d_kernels, const wpg_kdesc *desc, wpg_prec prec, void *d_vis_out,
+                void *d_workspace, size_t workspace_bytes, int64_t *h_counts2_or_null);
+
 /* Machine-limit microbenchmarks (instrumentation; SURVEY.md §8(d) wants fractions of MEASURED peaks).
  * which: 0 = red.global.add.v2.f32, a warp per 256-byte row segment at a pseudo-random place of the buffer (the
  *            naive gridder's pattern; "write access ... in an atomic manner");

@@ -1,0 +1,127 @@
+// Degridding (PAPER.md:36 names it as gridding's companion): the adjoint of the gridder
+// with unit weights, vis[r][c] = sum over the S x S window of grid * conj(K[p][ov][ou]) — a gather, no atomics.
+// A warp takes 32 visibilities: every lane does the fp64 position math (G1-G4, identical to the binning) of one of
+// them, then the warp walks the 32 windows together, lane <-> window cell, and sums across lanes.
+#include "wpg_common.h"
+
+namespace {
+
+template <typename T> struct Cx;
+template <> struct Cx<float> { using type = float2; };
+template <> struct Cx<double> { using type = double2; };
+
+template <typename T>
+__device__ __forceinline__ T warp_sum(T v) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
+__global__ void dg_chan_scale_kernel(const double *__restrict__ freq, int nchan, double *__restrict__ fscale) {
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < nchan) fscale[c] = __ddiv_rn(freq[c], WPG_C0);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+degrid_kernel(const typename Cx<T>::type *__restrict__ grid, const double *__restrict__ uvw,
+              const double *__restrict__ fscale, const __grid_constant__ PlaneTab Tb, const __grid_constant__ BinParams P,
+              const typename Cx<T>::type *__restrict__ K, typename Cx<T>::type *__restrict__ vis_out,
+              unsigned long long *__restrict__ counts) {
+    using C = typename Cx<T>::type;
+    __shared__ uint2 s_tab[WPG_MAX_NW];
+    wpg_stage_planetab(s_tab, Tb, P.Nw);
+    __syncthreads();
+    const SmemPlaneTab ST{s_tab, nullptr};
+    const long long nvis = P.nrow * P.nchan;
+    const int lane = threadIdx.x & 31;
+    const long long nwarp = ((long long)gridDim.x * 256) >> 5;
+    unsigned n_pred = 0, n_out = 0;
+    for (long long base = (((long long)blockIdx.x * 256 + threadIdx.x) >> 5) * 32; base < nvis; base += nwarp * 32) {
+        // one visibility per lane: window start, coefficient slice, support
+        const long long i = base + lane;
+        unsigned pos = 0, koff = 0; int S = 0;
+        if (i < nvis) {
+            long long row = i; int ch = 0;
+            if (P.nchan > 1) { const unsigned r32 = (unsigned)i / (unsigned)P.nchan; row = r32; ch = (int)((unsigned)i - r32 * (unsigned)P.nchan); }
+            const VisPos r = wpg_locate(__ldg(uvw + 3 * row), __ldg(uvw + 3 * row + 1), __ldg(uvw + 3 * row + 2),
+                                        __ldg(fscale + ch), P, ST);
+            if (r.inside) { S = r.S; pos = (unsigned)r.j0u | ((unsigned)r.j0v << 16); koff = wpg_koff(r, P, ST); n_pred++; }
+            else n_out++;
+        }
+        C mine; mine.x = mine.y = (T)0;
+        const int cnt = (int)min((long long)32, nvis - base);
+        for (int j = 0; j < cnt; ++j) {
+            const int Sj = __shfl_sync(0xffffffffu, S, j);
+            if (Sj == 0) continue;                                  // outside the grid: predicted as 0
+            const unsigned pj = __shfl_sync(0xffffffffu, pos, j), kj = __shfl_sync(0xffffffffu, koff, j);
+            const C *g0 = grid + (size_t)(pj >> 16) * P.N + (pj & 0xFFFFu);
+            const C *k0 = K + kj;
+            T sr = (T)0, si = (T)0;
+            int iv = lane / Sj, iu = lane - iv * Sj;
+            const int dv = 32 / Sj, du_ = 32 - dv * Sj;
+            for (int c = lane; c < Sj * Sj; c += 32) {
+                const C g = __ldg(g0 + (size_t)iv * P.N + iu), k = __ldg(k0 + c);
+                sr = fma(g.x, k.x, sr); sr = fma(g.y, k.y, sr);    // g * conj(k)
+                si = fma(g.y, k.x, si); si = fma(-g.x, k.y, si);
+                iu += du_; iv += dv;
+                if (iu >= Sj) { iu -= Sj; iv += 1; }
+            }
+            sr = warp_sum(sr); si = warp_sum(si);
+            if (lane == j) { mine.x = sr; mine.y = si; }
+        }
+        if (i < nvis) vis_out[i] = mine;                            // one coalesced store of the 32 results
+    }
+    n_pred = __reduce_add_sync(0xffffffffu, n_pred); n_out = __reduce_add_sync(0xffffffffu, n_out);
+    if (lane == 0) {
+        if (n_pred) atomicAdd(&counts[2 * (blockIdx.x % kStatSlots)], (unsigned long long)n_pred);
+        if (n_out) atomicAdd(&counts[2 * (blockIdx.x % kStatSlots) + 1], (unsigned long long)n_out);
+    }
+}
+
+}  // namespace
+
+extern "C" size_t wpg_degrid_workspace_bytes(int nchan) {
+    return nchan < 1 ? 0 : (size_t)((nchan * 8 + 255) & ~255) + 256;
+}
+
+extern "C" int wpg_degrid(wpg_ctx *ctx, const void *d_grid, const double *d_uvw, const double *d_freq, int64_t nrow,
+                          int nchan, const void *d_kernels, const wpg_kdesc *desc, wpg_prec prec, void *d_vis_out,
+                          void *d_workspace, size_t workspace_bytes, int64_t *h_counts2) {
+    if (!ctx) return WPG_EINVAL;
+    if (!d_grid || !d_kernels || !d_freq || (nrow > 0 && (!d_uvw || !d_vis_out)))
+        return wpg_fail(ctx, WPG_EINVAL, "NULL pointer argument");
+    PlaneTab tab; BinParams bp; WorkspaceLayout ws0;
+    int rc = wpg_make_plan(ctx, desc, nrow, nchan, prec, &tab, &bp, &ws0);
+    if (rc) return rc;
+    const size_t need = wpg_degrid_workspace_bytes(nchan);
+    if (!d_workspace || workspace_bytes < need)
+        return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, need);
+    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t s = ctx->stream;
+    char *w = (char *)d_workspace;
+    unsigned long long *counts = (unsigned long long *)w;             // kStatSlots x {predicted, outside}
+    double *fscale = (double *)(w + 256);
+    WPG_CUDA(ctx, cudaMemsetAsync(counts, 0, 256, s));
+    dg_chan_scale_kernel<<<(nchan + 255) / 256, 256, 0, s>>>(d_freq, nchan, fscale);
+    const long long nvis = (long long)nrow * nchan;
+    if (nvis) {
+        const int blocks = (int)min((long long)ctx->sm_count * 8, (nvis + 255) / 256);
+        if (prec == WPG_F32)
+            degrid_kernel<float><<<blocks, 256, 0, s>>>((const float2 *)d_grid, d_uvw, fscale, tab, bp, (const float2 *)d_kernels,
+                                                        (float2 *)d_vis_out, counts);
+        else
+            degrid_kernel<double><<<blocks, 256, 0, s>>>((const double2 *)d_grid, d_uvw, fscale, tab, bp, (const double2 *)d_kernels,
+                                                         (double2 *)d_vis_out, counts);
+    }
+    ctx->n_launches += nvis ? 2 : 1;
+    WPG_CUDA(ctx, cudaGetLastError());
+    if (h_counts2) {
+        unsigned long long h[2 * kStatSlots];
+        WPG_CUDA(ctx, cudaMemcpyAsync(h, counts, sizeof h, cudaMemcpyDeviceToHost, s));
+        WPG_CUDA(ctx, cudaStreamSynchronize(s));
+        h_counts2[0] = h_counts2[1] = 0;
+        for (int k = 0; k < kStatSlots; ++k) { h_counts2[0] += (int64_t)h[2 * k]; h_counts2[1] += (int64_t)h[2 * k + 1]; }
+    }
+    return WPG_OK;
+}

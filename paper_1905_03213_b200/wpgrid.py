@@ -22,6 +22,7 @@ EXPORTS = (
     "wpg_grid", "wpg_grid_naive", "wpg_grid_host", "wpg_bin", "wpg_dirty_image_workspace_bytes",
     "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms", "wpg_microbench",
     "wpg_baseline_workspace_bytes", "wpg_baseline_reorder", "wpg_grid_baseline_order",
+    "wpg_degrid_workspace_bytes", "wpg_degrid",
 )
 
 
@@ -95,6 +96,9 @@ def load():
     lib.wpg_baseline_reorder.argtypes = [vp, vp, vp, cint, i64, vp, vp, vp, sz]; lib.wpg_baseline_reorder.restype = cint
     lib.wpg_grid_baseline_order.argtypes = [vp, vp, vp, vp, vp, vp, vp, cint, i64, cint, vp, kd, cint, vp, vp, sz, stp]
     lib.wpg_grid_baseline_order.restype = cint
+    lib.wpg_degrid_workspace_bytes.argtypes = [cint]; lib.wpg_degrid_workspace_bytes.restype = sz
+    lib.wpg_degrid.argtypes = [vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, vp, sz, ctypes.POINTER(i64)]
+    lib.wpg_degrid.restype = cint
     lib.wpg_microbench.argtypes = [vp, cint, cint, vp, sz, ctypes.POINTER(dbl)]; lib.wpg_microbench.restype = cint
     _lib = lib
     return lib
@@ -313,6 +317,24 @@ class Context:
             n_ant, nrow, nchan, stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec, grid.data_ptr(),
             workspace.data_ptr(), workspace.numel(), ctypes.byref(st) if stats else None))
         return grid, (st.as_dict() if stats else None)
+
+    # ---- degridding (adjoint of grid with unit weights)
+    def degrid(self, grid, uvw, freq, stack, out=None, counts=False):
+        """vis[r][c] = sum over the window of grid * conj(kernel slice).  Returns (vis, counts dict or None)."""
+        t = self.torch
+        N = stack.desc.grid_N
+        cdt = t.complex64 if stack.prec == F32 else t.complex128
+        assert grid.is_cuda and grid.is_contiguous() and grid.shape == (N, N) and grid.dtype == cdt
+        assert uvw.dtype == t.float64 and freq.dtype == t.float64 and uvw.is_cuda and freq.is_cuda
+        nrow, nchan = uvw.shape[0], freq.shape[0]
+        if out is None:
+            out = t.empty((nrow, nchan), dtype=cdt, device=self.device)
+        ws = t.empty(int(self.lib.wpg_degrid_workspace_bytes(nchan)), dtype=t.uint8, device=self.device)
+        c2 = (ctypes.c_int64 * 2)()
+        self._check(self.lib.wpg_degrid(self.h, grid.data_ptr(), uvw.data_ptr(), freq.data_ptr(), nrow, nchan,
+                                        stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec, out.data_ptr(),
+                                        ws.data_ptr(), ws.numel(), c2 if counts else None))
+        return out, ({"n_predicted": int(c2[0]), "n_outside": int(c2[1])} if counts else None)
 
     def bin(self, vis, uvw, weight, freq, stack, workspace=None):
         """Step a1 alone.  Returns (workspace tensor, BinInfo dict, stats dict)."""
