@@ -52,6 +52,8 @@ def parse_args():
     ap.add_argument("--order", default="position", choices=["position", "baseline"],
                     help="position: wpg_grid (sort by window start); baseline: the paper's Eq. (1)-(2) order, "
                          "wpg_grid_baseline_order (track-based workloads, uniform stacks)")
+    ap.add_argument("--op", default="grid", choices=["grid", "degrid"],
+                    help="grid: the headline step; degrid: wpg_degrid of a random grid for all visibilities (a4+ extra)")
     ap.add_argument("--no-row-block", action="store_true",
                     help="do not pass the rows-per-time-step hint of track-based workloads to the library")
     return ap.parse_args()
@@ -277,6 +279,8 @@ def run_b200(args):
     ws = torch.empty(ctx.grid_workspace_bytes(nrow, nchan, stack), dtype=torch.uint8, device=dev)
     iws = torch.empty(int(ctx.lib.wpg_dirty_image_workspace_bytes(wl.grid_N, prec)), dtype=torch.uint8, device=dev)
 
+    if args.op == "degrid":
+        return run_degrid(args, ctx, wl, stack, d_uvw, d_freq, prec, dev, world, rank, dist)
     if args.order == "baseline":
         n_ant = int(wl.notes["n_ant"])
         a1, a2 = synth.track_antennas(n_ant, nrow)
@@ -396,6 +400,35 @@ def run_b200(args):
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(wl)
     print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def run_degrid(args, ctx, wl, stack, d_uvw, d_freq, prec, dev, world, rank, dist):
+    """Degridding throughput (not the headline metric): K timed wpg_degrid calls of one random grid."""
+    import torch
+    from paper_1905_03213_b200 import wpgrid
+    N = wl.grid_N
+    gen = torch.Generator(device=dev).manual_seed(1)
+    g = torch.randn((N, N), dtype=torch.complex64 if prec == wpgrid.F32 else torch.complex128, device=dev, generator=gen)
+    out, cnt = ctx.degrid(g, d_uvw, d_freq, stack, counts=True)
+    sup = stack.support.astype(np.int64)
+    # updates = sum S_p^2 over predicted visibilities: exact for uniform stacks
+    n_updates = cnt["n_predicted"] * int(sup[0]) ** 2 if stack.uniform else None
+    for _ in range(max(args.warmup, 3)):
+        ctx.degrid(g, d_uvw, d_freq, stack, out=out)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ctx.degrid(g, d_uvw, d_freq, stack, out=out)
+    e1.record(); torch.cuda.synchronize()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, dev) / args.steps
+    if rank == 0:
+        print(json.dumps({"metric": "grid-point updates/sec (degridding, vis x support^2)", "unit": UNIT,
+                          "value": None if n_updates is None else aggregate_value(n_updates, world, ms),
+                          "ms_per_step": ms, "n_gpus": world, "steps": args.steps, "dtype": args.prec, "data": "synthetic",
+                          "config": workload_config(wl, args.prec), "counts": cnt, "op": "degrid"}))
     if dist is not None:
         dist.destroy_process_group()
 

@@ -17,7 +17,8 @@ wkernel    O3  K1-K6 oversampled W-kernel stack, direct-DFT form
                (PAPER.md:30 "new convolution kernel function"; PAPER.md:108
                "number of w-projection planes is 23, full support size 9")
 gridder    O4  G1-G7 convolutional gridding (data model
-               row x channel PAPER.md:56), plain C loops in grid_oracle.c
+               row x channel PAPER.md:56), plain C loops in grid_oracle.c;
+               degrid(): its adjoint with unit weights
 image      O5  dirty image = centred inverse FFT / taper
            O6  brute-force direct 3-D DFT image (pin for the whole chain)
 baseline_  Eqs. (1)-(2): baseline index from antenna IDs, count array C, exclusive
@@ -31,5 +32,6 @@ P4 w=0 separability, P5 slice sums ~ 1, P6/P7 worked index/plane examples
 image vs direct 3-D DFT, P10 single-visibility footprint, P11 flux
 conservation, P12 linearity/chunking; Eqs. (1)-(2): worked example, bijection onto the antenna
 triangle, closed-form row starts, numpy cumsum / stable argsort
-(tests/test_oracle_baseline_order.py).  No function here is "parity unpinned".
+(tests/test_oracle_baseline_order.py); degridder: adjoint identity, single-cell
+grids, prediction of the measurement model (tests/test_oracle_degrid.py).  No function here is "parity unpinned".
 """

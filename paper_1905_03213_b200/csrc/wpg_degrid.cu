@@ -22,7 +22,8 @@ __global__ void dg_chan_scale_kernel(const double *__restrict__ freq, int nchan,
     if (c < nchan) fscale[c] = __ddiv_rn(freq[c], WPG_C0);
 }
 
-template <typename T>
+// SCT: compile-time support of a uniform stack (lane -> cell arithmetic folds to shifts and masks), 0 = per-visibility S
+template <typename T, int SCT>
 __global__ void __launch_bounds__(256)
 degrid_kernel(const typename Cx<T>::type *__restrict__ grid, const double *__restrict__ uvw,
               const double *__restrict__ fscale, const __grid_constant__ PlaneTab Tb, const __grid_constant__ BinParams P,
@@ -52,8 +53,9 @@ degrid_kernel(const typename Cx<T>::type *__restrict__ grid, const double *__res
         C mine; mine.x = mine.y = (T)0;
         const int cnt = (int)min((long long)32, nvis - base);
         for (int j = 0; j < cnt; ++j) {
-            const int Sj = __shfl_sync(0xffffffffu, S, j);
-            if (Sj == 0) continue;                                  // outside the grid: predicted as 0
+            const int Sq = __shfl_sync(0xffffffffu, S, j);
+            if (Sq == 0) continue;
+            const int Sj = SCT ? SCT : Sq;                                  // outside the grid: predicted as 0
             const unsigned pj = __shfl_sync(0xffffffffu, pos, j), kj = __shfl_sync(0xffffffffu, koff, j);
             const C *g0 = grid + (size_t)(pj >> 16) * P.N + (pj & 0xFFFFu);
             const C *k0 = K + kj;
@@ -107,12 +109,11 @@ extern "C" int wpg_degrid(wpg_ctx *ctx, const void *d_grid, const double *d_uvw,
     const long long nvis = (long long)nrow * nchan;
     if (nvis) {
         const int blocks = (int)min((long long)ctx->sm_count * 8, (nvis + 255) / 256);
-        if (prec == WPG_F32)
-            degrid_kernel<float><<<blocks, 256, 0, s>>>((const float2 *)d_grid, d_uvw, fscale, tab, bp, (const float2 *)d_kernels,
-                                                        (float2 *)d_vis_out, counts);
-        else
-            degrid_kernel<double><<<blocks, 256, 0, s>>>((const double2 *)d_grid, d_uvw, fscale, tab, bp, (const double2 *)d_kernels,
-                                                         (double2 *)d_vis_out, counts);
+        const int S1 = bp.ncls == 1 ? tab.clsS[0] : 0;
+#define WPG_DG(TT, CC, SS) degrid_kernel<TT, SS><<<blocks, 256, 0, s>>>((const CC *)d_grid, d_uvw, fscale, tab, bp, (const CC *)d_kernels, (CC *)d_vis_out, counts)
+        if (prec == WPG_F32) { if (S1 == 8) WPG_DG(float, float2, 8); else if (S1 == 16) WPG_DG(float, float2, 16); else if (S1 == 4) WPG_DG(float, float2, 4); else WPG_DG(float, float2, 0); }
+        else { if (S1 == 8) WPG_DG(double, double2, 8); else if (S1 == 16) WPG_DG(double, double2, 16); else if (S1 == 4) WPG_DG(double, double2, 4); else WPG_DG(double, double2, 0); }
+#undef WPG_DG
     }
     ctx->n_launches += nvis ? 2 : 1;
     WPG_CUDA(ctx, cudaGetLastError());
