@@ -22,20 +22,25 @@ __global__ void dg_chan_scale_kernel(const double *__restrict__ freq, int nchan,
     if (c < nchan) fscale[c] = __ddiv_rn(freq[c], WPG_C0);
 }
 
-// SCT: compile-time support of a uniform stack (lane -> cell arithmetic folds to shifts and masks), 0 = per-visibility S
-template <typename T, int SCT>
+// SCT: compile-time support of a uniform stack (lane -> cell arithmetic folds to shifts and masks), 0 = per-visibility
+// S.  LPV lanes work on one visibility, 32 / LPV visibilities side by side in the warp (S = 8: two half-warps, four
+// cells per lane, a 4-step sum): the loads stay coalesced (a group covers whole window rows), the cross-lane sum
+// and the per-visibility broadcasts are shared.
+template <typename T, int SCT, int LPV>
 __global__ void __launch_bounds__(256)
 degrid_kernel(const typename Cx<T>::type *__restrict__ grid, const double *__restrict__ uvw,
               const double *__restrict__ fscale, const __grid_constant__ PlaneTab Tb, const __grid_constant__ BinParams P,
               const typename Cx<T>::type *__restrict__ K, typename Cx<T>::type *__restrict__ vis_out,
               unsigned long long *__restrict__ counts) {
     using C = typename Cx<T>::type;
+    constexpr int VPW = 32 / LPV;
     __shared__ uint2 s_tab[WPG_MAX_NW];
     wpg_stage_planetab(s_tab, Tb, P.Nw);
     __syncthreads();
     const SmemPlaneTab ST{s_tab, nullptr};
     const long long nvis = P.nrow * P.nchan;
     const int lane = threadIdx.x & 31;
+    const int gl = lane % LPV, sub = lane / LPV;                    // lane inside its group, group = visibility slot
     const long long nwarp = ((long long)gridDim.x * 256) >> 5;
     unsigned n_pred = 0, n_out = 0;
     for (long long base = (((long long)blockIdx.x * 256 + threadIdx.x) >> 5) * 32; base < nvis; base += nwarp * 32) {
@@ -52,25 +57,33 @@ degrid_kernel(const typename Cx<T>::type *__restrict__ grid, const double *__res
         }
         C mine; mine.x = mine.y = (T)0;
         const int cnt = (int)min((long long)32, nvis - base);
-        for (int j = 0; j < cnt; ++j) {
+        for (int it = 0; it * VPW < cnt; ++it) {
+            const int j = it * VPW + sub;                           // the visibility this lane's group works on (S = 0 past the end)
             const int Sq = __shfl_sync(0xffffffffu, S, j);
-            if (Sq == 0) continue;
-            const int Sj = SCT ? SCT : Sq;                                  // outside the grid: predicted as 0
             const unsigned pj = __shfl_sync(0xffffffffu, pos, j), kj = __shfl_sync(0xffffffffu, koff, j);
-            const C *g0 = grid + (size_t)(pj >> 16) * P.N + (pj & 0xFFFFu);
-            const C *k0 = K + kj;
             T sr = (T)0, si = (T)0;
-            int iv = lane / Sj, iu = lane - iv * Sj;
-            const int dv = 32 / Sj, du_ = 32 - dv * Sj;
-            for (int c = lane; c < Sj * Sj; c += 32) {
-                const C g = __ldg(g0 + (size_t)iv * P.N + iu), k = __ldg(k0 + c);
-                sr = fma(g.x, k.x, sr); sr = fma(g.y, k.y, sr);    // g * conj(k)
-                si = fma(g.y, k.x, si); si = fma(-g.x, k.y, si);
-                iu += du_; iv += dv;
-                if (iu >= Sj) { iu -= Sj; iv += 1; }
+            if (Sq) {                                               // 0: outside the grid, predicted as 0
+                const int Sj = SCT ? SCT : Sq;
+                const C *g0 = grid + (size_t)(pj >> 16) * P.N + (pj & 0xFFFFu);
+                const C *k0 = K + kj;
+                int iv = gl / Sj, iu = gl - iv * Sj;
+                const int dv = LPV / Sj, du_ = LPV - dv * Sj;
+                for (int c = gl; c < Sj * Sj; c += LPV) {
+                    const C g = __ldg(g0 + (size_t)iv * P.N + iu), k = __ldg(k0 + c);
+                    sr = fma(g.x, k.x, sr); sr = fma(g.y, k.y, sr);    // g * conj(k)
+                    si = fma(g.y, k.x, si); si = fma(-g.x, k.y, si);
+                    iu += du_; iv += dv;
+                    if (iu >= Sj) { iu -= Sj; iv += 1; }
+                }
             }
-            sr = warp_sum(sr); si = warp_sum(si);
-            if (lane == j) { mine.x = sr; mine.y = si; }
+#pragma unroll
+            for (int d = LPV / 2; d > 0; d >>= 1) {
+                sr += __shfl_xor_sync(0xffffffffu, sr, d);
+                si += __shfl_xor_sync(0xffffffffu, si, d);
+            }
+            // visibility L of the batch was summed in trip L / VPW by group L % VPW (every lane of the group has the sum)
+            const T vr = __shfl_sync(0xffffffffu, sr, (lane % VPW) * LPV), vi = __shfl_sync(0xffffffffu, si, (lane % VPW) * LPV);
+            if (lane / VPW == it) { mine.x = vr; mine.y = vi; }
         }
         if (i < nvis) vis_out[i] = mine;                            // one coalesced store of the 32 results
     }
@@ -110,9 +123,9 @@ extern "C" int wpg_degrid(wpg_ctx *ctx, const void *d_grid, const double *d_uvw,
     if (nvis) {
         const int blocks = (int)min((long long)ctx->sm_count * 8, (nvis + 255) / 256);
         const int S1 = bp.ncls == 1 ? tab.clsS[0] : 0;
-#define WPG_DG(TT, CC, SS) degrid_kernel<TT, SS><<<blocks, 256, 0, s>>>((const CC *)d_grid, d_uvw, fscale, tab, bp, (const CC *)d_kernels, (CC *)d_vis_out, counts)
-        if (prec == WPG_F32) { if (S1 == 8) WPG_DG(float, float2, 8); else if (S1 == 16) WPG_DG(float, float2, 16); else if (S1 == 4) WPG_DG(float, float2, 4); else WPG_DG(float, float2, 0); }
-        else { if (S1 == 8) WPG_DG(double, double2, 8); else if (S1 == 16) WPG_DG(double, double2, 16); else if (S1 == 4) WPG_DG(double, double2, 4); else WPG_DG(double, double2, 0); }
+#define WPG_DG(TT, CC, SS, LL) degrid_kernel<TT, SS, LL><<<blocks, 256, 0, s>>>((const CC *)d_grid, d_uvw, fscale, tab, bp, (const CC *)d_kernels, (CC *)d_vis_out, counts)
+        if (prec == WPG_F32) { if (S1 == 8) WPG_DG(float, float2, 8, 16); else if (S1 == 16) WPG_DG(float, float2, 16, 32); else if (S1 == 4) WPG_DG(float, float2, 4, 8); else WPG_DG(float, float2, 0, 32); }
+        else { if (S1 == 8) WPG_DG(double, double2, 8, 16); else if (S1 == 16) WPG_DG(double, double2, 16, 32); else if (S1 == 4) WPG_DG(double, double2, 4, 8); else WPG_DG(double, double2, 0, 32); }
 #undef WPG_DG
     }
     ctx->n_launches += nvis ? 2 : 1;
