@@ -377,7 +377,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         for (unsigned c = 0; c < 2; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
 
         U64 acc0[NSLOT], acc1[NSLOT];                       // (re, im) sums of the pair's two cells
-        unsigned qcur[NSLOT];                               // (column | row << 16) of the pair's first cell
+        unsigned qcur[NSLOT] = {};                          // (column | row << 16) of the pair's first cell
 #pragma unroll
         for (int k = 0; k < NSLOT; ++k) { acc0[k] = acc1[k] = 0ull; qcur[k] = 0xFFFFFFFFu; }
 
@@ -579,7 +579,7 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
         for (unsigned c = 0; c < 2; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
 
         double accx[NSLOT], accy[NSLOT];
-        unsigned qcur[NSLOT];
+        unsigned qcur[NSLOT] = {};
 #pragma unroll
         for (int k = 0; k < NSLOT; ++k) { accx[k] = accy[k] = 0.0; qcur[k] = 0xFFFFFFFFu; }
         double2 cf[DEPTH][NSLOT];
