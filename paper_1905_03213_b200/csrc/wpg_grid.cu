@@ -297,9 +297,10 @@ __device__ __forceinline__ void ldg128(const float2 *p, unsigned long long &c0, 
     asm volatile("ld.global.nc.v2.b64 {%0, %1}, [%2];" : "=l"(c0), "=l"(c1) : "l"(p));
 }
 
-// G > 1 (small supports: S*S/2 <= 32/G pairs, NSLOT = 1): the warp is split into G groups of 32/G lanes and
-// every group takes its own record, G records per step (record t*G + g goes to group g), so that a 4x4
-// support does not leave three quarters of the warp idle.
+// G > 1: the warp is split into G groups of 32/G lanes and every group takes its own record, G records per step
+// (record t*G + g goes to group g); a group's NSLOT * 32/G lane-slots hold the S*S/2 pairs of its window.  For
+// S = 4 (8 pairs) this fills the warp; for S = 8 (two half-warps, two pairs per lane) it halves the per-record
+// share of everything that is not a coefficient load or an FMA — record fetch, window test, loop control.
 // RPS > 0: a slot holds RPS whole window rows (RPS * S/2 <= 32 lanes, the rest idle) instead of 32 consecutive
 // pairs: for S = 12 four rows are 384 bytes = three whole 128-byte lines of the slice, where 32 consecutive pairs
 // (5 1/3 rows) straddle five, and the coefficient loads are bound by the lines they touch.
@@ -312,7 +313,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
                   const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
                   const float2 *__restrict__ K, float2 *__restrict__ grid, int N, unsigned seg) {
     static_assert(kChunk % (DEPTH * G) == 0, "a look-ahead step divides the chunk");
-    static_assert(G == 1 || NSLOT == 1, "lane groups only for one-slot supports");
+    static_assert(G == 1 || RPS == 0, "lane groups use the packed pair -> lane-slot mapping");
     static_assert(!ST || G == 1, "window tracking in the producer needs one window per warp");
     constexpr int LPG = 32 / G;                          // lanes per group
     using U64 = unsigned long long;
@@ -337,7 +338,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     bool act[NSLOT];
 #pragma unroll
     for (int k = 0; k < NSLOT; ++k) {
-        int r = k * 32 + (G > 1 ? lane % LPG : lane);
+        int r = k * LPG + lane % LPG;                    // (G = 1: k * 32 + lane)
         act[k] = r < NP;
         if (RPS) {                                       // RPS rows per slot
             const int row = k * RPS + lane / H;
@@ -702,7 +703,7 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     if (F && S % 2 == 0 && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp32, even support: the pair gridder (S*S/2 pairs over 32 lanes)
         const int np = S * S / 2, nslot = (np + 31) / 32;
-        if (S == 8) return launch_pairs<8, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 8) return launch_pairs<8, 2, 4, 3, 2>(ctx, bp, ws, K, grid, w, cls, S);        // two half-warps, two pairs per lane
         if (S == 16) return launch_pairs<16, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
         if (S == 4) return launch_pairs<4, 1, 4, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);        // 8 pairs: 4 records per step
         if (S == 12) return launch_pairs<12, 3, 2, 3, 1, 4, true>(ctx, bp, ws, K, grid, w, cls, S);     // 4 rows per slot
