@@ -385,3 +385,51 @@ def test_row_block_hint_changes_nothing_but_speed(ctx):
         ctx.set_option("row_block", rb)
         check_all_paths(ctx, wl2, st, ref, rstats)
     ctx.set_option("row_block", 0)
+
+
+def test_binning_exactness_on_ties_and_near_ties(ctx):
+    """Exactness rule G6 under the constant-divisor fast path: visibilities whose oversampled coordinate
+    x*Q + 1/2 lands exactly on an integer (rounding ties), one ulp to either side, and whose w sits on plane
+    boundaries, for cell sizes whose reciprocal is not a power of two.  Every record (window start, coefficient
+    slice) must equal the oracle's integer decisions bit for bit."""
+    rng = np.random.default_rng(99)
+    for N, fov, S, Q, Nw, w_max in ((256, 0.1, 8, 8, 16, 77.7), (1000, 0.0731, 7, 8, 9, 310.0), (512, 0.0509, 12, 4, 5, 55.5)):
+        cell = fov / N
+        du = 1.0 / fov
+        n = 6000
+        # coordinates in cells at multiples of 1/(2Q) (ties of the nearest-oversample-point rule) -> wavelengths,
+        # then nudged by 0, +-1, +-2 ulps
+        k = rng.integers(-int(0.4 * N) * 2 * Q, int(0.4 * N) * 2 * Q, size=(n, 2))
+        uv = (k / (2.0 * Q)) * du
+        nudge = rng.integers(-2, 3, size=(n, 2))
+        for _ in range(2):
+            uv = np.where(nudge > 0, np.nextafter(uv, np.inf), np.where(nudge < 0, np.nextafter(uv, -np.inf), uv))
+            nudge = nudge - np.sign(nudge)
+        dw = 2.0 * w_max / Nw
+        w = -w_max + dw * rng.integers(0, Nw + 1, n)                  # plane boundaries
+        wn = rng.integers(-1, 2, n)
+        w = np.where(wn > 0, np.nextafter(w, np.inf), np.where(wn < 0, np.nextafter(w, -np.inf), w))
+        uvw = np.ascontiguousarray(np.stack([uv[:, 0], uv[:, 1], w], 1))
+        vis = (np.arange(n) + 1j).astype(np.complex64)[:, None]
+        wt = np.ones((n, 1), np.float32)
+        freq = np.array([synth.C0])
+        st = owk.build_stack(Nw, w_max, S, Q, N, cell)
+        ks = upload(ctx, st, wpgrid.F32)
+        exp = []
+        for i in range(n):
+            j0u, ou = ogrid.index_map(uvw[i, 0], N, cell, S, Q)
+            j0v, ov = ogrid.index_map(uvw[i, 1], N, cell, S, Q)
+            p, _ = ogrid.plane_of(uvw[i, 2], w_max, Nw)
+            if j0u < 0 or j0v < 0 or j0u + S > N or j0v + S > N:
+                continue
+            exp.append((j0u | (j0v << 16), (p * Q * Q + ov * Q + ou) * S * S, i))
+        d = (torch.from_numpy(vis).cuda(), torch.from_numpy(uvw).cuda(), torch.from_numpy(wt).cuda(), torch.from_numpy(freq).cuda())
+        for rb in (0, 7):
+            ctx.set_option("row_block", rb)
+            ws, info, stats = ctx.bin(*d, ks)
+            assert info["n_records"] == len(exp)
+            raw = ws.cpu().numpy()
+            rec = raw[info["off_records"]:info["off_records"] + 16 * len(exp)].view(np.uint32).reshape(-1, 4)
+            got = sorted((int(r[2]), int(r[3]), int(round(float(np.array([r[0]], np.uint32).view(np.float32)[0])))) for r in rec)
+            assert got == sorted(exp)
+        ctx.set_option("row_block", 0)
