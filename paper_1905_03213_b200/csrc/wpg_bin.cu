@@ -373,6 +373,56 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
     }
 }
 
+// Pass 3 for NPOL correlations per (row, channel): vis[row][chan][pol]; one record carries all of them.
+template <int NPOL>
+__global__ void __launch_bounds__(256, 3)
+scatter_pol_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, const float *__restrict__ weight,
+                   const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
+                   const __grid_constant__ BinParams P, const Counters *__restrict__ ctr, unsigned *__restrict__ cursor,
+                   RecP<NPOL> *__restrict__ rec) {
+    const long long nvis = P.nrow * P.nchan;
+    unsigned idx[kVpt];
+    vis_indices(P, idx);
+    Located L[kVpt];
+    float wt[kVpt];
+    unsigned dst[kVpt];
+    __shared__ uint2 s_tab[WPG_MAX_NW];
+    __shared__ uint4 s_ck[WPG_MAX_CLS];
+    const SmemPlaneTab ST{s_tab, s_ck};
+    {
+        RawVis raw[kVpt];
+#pragma unroll
+        for (int j = 0; j < kVpt; ++j) raw[j] = load_vis(idx[j], nvis, uvw, weight, fscale, P);
+#pragma unroll
+        for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
+        wpg_stage_planetab(s_tab, T, P.Nw);
+        wpg_stage_classkeys(s_ck, ctr, P);
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < kVpt; ++j) { L[j] = locate_vis(raw[j], ST, P); wt[j] = raw[j].wt; }
+    }
+    unsigned key[kVpt], len[kVpt];
+    bool head[kVpt];
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) key[j] = L[j].key;
+    key_runs(key, head, len);
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) dst[j] = head[j] ? atomicAdd(cursor + key[j], len[j]) : 0u;
+#pragma unroll
+    for (int j = 1; j < kVpt; ++j)
+        if (key[j] != WPG_NO_KEY && !head[j]) dst[j] = dst[j - 1] + 1u;
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) {
+        if (key[j] == WPG_NO_KEY) continue;
+        const float2 *src = vis + (size_t)idx[j] * NPOL;
+        RecP<NPOL> out;
+#pragma unroll
+        for (int p = 0; p < NPOL; ++p) { const float2 v = __ldg(src + p); out.v[p] = make_float2(wt[j] * v.x, wt[j] * v.y); }
+        out.pos = L[j].pos; out.koff = L[j].koff;
+        rec[dst[j]] = out;
+    }
+}
+
 }  // namespace
 
 // Exclusive prefix sum of hist[0 .. n-1] in place, hist[n] = total (also written to ctr->n_records);
@@ -424,6 +474,40 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
         else
             scatter_kernel<double><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
                                                        (Rec<double> *)(w + ws.off_records));
+    }
+    ctx->n_launches += nb ? 6 : 4;
+    WPG_CUDA(ctx, cudaGetLastError());
+    return WPG_OK;
+}
+
+// Binning for the polarised gridder: the count pass and the scan are those of wpg_launch_bin (positions do not
+// depend on the correlation), the scatter writes RecP<npol> records.
+int wpg_launch_bin_pol(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight, const double *d_freq,
+                       const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, int npol, char *w) {
+    long long nvis = bp.nrow * bp.nchan;
+    Counters *ctr = (Counters *)(w + ws.off_counters);
+    unsigned *bucket_start = (unsigned *)(w + ws.off_hist);
+    unsigned *hist = bucket_start + 1;
+    unsigned *blocksum = (unsigned *)(w + ws.off_blocksum);
+    cudaStream_t s = ctx->stream;
+    double *fscale = (double *)(w + ws.off_fscale);
+    unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
+    if (bp.vis_block) {
+        const long long nd = (nvis + bp.vis_block - 1) / bp.vis_block;
+        nb = (unsigned)((((nd + kVpt - 1) / kVpt) * bp.vis_block + 255) / 256);
+    }
+    chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale, bp, ctr);
+    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
+    scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
+    scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
+    scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
+    if (nb) {
+        if (npol == 4)
+            scatter_pol_kernel<4><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
+                                                     (RecP<4> *)(w + ws.off_records));
+        else
+            scatter_pol_kernel<2><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
+                                                     (RecP<2> *)(w + ws.off_records));
     }
     ctx->n_launches += nb ? 6 : 4;
     WPG_CUDA(ctx, cudaGetLastError());

@@ -521,6 +521,152 @@ int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     return WPG_OK;
 }
 
+// ------------------------------------------------------------------------------------ pairs, NPOL correlations
+// SURVEY.md §8(f) item 4 (data are row x channel x polarisation): the NPOL correlations of a
+// (row, channel) share window and coefficient slice, so one LDG.128 feeds 2 * NPOL updates — the one change that
+// lifts the L1 coefficient-feed bound of the single-correlation gridder.  Same structure as grid_pairs_kernel
+// (power-of-two S, one record per warp step); grid[pol][N][N].
+template <int NPOL>
+__device__ __forceinline__ void ring_fill_pol(RecP<NPOL> *ring, const RecP<NPOL> *rec, unsigned i0, unsigned i1, unsigned c, int lane) {
+    constexpr unsigned PIECES = sizeof(RecP<NPOL>) / 8;           // 8-byte pieces per record
+    const unsigned long long *g = reinterpret_cast<const unsigned long long *>(rec + i0 + c * kChunk);
+    unsigned long long *sm = reinterpret_cast<unsigned long long *>(ring + ((c * kChunk) & kRingMask));
+    const unsigned first = i0 + c * kChunk;
+    const unsigned npiece = first < i1 ? PIECES * min((unsigned)kChunk, i1 - first) : 0u;
+    for (unsigned q = lane; q < npiece; q += 32)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(sm + q)), "l"(g + q) : "memory");
+}
+
+template <int SCT, int NSLOT, int DEPTH, int MINB, int NPOL>
+__global__ void __launch_bounds__(kRunThreads, MINB)
+grid_pairs_pol_kernel(const RecP<NPOL> *__restrict__ rec, const unsigned *__restrict__ bucket_start, unsigned key_lo,
+                      unsigned key_hi, unsigned *__restrict__ cursor, const float2 *__restrict__ K,
+                      float2 *__restrict__ grid, int N, unsigned seg) {
+    static_assert(kChunk % DEPTH == 0 && SCT > 0 && (SCT & (SCT - 1)) == 0 && SCT * SCT / 2 == NSLOT * 32, "power-of-two support, full warps");
+    using U64 = unsigned long long;
+    constexpr int S = SCT, H = S >> 1;
+    const int lane = threadIdx.x & 31;
+    const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
+    const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
+    const size_t plane = (size_t)N * N;
+
+    __shared__ __align__(16) RecP<NPOL> ring_all[kRunThreads / 32][kChunk * kRing];
+    RecP<NPOL> *ring = ring_all[threadIdx.x >> 5];
+
+    unsigned RG[NSLOT];
+#pragma unroll
+    for (int k = 0; k < NSLOT; ++k) {
+        const int r = k * 32 + lane, rb = r / H, ra2p1 = 2 * (r - rb * H) + 1;
+        RG[k] = (0x8000u + (unsigned)ra2p1) | ((0x8000u + (unsigned)rb) << 16);
+    }
+    constexpr unsigned M = (unsigned)(S - 2) | ((unsigned)(S - 1) << 16);
+
+    for (;;) {
+        unsigned item = 0;
+        if (lane == 0) item = atomicAdd(cursor, 1u);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= nitems) break;
+        const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
+        const unsigned cnt = i1 - i0;
+
+        __syncwarp();
+#pragma unroll
+        for (unsigned c = 0; c < 2; ++c) { ring_fill_pol<NPOL>(ring, rec, i0, i1, c, lane); cp_async_commit(); }
+
+        U64 acc0[NSLOT][NPOL], acc1[NSLOT][NPOL];
+        unsigned qcur[NSLOT] = {};
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) {
+            qcur[k] = 0xFFFFFFFFu;
+#pragma unroll
+            for (int p = 0; p < NPOL; ++p) acc0[k][p] = acc1[k][p] = 0ull;
+        }
+        U64 c0[DEPTH][NSLOT], c1[DEPTH][NSLOT], vis[DEPTH][NPOL];
+        unsigned qn[DEPTH][NSLOT];
+
+        auto flush = [&](int k) {
+            const unsigned q = qcur[k];
+            float2 *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
+#pragma unroll
+            for (int p = 0; p < NPOL; ++p)
+                asm volatile("{ .reg .f32 a, b, c, d;\n\t"
+                             "mov.b64 {a, b}, %0; mov.b64 {c, d}, %1;\n\t"
+                             "red.global.add.v2.f32 [%2], {a, b};\n\t"
+                             "red.global.add.v2.f32 [%2 + 8], {c, d};\n\t"
+                             "mov.b64 %0, 0; mov.b64 %1, 0; }"
+                             : "+l"(acc0[k][p]), "+l"(acc1[k][p]) : "l"(g + p * plane) : "memory");
+        };
+        auto produce = [&](int s, const RecP<NPOL> *rp) {
+#pragma unroll
+            for (int p = 0; p < NPOL; ++p) vis[s][p] = *reinterpret_cast<const U64 *>(&rp->v[p]);
+            const uint2 pk = *reinterpret_cast<const uint2 *>(&rp->pos);
+            const unsigned pos = pk.x, koff = pk.y;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) {
+                const unsigned d = (RG[k] - pos) & M;
+                qn[s][k] = pos + d;
+                ldg128(K + (koff + (d >> 16) * (unsigned)S + (d & 0xFFFFu)), c0[s][k], c1[s][k]);
+            }
+        };
+        auto consume = [&](int s) {
+            bool any = false;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) any |= qn[s][k] != qcur[k];
+            if (__any_sync(0xffffffffu, any)) {
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    if (qn[s][k] != qcur[k]) {
+                        if (qcur[k] != 0xFFFFFFFFu) flush(k);
+                        asm volatile("mov.b32 %0, %1;" : "+r"(qcur[k]) : "r"(qn[s][k]));
+                    }
+                }
+            }
+#pragma unroll
+            for (int p = 0; p < NPOL; ++p) {
+                const float2 vv = unpack2(vis[s][p]);
+                const U64 v1 = vis[s][p], v2 = pack2(-vv.y, vv.x);
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    const float2 k0 = unpack2(c0[s][k]), k1 = unpack2(c1[s][k]);
+                    fma2(acc0[k][p], v1, pack2(k0.x, k0.x)); fma2(acc0[k][p], v2, pack2(k0.y, k0.y));
+                    fma2(acc1[k][p], v1, pack2(k1.x, k1.x)); fma2(acc1[k][p], v2, pack2(k1.y, k1.y));
+                }
+            }
+        };
+        auto enter_chunk = [&](unsigned c) {
+            __syncwarp();
+            ring_fill_pol<NPOL>(ring, rec, i0, i1, c + 2, lane);
+            cp_async_commit();
+            cp_async_wait<2>();
+            __syncwarp();
+        };
+
+        enter_chunk(0);
+#pragma unroll
+        for (int s = 0; s < DEPTH; ++s)
+            if ((unsigned)s < cnt) produce(s, ring + s);
+        for (unsigned j = 0; j < cnt; j += DEPTH) {
+            const unsigned jp = j + DEPTH;
+            if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
+            const RecP<NPOL> *rp = ring + (jp & kRingMask);
+            if (jp + DEPTH <= cnt) {
+#pragma unroll
+                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, rp + s); }
+            } else {
+#pragma unroll
+                for (int s = 0; s < DEPTH; ++s) {
+                    if (j + s < cnt) consume(s);
+                    if (jp + s < cnt) produce(s, rp + s);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k)
+            if (qcur[k] != 0xFFFFFFFFu) flush(k);
+        cp_async_wait<0>();
+    }
+}
+
 // ------------------------------------------------------------------------------------ cells (fp64)
 // The fp64 counterpart of the pair gridder: a c128 coefficient is 16 bytes, so a lane-slot owns ONE cell
 // (residue (rb, ra) of the window, any S) and one LDG.128 feeds one update of four DFMA.  Same structure
@@ -783,6 +929,29 @@ int wpg_launch_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const
     else
         grid_naive_kernel<double><<<blocks, 256, 0, ctx->stream>>>((const float2 *)d_vis, d_uvw, d_weight, d_freq, tab, bp,
                                                                     (const double2 *)K, (double2 *)grid, d_c);
+    ctx->n_launches += 1;
+    WPG_CUDA(ctx, cudaGetLastError());
+    return WPG_OK;
+}
+
+int wpg_launch_grid_pol(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, int npol,
+                        const void *K, void *grid, char *w) {
+    if (bp.nrow == 0) return WPG_OK;
+    const int S = tab.clsS[0];
+    Counters *ctr = (Counters *)(w + ws.off_counters);
+    const unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
+    const unsigned *bs = (const unsigned *)(w + ws.off_hist);
+    cudaStream_t s = ctx->stream;
+#define WPG_POL(SS, NS, DD, MB, NP)                                                                                     \
+    grid_pairs_pol_kernel<SS, NS, DD, MB, NP><<<ctx->sm_count * (ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MB),     \
+        kRunThreads, 0, s>>>((const RecP<NP> *)(w + ws.off_records), bs, 0u, bp.keys_per_class, &ctr->cursor[0],        \
+                             (const float2 *)K, (float2 *)grid, bp.N, seg)
+    if (S == 8 && npol == 4) WPG_POL(8, 1, 2, 3, 4);
+    else if (S == 8 && npol == 2) WPG_POL(8, 1, 4, 3, 2);
+    else if (S == 16 && npol == 4) WPG_POL(16, 4, 1, 1, 4);
+    else if (S == 16 && npol == 2) WPG_POL(16, 4, 2, 1, 2);
+    else return wpg_fail(ctx, WPG_EINVAL, "the polarised gridder takes uniform supports 8 or 16 and 2 or 4 correlations");
+#undef WPG_POL
     ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;

@@ -22,7 +22,7 @@ EXPORTS = (
     "wpg_grid", "wpg_grid_naive", "wpg_grid_host", "wpg_bin", "wpg_dirty_image_workspace_bytes",
     "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms", "wpg_microbench",
     "wpg_baseline_workspace_bytes", "wpg_baseline_reorder", "wpg_grid_baseline_order",
-    "wpg_degrid_workspace_bytes", "wpg_degrid",
+    "wpg_degrid_workspace_bytes", "wpg_degrid", "wpg_grid_pol_workspace_bytes", "wpg_grid_pol",
 )
 
 
@@ -99,6 +99,8 @@ def load():
     lib.wpg_degrid_workspace_bytes.argtypes = [cint]; lib.wpg_degrid_workspace_bytes.restype = sz
     lib.wpg_degrid.argtypes = [vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, vp, sz, ctypes.POINTER(i64)]
     lib.wpg_degrid.restype = cint
+    lib.wpg_grid_pol_workspace_bytes.argtypes = [vp, i64, cint, cint, kd]; lib.wpg_grid_pol_workspace_bytes.restype = sz
+    lib.wpg_grid_pol.argtypes = [vp, vp, vp, vp, vp, i64, cint, cint, vp, kd, vp, vp, sz, stp]; lib.wpg_grid_pol.restype = cint
     lib.wpg_microbench.argtypes = [vp, cint, cint, vp, sz, ctypes.POINTER(dbl)]; lib.wpg_microbench.restype = cint
     _lib = lib
     return lib
@@ -316,6 +318,28 @@ class Context:
             self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(), ant1.data_ptr(), ant2.data_ptr(),
             n_ant, nrow, nchan, stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec, grid.data_ptr(),
             workspace.data_ptr(), workspace.numel(), ctypes.byref(st) if stats else None))
+        return grid, (st.as_dict() if stats else None)
+
+    # ---- polarisation axis
+    def grid_pol(self, vis, uvw, weight, freq, stack, grid=None, workspace=None, stats=False):
+        """vis [nrow][nchan][npol] complex64 -> grid [npol][N][N] (accumulated into), fp32 stacks of support 8 / 16."""
+        t = self.torch
+        assert vis.dtype == t.complex64 and vis.dim() == 3 and vis.is_cuda and vis.is_contiguous()
+        nrow, nchan, npol = vis.shape
+        assert uvw.shape == (nrow, 3) and weight.numel() == nrow * nchan and freq.shape[0] == nchan and stack.prec == F32
+        N = stack.desc.grid_N
+        if grid is None:
+            grid = t.zeros((npol, N, N), dtype=t.complex64, device=self.device)
+        if workspace is None:
+            need = int(self.lib.wpg_grid_pol_workspace_bytes(self.h, nrow, nchan, npol, ctypes.byref(stack.desc)))
+            if need == 0:
+                raise WpgError(EINVAL, "wpg_grid_pol_workspace_bytes: bad arguments (npol 2|4, uniform support 8|16)")
+            workspace = t.empty(need, dtype=t.uint8, device=self.device)
+        st = Stats()
+        self._check(self.lib.wpg_grid_pol(self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(),
+                                          nrow, nchan, npol, stack.data.data_ptr(), ctypes.byref(stack.desc),
+                                          grid.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                          ctypes.byref(st) if stats else None))
         return grid, (st.as_dict() if stats else None)
 
     # ---- degridding (adjoint of grid with unit weights)
