@@ -17,6 +17,7 @@ under torchrun runs N independent replicas ("replicas only") and 
 prefix of the same workload; rank 0 only.
 """
 import argparse
+import ctypes
 import json
 import os
 import sys
@@ -54,6 +55,8 @@ def parse_args():
                          "wpg_grid_baseline_order (track-based workloads, uniform stacks)")
     ap.add_argument("--op", default="grid", choices=["grid", "degrid"],
                     help="grid: the headline step; degrid: wpg_degrid of a random grid for all visibilities (a4+ extra)")
+    ap.add_argument("--npol", type=int, default=1, choices=[1, 2, 4],
+                    help="2 | 4: wpg_grid_pol with N(0,1) visibilities of that many correlations (not the headline config)")
     ap.add_argument("--no-row-block", action="store_true",
                     help="do not pass the rows-per-time-step hint of track-based workloads to the library")
     return ap.parse_args()
@@ -279,6 +282,8 @@ def run_b200(args):
     ws = torch.empty(ctx.grid_workspace_bytes(nrow, nchan, stack), dtype=torch.uint8, device=dev)
     iws = torch.empty(int(ctx.lib.wpg_dirty_image_workspace_bytes(wl.grid_N, prec)), dtype=torch.uint8, device=dev)
 
+    if args.npol > 1:
+        return run_pol(args, ctx, wl, stack, d_uvw, d_wt, d_freq, dev, world, rank, dist)
     if args.op == "degrid":
         return run_degrid(args, ctx, wl, stack, d_uvw, d_freq, prec, dev, world, rank, dist)
     if args.order == "baseline":
@@ -400,6 +405,51 @@ def run_b200(args):
     if not args.no_cpu_baseline and world == 1:
         out["cpu_baseline"] = cpu_baseline(wl)
     print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def run_pol(args, ctx, wl, stack, d_uvw, d_wt, d_freq, dev, world, rank, dist):
+    """Polarised gridding, not the headline metric: a step = zero-fill of the npol grids +
+    binning + polarised gridder + one dirty image per correlation."""
+    import torch
+    npol = args.npol
+    nrow, nchan, N = d_uvw.shape[0], d_freq.shape[0], wl.grid_N
+    gen = torch.Generator(device=dev).manual_seed(3)
+    vis = torch.view_as_complex(torch.randn((nrow, nchan, npol, 2), dtype=torch.float32, device=dev, generator=gen))
+    need = int(ctx.lib.wpg_grid_pol_workspace_bytes(ctx.h, nrow, nchan, npol, ctypes.byref(stack.desc)))
+    ws = torch.empty(need, dtype=torch.uint8, device=dev)
+    grid = torch.zeros((npol, N, N), dtype=torch.complex64, device=dev)
+    iws = torch.empty(int(ctx.lib.wpg_dirty_image_workspace_bytes(N, stack.prec)), dtype=torch.uint8, device=dev)
+    wsum = float(wl.weight.sum())
+    _, stats = ctx.grid_pol(vis, d_uvw, d_wt, d_freq, stack, grid=torch.zeros_like(grid), workspace=ws, stats=True)
+    n_updates = stats["n_updates"] * npol
+
+    def step():
+        grid.zero_()
+        ctx.grid_pol(vis, d_uvw, d_wt, d_freq, stack, grid=grid, workspace=ws)
+        for p in range(npol):
+            ctx.dirty_image(grid[p], stack, wsum, workspace=iws)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize(); ctx.phase_ms()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record(); torch.cuda.synchronize()
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, dev) / args.steps
+    bin_ms, grid_ms = ctx.phase_ms()
+    if rank == 0:
+        ups = n_updates / (grid_ms * 1e-3)
+        print(json.dumps({"metric": METRIC + ", %d correlations" % npol, "unit": UNIT, "value": aggregate_value(n_updates, world, ms),
+                          "ms_per_step": ms, "n_gpus": world, "steps": args.steps, "dtype": "f32", "data": "synthetic",
+                          "config": dict(workload_config(wl, "f32"), npol=npol), "stats": stats,
+                          "roofline": {"bound": "alu", "binning_ms": bin_ms, "gridder_ms": grid_ms, "gridder_updates_per_s": ups,
+                                       "achieved": ups * FLOP_PER_UPDATE / 1e12,
+                                       "peak": SM_COUNT * FP32_LANES * 2 * SM_MAX_GHZ / 1e3,
+                                       "frac": ups * FLOP_PER_UPDATE / 1e12 / (SM_COUNT * FP32_LANES * 2 * SM_MAX_GHZ / 1e3)}}))
     if dist is not None:
         dist.destroy_process_group()
 
