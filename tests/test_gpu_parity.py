@@ -279,6 +279,7 @@ def test_config2_full_size_as_benchmarked(ctx):
         g, s = ctx.grid(*d, ks, grid=grid, workspace=ws, stats=True)
         assert s == rstats
         gh = g.cpu().numpy()
+        print("config2 full size fp32 relerr %.3e" % relerr(gh, ref))          # (-s shows it; profiles/r01_precision.md)
         assert relerr(gh, ref) <= TOL[wpgrid.F32]
         assert abs(gh.sum(dtype=np.complex128) - ref.sum()) <= 1e-5 * abs(ref.sum())
     ctx.set_option("row_block", 0)
@@ -302,6 +303,7 @@ def test_config5_1e7_both_precisions_full_grid(ctx):
         g, s = ctx.grid(*d, ks, stats=True)
         assert s == rstats
         e = relerr(g.cpu().numpy(), ref)
+        print("config5 1e7 prec %d relerr %.3e" % (prec, e))
         assert e <= TOL[prec], (prec, e)
         del g
 
@@ -318,6 +320,7 @@ def test_config3_large_grid_uniform(ctx):
         g, s = ctx.grid(*d, ks, stats=True)
         assert s == rstats
         e = relerr(g.cpu().numpy(), ref)
+        print("config3 N=8192 S=12 prec %d relerr %.3e" % (prec, e))
         assert e <= TOL[prec], (prec, e)
         del g
 
