@@ -946,7 +946,7 @@ int wpg_launch_grid_pol(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, 
     grid_pairs_pol_kernel<SS, NS, DD, MB, NP><<<ctx->sm_count * (ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MB),     \
         kRunThreads, 0, s>>>((const RecP<NP> *)(w + ws.off_records), bs, 0u, bp.keys_per_class, &ctr->cursor[0],        \
                              (const float2 *)K, (float2 *)grid, bp.N, seg)
-    if (S == 8 && npol == 4) WPG_POL(8, 1, 2, 3, 4);
+    if (S == 8 && npol == 4) WPG_POL(8, 1, 4, 3, 4);
     else if (S == 8 && npol == 2) WPG_POL(8, 1, 4, 3, 2);
     else if (S == 16 && npol == 4) WPG_POL(16, 4, 1, 1, 4);
     else if (S == 16 && npol == 2) WPG_POL(16, 4, 2, 1, 2);
