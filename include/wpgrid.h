@@ -122,7 +122,8 @@ int  wpg_grid_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const 
                     const double *d_freq, int64_t nrow, int nchan, const void *d_kernels,
                     const wpg_kdesc *desc, wpg_prec prec, void *d_grid, wpg_stats *h_stats_or_null);
 /* End-to-end variant with HOST buffers: copies the inputs to device scratch owned by the
- * context (grown on demand), zero-fills a device grid, runs wpg_grid, copies the grid to
+ * context (grown on demand; from 2^20 rows on in four row chunks on a copy stream, chunk k being binned and
+ * gridded while chunk k + 1 crosses PCIe — gridding is additive), zero-fills a device grid, runs wpg_grid, copies the grid to
  * h_grid_out (overwritten, [N][N] c64|c128) and synchronises.  d_kernels stays on the device.
  * If h_image_out_or_null is non-NULL the dirty image (wpg_dirty_image with weight_sum) is formed
  * on the device as well and copied to it ([N][N] fp32|fp64). */

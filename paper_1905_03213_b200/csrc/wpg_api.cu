@@ -51,6 +51,9 @@ extern "C" void wpg_destroy(wpg_ctx *ctx) {
         if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
     }
     if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
+    for (int i = 0; i < 4; ++i) if (ctx->ev_chunk[i]) cudaEventDestroy(ctx->ev_chunk[i]);
     if (ctx->plan) cufftDestroy(ctx->plan);
     if (ctx->d_taper) cudaFree(ctx->d_taper);
     if (ctx->d_host_scratch) cudaFree(ctx->d_host_scratch);
@@ -394,19 +397,45 @@ extern "C" int wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uv
     char *base = (char *)ctx->d_host_scratch;
     char *dv = base, *du = dv + b_vis, *dw = du + b_uvw, *df = dw + b_wt, *dg = df + b_freq, *dws = dg + b_grid;
     cudaStream_t s = ctx->stream;
-    WPG_CUDA(ctx, cudaMemcpyAsync(dv, h_vis, (size_t)nvis * 8, cudaMemcpyHostToDevice, s));
-    WPG_CUDA(ctx, cudaMemcpyAsync(du, h_uvw, (size_t)nrow * 24, cudaMemcpyHostToDevice, s));
-    WPG_CUDA(ctx, cudaMemcpyAsync(dw, h_weight, (size_t)nvis * 4, cudaMemcpyHostToDevice, s));
+    // Pipeline over row chunks: gridding is additive (P12), so chunk k is binned and gridded into the same grid
+    // while chunk k + 1 is still crossing PCIe on the copy stream; only the last chunk's compute is exposed.
+    if (!ctx->copy_stream) {
+        WPG_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        WPG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_start, cudaEventDisableTiming));
+        for (int i = 0; i < 4; ++i) WPG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_chunk[i], cudaEventDisableTiming));
+    }
+    const int nchunk = nrow >= (1 << 20) ? 4 : 1;
+    int64_t rows_per = (nrow + nchunk - 1) / nchunk;
+    if (ctx->opt_row_block > 0) rows_per = (rows_per + ctx->opt_row_block - 1) / ctx->opt_row_block * ctx->opt_row_block;
+    WPG_CUDA(ctx, cudaEventRecord(ctx->ev_start, s));                       // the previous call has consumed the buffers
+    WPG_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_stream, ctx->ev_start, 0));
     WPG_CUDA(ctx, cudaMemcpyAsync(df, h_freq, (size_t)nchan * 8, cudaMemcpyHostToDevice, s));
     WPG_CUDA(ctx, cudaMemsetAsync(dg, 0, (size_t)desc->grid_N * desc->grid_N * cplx, s));
-    rc = wpg_grid(ctx, dv, (const double *)du, (const float *)dw, (const double *)df, nrow, nchan, d_kernels, desc,
-                  prec, dg, dws, ws.total, nullptr);
-    if (rc) return rc;
-    WPG_CUDA(ctx, cudaMemcpyAsync(h_grid_out, dg, (size_t)desc->grid_N * desc->grid_N * cplx, cudaMemcpyDeviceToHost, s));
-    if (h_stats) {                                  // before the image step reuses the workspace
-        rc = read_stats(ctx, (const Counters *)(dws + ws.off_counters), h_stats, nullptr);
-        if (rc) return rc;
+    for (int k = 0; k < nchunk; ++k) {
+        const int64_t r0 = std::min(nrow, k * rows_per), r1 = std::min(nrow, r0 + rows_per);
+        if (r1 > r0) {
+            cudaStream_t c = ctx->copy_stream;
+            WPG_CUDA(ctx, cudaMemcpyAsync(dv + r0 * nchan * 8, (const char *)h_vis + r0 * nchan * 8, (size_t)(r1 - r0) * nchan * 8, cudaMemcpyHostToDevice, c));
+            WPG_CUDA(ctx, cudaMemcpyAsync(du + r0 * 24, (const char *)h_uvw + r0 * 24, (size_t)(r1 - r0) * 24, cudaMemcpyHostToDevice, c));
+            WPG_CUDA(ctx, cudaMemcpyAsync(dw + r0 * nchan * 4, (const char *)h_weight + r0 * nchan * 4, (size_t)(r1 - r0) * nchan * 4, cudaMemcpyHostToDevice, c));
+        }
+        WPG_CUDA(ctx, cudaEventRecord(ctx->ev_chunk[k], ctx->copy_stream));
     }
+    wpg_stats tot; memset(&tot, 0, sizeof tot);
+    for (int k = 0; k < nchunk; ++k) {
+        const int64_t r0 = std::min(nrow, k * rows_per), r1 = std::min(nrow, r0 + rows_per);
+        WPG_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_chunk[k], 0));
+        if (r1 <= r0 && k > 0) continue;
+        wpg_stats part; memset(&part, 0, sizeof part);
+        rc = wpg_grid(ctx, dv + r0 * nchan * 8, (const double *)(du + r0 * 24), (const float *)(dw + r0 * nchan * 4),
+                      (const double *)df, r1 - r0, nchan, d_kernels, desc, prec, dg, dws, ws.total, h_stats ? &part : nullptr);
+        if (rc) return rc;
+        tot.n_gridded += part.n_gridded; tot.n_skipped_oob += part.n_skipped_oob;
+        tot.n_skipped_zero_weight += part.n_skipped_zero_weight; tot.n_clamped_w += part.n_clamped_w;
+        tot.n_updates += part.n_updates;
+    }
+    if (h_stats) *h_stats = tot;
+    WPG_CUDA(ctx, cudaMemcpyAsync(h_grid_out, dg, (size_t)desc->grid_N * desc->grid_N * cplx, cudaMemcpyDeviceToHost, s));
     if (h_image_out) {
         size_t b_fft = align_up(wpg_dirty_image_workspace_bytes(desc->grid_N, prec));
         char *dimg = dws + b_fft;

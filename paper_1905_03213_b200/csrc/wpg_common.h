@@ -92,6 +92,9 @@ struct wpg_ctx {
     // side streams for the gridder launches of ragged stacks (one launch per support class; created lazily)
     cudaStream_t side[3] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
+    // copy stream and events of the host-buffer pipeline (wpg_grid_host; created lazily)
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_chunk[4] = {nullptr, nullptr, nullptr, nullptr};
     // cuFFT plan cache
     cufftHandle plan = 0; int plan_N = 0; int plan_prec = -1;
     // taper table cache for dirty_image

@@ -282,7 +282,13 @@ def test_config2_full_size_as_benchmarked(ctx):
         print("config2 full size fp32 relerr %.3e" % relerr(gh, ref))          # (-s shows it; profiles/r01_precision.md)
         assert relerr(gh, ref) <= TOL[wpgrid.F32]
         assert abs(gh.sum(dtype=np.complex128) - ref.sum()) <= 1e-5 * abs(ref.sum())
+    # the host-buffer entry point pipelines four row chunks (copy of chunk k + 1 under the gridding of chunk k)
+    out, s_host = ctx.grid_host(wl.vis, wl.uvw, wl.weight, wl.freq, ks, stats=True)
+    assert s_host == rstats and relerr(out, ref) <= TOL[wpgrid.F32]
     ctx.set_option("row_block", 0)
+    out, s_host = ctx.grid_host(wl.vis[:1_300_001], wl.uvw[:1_300_001], wl.weight[:1_300_001], wl.freq, ks, stats=True)
+    ref13, rstats13 = ogrid.grid(wl.uvw[:1_300_001], wl.vis[:1_300_001], wl.weight[:1_300_001], wl.freq, st, threads=8)
+    assert s_host == rstats13 and relerr(out, ref13) <= TOL[wpgrid.F32]
     # dirty image of the full grid
     wsum = float(wl.weight.sum())
     img = ctx.dirty_image(g, ks, wsum).cpu().numpy().astype(np.float64)
