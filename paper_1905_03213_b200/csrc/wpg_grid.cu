@@ -298,7 +298,8 @@ __device__ __forceinline__ void ldg128(const float2 *p, unsigned long long &c0, 
 }
 
 // G > 1: the warp is split into G groups of 32/G lanes and every group takes its own record, G records per step
-// (record t*G + g goes to group g); a group's NSLOT * 32/G lane-slots hold the S*S/2 pairs of its window.  For
+// (group g walks the g-th contiguous part of the item); a group's NSLOT * 32/G lane-slots hold the S*S/2 pairs of
+// its window.  For
 // S = 4 (8 pairs) this fills the warp; for S = 8 (two half-warps, two pairs per lane) it halves the per-record
 // share of everything that is not a coefficient load or an FMA — record fetch, window test, loop control.
 // RPS > 0: a slot holds RPS whole window rows (RPS * S/2 <= 32 lanes, the rest idle) instead of 32 consecutive
@@ -312,7 +313,8 @@ __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
                   const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
                   const float2 *__restrict__ K, float2 *__restrict__ grid, int N, unsigned seg) {
-    static_assert(kChunk % (DEPTH * G) == 0, "a look-ahead step divides the chunk");
+    static_assert((kChunk / G) % DEPTH == 0, "a look-ahead step divides a group's share of a chunk");
+    constexpr unsigned CL = kChunk / G;                  // records of one group in a chunk of the ring
     static_assert(G == 1 || RPS == 0, "lane groups use the packed pair -> lane-slot mapping");
     static_assert(!ST || G == 1, "window tracking in the producer needs one window per warp");
     constexpr int LPG = 32 / G;                          // lanes per group
@@ -321,7 +323,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     const int H = S >> 1;                                // pairs per window row
     const int NP = S * H;                                // pairs per window
     const int lane = threadIdx.x & 31;
-    const int grp = G > 1 ? lane / LPG : 0;              // this lane's group: takes record t*G + grp of step t
+    const int grp = G > 1 ? lane / LPG : 0;              // this lane's group: takes the grp-th contiguous part of an item
     // key range of this support class: from the device table (ragged stacks) or by value (key_base == nullptr)
     if (key_base) { key_lo = __ldg(key_base + cls); key_hi = __ldg(key_base + cls + 1); }
     const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
@@ -373,9 +375,22 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
         const unsigned cnt = i1 - i0;
 
+        // group g walks records [g * glen, g * glen + cnt_g) of the item (contiguous parts, so that a run of equal
+        // windows stays with one group); chunk c of the ring holds local records [c * CL, (c + 1) * CL) of every group
+        const unsigned glen = (cnt + G - 1) / G;
+        auto part_len = [&](unsigned g) { return g * glen < cnt ? min(glen, cnt - g * glen) : 0u; };
+        const unsigned my_cnt = part_len((unsigned)grp), min_cnt = part_len(G - 1);
+        auto fill = [&](unsigned c) {
+            const unsigned g = (unsigned)lane / CL, t = c * CL + (unsigned)lane % CL;
+            if (lane < kChunk && t < part_len(g))
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(ring + ((c * kChunk + lane) & kRingMask))),
+                             "l"(rec + (i0 + g * glen + t)) : "memory");
+        };
+        auto slot_of = [&](unsigned t) { return ring + (((t / CL) * kChunk + (unsigned)grp * CL + t % CL) & kRingMask); };
+
         __syncwarp();                          // the previous item's ring reads are done
 #pragma unroll
-        for (unsigned c = 0; c < 2; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
+        for (unsigned c = 0; c < 2; ++c) { fill(c); cp_async_commit(); }
 
         U64 acc0[NSLOT], acc1[NSLOT];                       // (re, im) sums of the pair's two cells
         unsigned qcur[NSLOT] = {};                          // (column | row << 16) of the pair's first cell
@@ -468,32 +483,31 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         // records behind, may still re-read window starts of chunk c - 1), make chunks <= c visible
         auto enter_chunk = [&](unsigned c) {
             __syncwarp();
-            ring_fill(ring, rec, i0, i1, c + 2, lane);
+            fill(c + 2);
             cp_async_commit();
             cp_async_wait<2>();
             __syncwarp();
         };
 
-        // prologue: records 0 .. DEPTH-1 into the look-ahead ring
+        // prologue: local records 0 .. DEPTH-1 of every group into the look-ahead ring
         enter_chunk(0);
 #pragma unroll
         for (int s = 0; s < DEPTH; ++s)
-            if ((unsigned)(s * G) < cnt) produce(s, ring + s * G + grp, (unsigned)(s * G + grp) < cnt);
+            if ((unsigned)s < glen) produce(s, slot_of((unsigned)s), (unsigned)s < my_cnt);
 
-        constexpr unsigned STEP = DEPTH * G;                 // records per trip of the loop
-        for (unsigned j = 0; j < cnt; j += STEP) {
-            // the producer is at records j + STEP .. j + 2 STEP - 1: all in one chunk (STEP divides kChunk)
-            const unsigned jp = j + STEP;
-            if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
-            const Rec<float> *rp = ring + (jp & kRingMask) + grp;
-            if (jp + STEP <= cnt) {
+        for (unsigned t = 0; t < glen; t += DEPTH) {
+            // the producer is at local records t + DEPTH .. t + 2 DEPTH - 1: all in one chunk (DEPTH divides CL)
+            const unsigned tp = t + DEPTH;
+            if (tp % CL == 0 && tp < glen) enter_chunk(tp / CL);
+            const Rec<float> *rp = slot_of(tp);
+            if (tp + DEPTH <= min_cnt) {             // every group has all of them
 #pragma unroll
-                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, rp + s * G, true); }
+                for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, rp + s, true); }
             } else {
 #pragma unroll
                 for (int s = 0; s < DEPTH; ++s) {
-                    if (j + s * G < cnt) consume(s);
-                    if (jp + s * G < cnt) produce(s, rp + s * G, jp + s * G + grp < cnt);
+                    if (t + s < glen) consume(s);
+                    if (tp + s < glen) produce(s, rp + s, tp + s < my_cnt);
                 }
             }
         }
