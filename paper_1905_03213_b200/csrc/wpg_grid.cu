@@ -377,16 +377,19 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
 
         // group g walks records [g * glen, g * glen + cnt_g) of the item (contiguous parts, so that a run of equal
         // windows stays with one group); chunk c of the ring holds local records [c * CL, (c + 1) * CL) of every group
-        const unsigned glen = (cnt + G - 1) / G;
-        auto part_len = [&](unsigned g) { return g * glen < cnt ? min(glen, cnt - g * glen) : 0u; };
+        const unsigned glen = G == 1 ? cnt : (cnt + G - 1) / G;
+        auto part_len = [&](unsigned g) { return G == 1 ? cnt : (g * glen < cnt ? min(glen, cnt - g * glen) : 0u); };
         const unsigned my_cnt = part_len((unsigned)grp), min_cnt = part_len(G - 1);
         auto fill = [&](unsigned c) {
+            if (G == 1) { ring_fill(ring, rec, i0, i1, c, lane); return; }
             const unsigned g = (unsigned)lane / CL, t = c * CL + (unsigned)lane % CL;
             if (lane < kChunk && t < part_len(g))
                 asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(ring + ((c * kChunk + lane) & kRingMask))),
                              "l"(rec + (i0 + g * glen + t)) : "memory");
         };
-        auto slot_of = [&](unsigned t) { return ring + (((t / CL) * kChunk + (unsigned)grp * CL + t % CL) & kRingMask); };
+        auto slot_of = [&](unsigned t) {
+            return G == 1 ? ring + (t & kRingMask) : ring + (((t / CL) * kChunk + (unsigned)grp * CL + t % CL) & kRingMask);
+        };
 
         __syncwarp();                          // the previous item's ring reads are done
 #pragma unroll
