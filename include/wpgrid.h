@@ -64,9 +64,11 @@ const char *wpg_last_error(const wpg_ctx *ctx);   /* ctx may be NULL: last error
 int  wpg_version(void);
 
 /* Tuning knobs (all have defaults, 0 = default): "segment" = records per gridder work item;
- * "ctas_per_sm" = gridder CTAs per SM; "key_bits" = log2 cap of the binning sort-key space
- * (default 24 — a 64 MB offset table that stays in L2 — or 26 for ragged stacks: the key is (support class, j0u, j0v) at full resolution unless that exceeds the cap,
- * then low bits of j0v are dropped); "timing" 0/1 (see wpg_phase_ms); "no_pairs" 0/1 (1: fp32 even
+ * "ctas_per_sm" = gridder CTAs per SM; "key_bits" = log2 cap of the binning sort-key space.  Uniform stacks
+ * (default 24: a 64 MB offset table that stays in L2): the key is (support class, j0u, j0v) at full resolution
+ * unless that exceeds the cap,
+ * then low bits of j0v are dropped.  Ragged stacks: the cap is a budget (default: about one key per visibility,
+ * 2^24 .. 2^27) split among the support classes on the device after a census of the classes.  "timing" 0/1 (see wpg_phase_ms); "no_pairs" 0/1 (1: fp32 even
  * supports go through the generic run gridder instead of the pair gridder — for A/B comparison);
  * "row_block" = rows per time step when the rows come time-major, baseline-minor (the row order of a
  * Measurement Set; 0 = unknown, the default): a binning thread then handles the same
