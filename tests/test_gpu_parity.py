@@ -442,3 +442,21 @@ def test_binning_exactness_on_ties_and_near_ties(ctx):
             got = sorted((int(r[2]), int(r[3]), int(round(float(np.array([r[0]], np.uint32).view(np.float32)[0])))) for r in rec)
             assert got == sorted(exp)
         ctx.set_option("row_block", 0)
+
+
+def test_odd_grid_size_and_small_grids(ctx):
+    """Grid sizes that are odd, not a multiple of the support, or barely larger than the window."""
+    rng = np.random.default_rng(77)
+    for N, S, Q in ((255, 7, 8), (101, 8, 4), (12, 8, 8), (9, 4, 2)):
+        cell = 0.05 / N
+        du = 1.0 / 0.05
+        n = 4000
+        uvw = np.stack([rng.uniform(-0.55, 0.55, n) * N * du, rng.uniform(-0.55, 0.55, n) * N * du, rng.uniform(-30, 30, n)], 1)
+        vis = (rng.standard_normal((n, 1)) + 1j * rng.standard_normal((n, 1))).astype(np.complex64)
+        wt = np.ones((n, 1), np.float32)
+        freq = np.array([synth.C0])
+        st = owk.build_stack(3, 25.0, S, Q, N, cell)
+        ref, rstats = ogrid.grid(uvw, vis, wt, freq, st)
+        assert rstats["n_gridded"] > 100 and rstats["n_skipped_oob"] > 100
+        wl = synth.Workload("odd%d" % N, uvw, freq, vis, wt, N, cell, 3, 25.0, S, Q)
+        check_all_paths(ctx, wl, st, ref, rstats)
