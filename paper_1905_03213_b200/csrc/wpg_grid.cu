@@ -308,7 +308,10 @@ __device__ __forceinline__ void ldg128(const float2 *p, unsigned long long &c0, 
 // ST: the producer keeps the lane-slots' offsets of the current window and re-derives them only when the window
 // start changes (supports that are not a power of two pay ~25 instructions per slot for the modulo arithmetic;
 // for powers of two the two-instruction stateless form is cheaper than the test).
-template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1, int RPS = 0, bool ST = false>
+// WS > 1: the window is split over WS work items (each takes all records of its segment but only NSLOT of the
+// WS * NSLOT lane-slot sets): a 16 x 16 window as two items of two slots needs half the registers of one item of
+// four, so twice as many warps are resident.
+template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1, int RPS = 0, bool ST = false, int WS = 1>
 __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
                   const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
@@ -327,7 +330,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     // key range of this support class: from the device table (ragged stacks) or by value (key_base == nullptr)
     if (key_base) { key_lo = __ldg(key_base + cls); key_hi = __ldg(key_base + cls + 1); }
     const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
-    const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
+    const unsigned nitems = WS * ((r_end - r_begin + seg - 1) / seg);
 
     __shared__ __align__(16) Rec<float> ring_all[kRunThreads / 32][kChunk * kRing];
     Rec<float> *ring = ring_all[threadIdx.x >> 5];
@@ -335,12 +338,14 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     // lane-slot constants.  Power-of-two S: RG packs (ra2 + 1, rb) with a guard bit so that
     // (RG - pos) & M is (iu0 | iv << 16) in two instructions: iu0 = (ra2 + par - j0u) mod S equals
     // ((ra2 + 1 - j0u) mod S) & ~1 because S and ra2 are even.
+    static_assert(WS == 1 || (G == 1 && RPS == 0), "window splitting only for the plain one-group mapping");
     unsigned RG[NSLOT];
     int ra2p1[NSLOT], rb[NSLOT];
     bool act[NSLOT];
+    auto set_slots = [&](int part) {                     // part: which NSLOT of the WS * NSLOT slot sets (0 if WS = 1)
 #pragma unroll
     for (int k = 0; k < NSLOT; ++k) {
-        int r = k * LPG + lane % LPG;                    // (G = 1: k * 32 + lane)
+        int r = (part * NSLOT + k) * LPG + lane % LPG;   // (G = 1: slot * 32 + lane)
         act[k] = r < NP;
         if (RPS) {                                       // RPS rows per slot
             const int row = k * RPS + lane / H;
@@ -352,6 +357,8 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         ra2p1[k] = 2 * (r - rb[k] * H) + 1;
         RG[k] = (0x8000u + (unsigned)ra2p1[k]) | ((0x8000u + (unsigned)rb[k]) << 16);
     }
+    };
+    set_slots(0);
     constexpr bool POW2 = SCT > 0 && (SCT & (SCT - 1)) == 0;       // compile-time S that is not a power of two: generic formula, constant folded
     constexpr unsigned M = POW2 ? ((unsigned)(SCT - 2) | ((unsigned)(SCT - 1) << 16)) : 0u;
 
@@ -372,6 +379,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         if (lane == 0) item = atomicAdd(cursor, 1u);
         item = __shfl_sync(0xffffffffu, item, 0);
         if (item >= nitems) break;
+        if (WS > 1) { set_slots((int)(item % WS)); item /= WS; }
         const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
         const unsigned cnt = i1 - i0;
 
@@ -521,7 +529,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
     }
 }
 
-template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1, int RPS = 0, bool ST = false>
+template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1, int RPS = 0, bool ST = false, int WS = 1>
 int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                  int cls, int S) {
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
@@ -529,7 +537,7 @@ int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;         // (x * magicS) >> 20 == x / S for x < 2^13, S <= 32
-    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB, G, RPS, ST><<<blocks, kRunThreads, 0, ctx->stream>>>(
+    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB, G, RPS, ST, WS><<<blocks, kRunThreads, 0, ctx->stream>>>(
         (const Rec<float> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
         bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
         (const float2 *)K, (float2 *)grid, bp.N, seg);
@@ -867,7 +875,7 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
         // fp32, even support: the pair gridder (S*S/2 pairs over 32 lanes)
         const int np = S * S / 2, nslot = (np + 31) / 32;
         if (S == 8) return launch_pairs<8, 2, 4, 3, 2>(ctx, bp, ws, K, grid, w, cls, S);        // two half-warps, two pairs per lane
-        if (S == 16) return launch_pairs<16, 4, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 16) return launch_pairs<16, 2, 4, 3, 1, 0, false, 2>(ctx, bp, ws, K, grid, w, cls, S);   // window split over two work items
         if (S == 4) return launch_pairs<4, 1, 4, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);        // 8 pairs: 4 records per step
         if (S == 12) return launch_pairs<12, 3, 2, 3, 1, 4, true>(ctx, bp, ws, K, grid, w, cls, S);     // 4 rows per slot
         if (nslot <= 1) return launch_pairs<0, 1, 4, 4, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
