@@ -697,7 +697,8 @@ grid_pairs_pol_kernel(const RecP<NPOL> *__restrict__ rec, const unsigned *__rest
 // (residue (rb, ra) of the window, any S) and one LDG.128 feeds one update of four DFMA.  Same structure
 // otherwise: cp.async record ring (24-byte records), stateless look-ahead DEPTH records deep, write-out
 // (two red.global.add.f64) as one asm with the sums as read-write operands.
-template <int SCT, int NSLOT, int DEPTH, int MINB>
+// WS > 1: the window is split over WS work items (NSLOT of the WS * NSLOT lane-slot sets each), as in grid_pairs_kernel.
+template <int SCT, int NSLOT, int DEPTH, int MINB, int WS = 1>
 __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
                     const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
@@ -709,7 +710,7 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
     // key range of this support class: from the device table (ragged stacks) or by value (key_base == nullptr)
     if (key_base) { key_lo = __ldg(key_base + cls); key_hi = __ldg(key_base + cls + 1); }
     const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
-    const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
+    const unsigned nitems = WS * ((r_end - r_begin + seg - 1) / seg);
 
     __shared__ __align__(16) Rec<double> ring_all[kRunThreads / 32][kChunk * kRing];
     Rec<double> *ring = ring_all[threadIdx.x >> 5];
@@ -717,15 +718,18 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
     unsigned RG[NSLOT];
     int ra[NSLOT], rb[NSLOT];
     bool act[NSLOT];
+    auto set_slots = [&](int part) {
 #pragma unroll
     for (int k = 0; k < NSLOT; ++k) {
-        int r = k * 32 + lane;
+        int r = (part * NSLOT + k) * 32 + lane;
         act[k] = r < NC;
         r = act[k] ? r : 0;
         rb[k] = r / S;
         ra[k] = r - rb[k] * S;
         RG[k] = (0x8000u + (unsigned)ra[k]) | ((0x8000u + (unsigned)rb[k]) << 16);
     }
+    };
+    set_slots(0);
     constexpr unsigned M = SCT ? ((unsigned)(SCT - 1) | ((unsigned)(SCT - 1) << 16)) : 0u;
     // (iu | iv << 16) of this lane-slot's cell for a window starting at pos = j0u | j0v << 16
     auto offset_in_window = [&](unsigned pos, int k) -> unsigned {
@@ -743,6 +747,7 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
         if (lane == 0) item = atomicAdd(cursor, 1u);
         item = __shfl_sync(0xffffffffu, item, 0);
         if (item >= nitems) break;
+        if (WS > 1) { set_slots((int)(item % WS)); item /= WS; }
         const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
         const unsigned cnt = i1 - i0;
 
@@ -833,7 +838,7 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
     }
 }
 
-template <int SCT, int NSLOT, int DEPTH, int MINB>
+template <int SCT, int NSLOT, int DEPTH, int MINB, int WS = 1>
 int launch_cells64(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                    int cls, int S) {
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
@@ -841,7 +846,7 @@ int launch_cells64(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws,
     unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;
-    grid_cells64_kernel<SCT, NSLOT, DEPTH, MINB><<<blocks, kRunThreads, 0, ctx->stream>>>(
+    grid_cells64_kernel<SCT, NSLOT, DEPTH, MINB, WS><<<blocks, kRunThreads, 0, ctx->stream>>>(
         (const Rec<double> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
         bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
         (const double2 *)K, (double2 *)grid, bp.N, seg);
@@ -888,8 +893,8 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     if (!F && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp64: one cell per lane-slot, S*S cells over 32 lanes
         const int nslot = (S * S + 31) / 32;
-        if (S == 8) return launch_cells64<8, 2, 4, 2>(ctx, bp, ws, K, grid, w, cls, S);
-        if (S == 16) return launch_cells64<16, 8, 2, 1>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 8) return launch_cells64<8, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 16) return launch_cells64<16, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);       // window split over two work items
         if (S == 4) return launch_cells64<4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 2) return launch_cells64<0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 5) return launch_cells64<0, 5, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
