@@ -898,7 +898,7 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
         if (S == 4) return launch_cells64<4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 2) return launch_cells64<0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 5) return launch_cells64<0, 5, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 8) return launch_cells64<0, 8, 2, 1>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 8) return launch_cells64<0, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
     }
     if (S == 8) return launch_runs<T, 8, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
     if (S == 16) return launch_runs<T, 16, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
