@@ -889,6 +889,8 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
         if (nslot <= 4) return launch_pairs<0, 4, 2, 2, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 6) return launch_pairs<0, 3, 2, 3, 1, 0, true, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 3 slot sets
         if (nslot <= 8) return launch_pairs<0, 4, 2, 2, 1, 0, true, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
+        if (nslot <= 12) return launch_pairs<0, 4, 2, 2, 1, 0, true, 3>(ctx, bp, ws, K, grid, w, cls, S);   // three (S = 24)
+        if (nslot <= 16) return launch_pairs<0, 4, 2, 2, 1, 0, true, 4>(ctx, bp, ws, K, grid, w, cls, S);   // four (S = 26 .. 32)
     }
     if (!F && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp64: one cell per lane-slot, S*S cells over 32 lanes

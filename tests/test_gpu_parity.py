@@ -332,10 +332,10 @@ def test_config3_large_grid_uniform(ctx):
 
 
 # ------------------------------------------------------------------ code paths added with the pair / cell gridders
-@pytest.mark.parametrize("S", [2, 4, 6, 8, 10, 16, 22, 24])
+@pytest.mark.parametrize("S", [2, 4, 6, 8, 10, 16, 22, 24, 28, 32])
 def test_even_supports_segments_and_tails(ctx, S):
     """Every instantiation of the pair gridder (lane groups at S = 4, power-of-two and generic supports, the
-    run-gridder fallback above S = 22) and of the fp64 cell gridder, with work-item lengths that leave ragged
+    window split over two to four work items above S = 16) and of the fp64 cell gridder, with work-item lengths that leave ragged
     tails in the look-ahead ring (1, 5, 17 records) and one item for everything."""
     rng = np.random.default_rng(100 + S)
     N, cell, Q, Nw, w_max, n = 128, 0.06 / 128, 4, 6, 80.0, 6000
