@@ -901,6 +901,12 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
         if (nslot <= 2) return launch_cells64<0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 5) return launch_cells64<0, 5, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
         if (nslot <= 8) return launch_cells64<0, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
+        if (nslot <= 12) return launch_cells64<0, 4, 2, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 16) return launch_cells64<0, 4, 2, 2, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 20) return launch_cells64<0, 4, 2, 2, 5>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 24) return launch_cells64<0, 4, 2, 2, 6>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 28) return launch_cells64<0, 4, 2, 2, 7>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 32) return launch_cells64<0, 4, 2, 2, 8>(ctx, bp, ws, K, grid, w, cls, S);    // S = 32: eight work items
     }
     if (S == 8) return launch_runs<T, 8, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
     if (S == 16) return launch_runs<T, 16, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
