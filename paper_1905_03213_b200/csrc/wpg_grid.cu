@@ -562,28 +562,31 @@ __device__ __forceinline__ void ring_fill_pol(RecP<NPOL> *ring, const RecP<NPOL>
         asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(sm + q)), "l"(g + q) : "memory");
 }
 
-template <int SCT, int NSLOT, int DEPTH, int MINB, int NPOL>
+template <int SCT, int NSLOT, int DEPTH, int MINB, int NPOL, int WS = 1>
 __global__ void __launch_bounds__(kRunThreads, MINB)
 grid_pairs_pol_kernel(const RecP<NPOL> *__restrict__ rec, const unsigned *__restrict__ bucket_start, unsigned key_lo,
                       unsigned key_hi, unsigned *__restrict__ cursor, const float2 *__restrict__ K,
                       float2 *__restrict__ grid, int N, unsigned seg) {
-    static_assert(kChunk % DEPTH == 0 && SCT > 0 && (SCT & (SCT - 1)) == 0 && SCT * SCT / 2 == NSLOT * 32, "power-of-two support, full warps");
+    static_assert(kChunk % DEPTH == 0 && SCT > 0 && (SCT & (SCT - 1)) == 0 && SCT * SCT / 2 == WS * NSLOT * 32, "power-of-two support, full warps");
     using U64 = unsigned long long;
     constexpr int S = SCT, H = S >> 1;
     const int lane = threadIdx.x & 31;
     const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
-    const unsigned nitems = (r_end - r_begin + seg - 1) / seg;
+    const unsigned nitems = WS * ((r_end - r_begin + seg - 1) / seg);   // WS > 1: the window split over WS work items
     const size_t plane = (size_t)N * N;
 
     __shared__ __align__(16) RecP<NPOL> ring_all[kRunThreads / 32][kChunk * kRing];
     RecP<NPOL> *ring = ring_all[threadIdx.x >> 5];
 
     unsigned RG[NSLOT];
+    auto set_slots = [&](int part) {
 #pragma unroll
-    for (int k = 0; k < NSLOT; ++k) {
-        const int r = k * 32 + lane, rb = r / H, ra2p1 = 2 * (r - rb * H) + 1;
-        RG[k] = (0x8000u + (unsigned)ra2p1) | ((0x8000u + (unsigned)rb) << 16);
-    }
+        for (int k = 0; k < NSLOT; ++k) {
+            const int r = (part * NSLOT + k) * 32 + lane, rb = r / H, ra2p1 = 2 * (r - rb * H) + 1;
+            RG[k] = (0x8000u + (unsigned)ra2p1) | ((0x8000u + (unsigned)rb) << 16);
+        }
+    };
+    set_slots(0);
     constexpr unsigned M = (unsigned)(S - 2) | ((unsigned)(S - 1) << 16);
 
     for (;;) {
@@ -591,6 +594,7 @@ grid_pairs_pol_kernel(const RecP<NPOL> *__restrict__ rec, const unsigned *__rest
         if (lane == 0) item = atomicAdd(cursor, 1u);
         item = __shfl_sync(0xffffffffu, item, 0);
         if (item >= nitems) break;
+        if (WS > 1) { set_slots((int)(item % WS)); item /= WS; }
         const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
         const unsigned cnt = i1 - i0;
 
@@ -980,14 +984,14 @@ int wpg_launch_grid_pol(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, 
     const unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     const unsigned *bs = (const unsigned *)(w + ws.off_hist);
     cudaStream_t s = ctx->stream;
-#define WPG_POL(SS, NS, DD, MB, NP)                                                                                     \
-    grid_pairs_pol_kernel<SS, NS, DD, MB, NP><<<ctx->sm_count * (ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MB),     \
+#define WPG_POL(SS, NS, DD, MB, NP, WW)                                                                                 \
+    grid_pairs_pol_kernel<SS, NS, DD, MB, NP, WW><<<ctx->sm_count * (ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MB),     \
         kRunThreads, 0, s>>>((const RecP<NP> *)(w + ws.off_records), bs, 0u, bp.keys_per_class, &ctr->cursor[0],        \
                              (const float2 *)K, (float2 *)grid, bp.N, seg)
-    if (S == 8 && npol == 4) WPG_POL(8, 1, 4, 3, 4);
-    else if (S == 8 && npol == 2) WPG_POL(8, 1, 4, 3, 2);
-    else if (S == 16 && npol == 4) WPG_POL(16, 4, 1, 1, 4);
-    else if (S == 16 && npol == 2) WPG_POL(16, 4, 2, 1, 2);
+    if (S == 8 && npol == 4) WPG_POL(8, 1, 4, 3, 4, 1);
+    else if (S == 8 && npol == 2) WPG_POL(8, 1, 4, 3, 2, 1);
+    else if (S == 16 && npol == 4) WPG_POL(16, 1, 4, 3, 4, 4);      // window split over four work items
+    else if (S == 16 && npol == 2) WPG_POL(16, 2, 2, 2, 2, 2);
     else return wpg_fail(ctx, WPG_EINVAL, "the polarised gridder takes uniform supports 8 or 16 and 2 or 4 correlations");
 #undef WPG_POL
     ctx->n_launches += 1;
