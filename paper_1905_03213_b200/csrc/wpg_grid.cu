@@ -701,12 +701,26 @@ grid_pairs_pol_kernel(const RecP<NPOL> *__restrict__ rec, const unsigned *__rest
 // (residue (rb, ra) of the window, any S) and one LDG.128 feeds one update of four DFMA.  Same structure
 // otherwise: cp.async record ring (24-byte records), stateless look-ahead DEPTH records deep, write-out
 // (two red.global.add.f64) as one asm with the sums as read-write operands.
+// Write one cell out and clear its sums (one asm statement with the sums as read-write operands, see the pair gridder).
+__device__ __forceinline__ void flush_cell(double2 *g, double &x, double &y) {
+    asm volatile("red.global.add.f64 [%2], %0;\n\t"
+                 "red.global.add.f64 [%2 + 8], %1;\n\t"
+                 "mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;"
+                 : "+d"(x), "+d"(y) : "l"(g) : "memory");
+}
+__device__ __forceinline__ void flush_cell(float2 *g, float &x, float &y) {
+    asm volatile("red.global.add.v2.f32 [%2], {%0, %1};\n\t"
+                 "mov.f32 %0, 0f00000000; mov.f32 %1, 0f00000000;"
+                 : "+f"(x), "+f"(y) : "l"(g) : "memory");
+}
+
 // WS > 1: the window is split over WS work items (NSLOT of the WS * NSLOT lane-slot sets each), as in grid_pairs_kernel.
-template <int SCT, int NSLOT, int DEPTH, int MINB, int WS = 1>
+template <typename T, int SCT, int NSLOT, int DEPTH, int MINB, int WS = 1>
 __global__ void __launch_bounds__(kRunThreads, MINB)
-grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
+grid_cells_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ bucket_start,
                     const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S_rt, unsigned magicS, unsigned *__restrict__ cursor,
-                    const double2 *__restrict__ K, double2 *__restrict__ grid, int N, unsigned seg) {
+                    const typename Cplx<T>::type *__restrict__ K, typename Cplx<T>::type *__restrict__ grid, int N, unsigned seg) {
+    using C = typename Cplx<T>::type;
     static_assert(kChunk % DEPTH == 0, "the look-ahead depth divides the chunk");
     const int S = SCT ? SCT : S_rt;
     const int NC = S * S;
@@ -716,8 +730,8 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
     const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
     const unsigned nitems = WS * ((r_end - r_begin + seg - 1) / seg);
 
-    __shared__ __align__(16) Rec<double> ring_all[kRunThreads / 32][kChunk * kRing];
-    Rec<double> *ring = ring_all[threadIdx.x >> 5];
+    __shared__ __align__(16) Rec<T> ring_all[kRunThreads / 32][kChunk * kRing];
+    Rec<T> *ring = ring_all[threadIdx.x >> 5];
 
     unsigned RG[NSLOT];
     int ra[NSLOT], rb[NSLOT];
@@ -759,32 +773,47 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
 #pragma unroll
         for (unsigned c = 0; c < 2; ++c) { ring_fill(ring, rec, i0, i1, c, lane); cp_async_commit(); }
 
-        double accx[NSLOT], accy[NSLOT];
+        T accx[NSLOT], accy[NSLOT];
         unsigned qcur[NSLOT] = {};
 #pragma unroll
-        for (int k = 0; k < NSLOT; ++k) { accx[k] = accy[k] = 0.0; qcur[k] = 0xFFFFFFFFu; }
-        double2 cf[DEPTH][NSLOT];
-        double vre[DEPTH], vim[DEPTH];
+        for (int k = 0; k < NSLOT; ++k) { accx[k] = accy[k] = (T)0; qcur[k] = 0xFFFFFFFFu; }
+        C cf[DEPTH][NSLOT];
+        T vre[DEPTH], vim[DEPTH];
         unsigned qn[DEPTH][NSLOT];
 
+        unsigned posP = 0xFFFFFFFFu, dP[NSLOT], cP[NSLOT];     // window of the last record produced, offsets in it
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) dP[k] = cP[k] = 0;
         auto flush = [&](int k) {
             const unsigned q = qcur[k];
-            double2 *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
-            asm volatile("red.global.add.f64 [%2], %0;\n\t"
-                         "red.global.add.f64 [%2 + 8], %1;\n\t"
-                         "mov.f64 %0, 0d0000000000000000; mov.f64 %1, 0d0000000000000000;"
-                         : "+d"(accx[k]), "+d"(accy[k]) : "l"(g) : "memory");
+            flush_cell(grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu)), accx[k], accy[k]);
         };
-        auto produce = [&](int s, const Rec<double> *rp) {
+        auto produce = [&](int s, const Rec<T> *rp) {
             vre[s] = rp->re; vim[s] = rp->im;
             const uint2 pk = *reinterpret_cast<const uint2 *>(&rp->pos);
             const unsigned pos = pk.x, koff = pk.y;
+            if (SCT == 0) {            // runtime support: offsets re-derived only when the window start changes
+                if (__any_sync(0xffffffffu, pos != posP)) {
 #pragma unroll
-            for (int k = 0; k < NSLOT; ++k) {
-                const unsigned d = offset_in_window(pos, k);
-                qn[s][k] = act[k] ? pos + d : 0xFFFFFFFFu;
-                const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
-                cf[s][k] = __ldg(K + (koff + (act[k] ? coff : 0u)));
+                    for (int k = 0; k < NSLOT; ++k) {
+                        dP[k] = offset_in_window(pos, k);
+                        cP[k] = act[k] ? (dP[k] >> 16) * (unsigned)S + (dP[k] & 0xFFFFu) : 0u;
+                    }
+                    posP = pos;
+                }
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    qn[s][k] = act[k] ? pos + dP[k] : 0xFFFFFFFFu;
+                    cf[s][k] = __ldg(K + (koff + cP[k]));
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    const unsigned d = offset_in_window(pos, k);
+                    qn[s][k] = act[k] ? pos + d : 0xFFFFFFFFu;
+                    const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
+                    cf[s][k] = __ldg(K + (koff + (act[k] ? coff : 0u)));
+                }
             }
         };
         auto consume = [&](int s) {
@@ -800,7 +829,7 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
                     }
                 }
             }
-            const double re = vre[s], im = vim[s];
+            const T re = vre[s], im = vim[s];
 #pragma unroll
             for (int k = 0; k < NSLOT; ++k) {
                 accx[k] = fma(re, cf[s][k].x, accx[k]); accx[k] = fma(-im, cf[s][k].y, accx[k]);
@@ -823,7 +852,7 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
         for (unsigned j = 0; j < cnt; j += DEPTH) {
             const unsigned jp = j + DEPTH;
             if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
-            const Rec<double> *rp = ring + (jp & kRingMask);
+            const Rec<T> *rp = ring + (jp & kRingMask);
             if (jp + DEPTH <= cnt) {
 #pragma unroll
                 for (int s = 0; s < DEPTH; ++s) { consume(s); produce(s, rp + s); }
@@ -842,18 +871,18 @@ grid_cells64_kernel(const Rec<double> *__restrict__ rec, const unsigned *__restr
     }
 }
 
-template <int SCT, int NSLOT, int DEPTH, int MINB, int WS = 1>
-int launch_cells64(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+template <typename T, int SCT, int NSLOT, int DEPTH, int MINB, int WS = 1>
+int launch_cells(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                    int cls, int S) {
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
     int blocks = ctx->sm_count * per_sm;
     unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;
-    grid_cells64_kernel<SCT, NSLOT, DEPTH, MINB, WS><<<blocks, kRunThreads, 0, ctx->stream>>>(
-        (const Rec<double> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
+    grid_cells_kernel<T, SCT, NSLOT, DEPTH, MINB, WS><<<blocks, kRunThreads, 0, ctx->stream>>>(
+        (const Rec<T> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
         bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
-        (const double2 *)K, (double2 *)grid, bp.N, seg);
+        (const typename Cplx<T>::type *)K, (typename Cplx<T>::type *)grid, bp.N, seg);
     ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
@@ -899,18 +928,27 @@ int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
     if (!F && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp64: one cell per lane-slot, S*S cells over 32 lanes
         const int nslot = (S * S + 31) / 32;
-        if (S == 8) return launch_cells64<8, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
-        if (S == 16) return launch_cells64<16, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);       // window split over two work items
-        if (S == 4) return launch_cells64<4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 2) return launch_cells64<0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 5) return launch_cells64<0, 5, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 8) return launch_cells64<0, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
-        if (nslot <= 12) return launch_cells64<0, 4, 2, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 16) return launch_cells64<0, 4, 2, 2, 4>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 20) return launch_cells64<0, 4, 2, 2, 5>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 24) return launch_cells64<0, 4, 2, 2, 6>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 28) return launch_cells64<0, 4, 2, 2, 7>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 32) return launch_cells64<0, 4, 2, 2, 8>(ctx, bp, ws, K, grid, w, cls, S);    // S = 32: eight work items
+        if (S == 8) return launch_cells<double, 8, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
+        if (S == 16) return launch_cells<double, 16, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);       // window split over two work items
+        if (S == 4) return launch_cells<double, 4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 2) return launch_cells<double, 0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 5) return launch_cells<double, 0, 5, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 8) return launch_cells<double, 0, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
+        if (nslot <= 12) return launch_cells<double, 0, 4, 2, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 16) return launch_cells<double, 0, 4, 2, 2, 4>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 20) return launch_cells<double, 0, 4, 2, 2, 5>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 24) return launch_cells<double, 0, 4, 2, 2, 6>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 28) return launch_cells<double, 0, 4, 2, 2, 7>(ctx, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 32) return launch_cells<double, 0, 4, 2, 2, 8>(ctx, bp, ws, K, grid, w, cls, S);    // S = 32: eight work items
+    }
+    if (F && !ctx->opt_no_pairs) {
+        // fp32, odd support (the paper's own experiments use full support 9): one cell per lane-slot
+        const int nslot = (S * S + 31) / 32;
+        if (nslot <= 2) return launch_cells<float, 0, 2, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);            // S <= 7
+        if (nslot <= 4) return launch_cells<float, 0, 4, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);            // S = 9, 11
+        if (nslot <= 8) return launch_cells<float, 0, 4, 2, 3, 2>(ctx, bp, ws, K, grid, w, cls, S);         // S = 13, 15
+        if (nslot <= 16) return launch_cells<float, 0, 4, 2, 3, 4>(ctx, bp, ws, K, grid, w, cls, S);        // S = 17 .. 21
+        if (nslot <= 32) return launch_cells<float, 0, 4, 2, 3, 8>(ctx, bp, ws, K, grid, w, cls, S);        // S = 23 .. 31
     }
     if (S == 8) return launch_runs<T, 8, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
     if (S == 16) return launch_runs<T, 16, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
