@@ -209,6 +209,55 @@ int oracle_degrid(const double *uvw, const double *freq, int64_t nrow, int nchan
     return 0;
 }
 
+/* P11: flux conservation, evaluated WITHOUT a grid, in O(nvis):
+ *   sum_cells grid            = sum_k wt_k V_k sigma [p_k][ov_k][ou_k],         sigma  = sum_{iv,iu} K
+ *   sum_cells grid * ju       = sum_k wt_k V_k (j0u_k sigma + sigma_u),         sigma_u = sum_{iv,iu} iu K
+ *   sum_cells grid * jv       = sum_k wt_k V_k (j0v_k sigma + sigma_v),         sigma_v = sum_{iv,iu} iv K
+ * (the two first moments also pin WHERE the flux went: a window placed one cell off changes them).
+ * The caller supplies the slice sums: sig[3 * s + {0,1,2}] complex (re, im pairs) for slice s = soff[p] + ov Q + ou,
+ * soff[p] = p Q^2.  Plane, window and sub-cell offsets, validity and counters exactly as in grid_rows (G1-G4).
+ * out: 8 doubles = {sum re, im; u-moment re, im; v-moment re, im; L1 = sum |wt V| |sigma|, 0}; stats_out: 5 int64. */
+int oracle_flux(const double *uvw, const float *vis, const float *weight, const double *freq,
+                int64_t nrow, int nchan, const double *sig, const int *support,
+                int Nw, int Q, int N, double cell, double w_max,
+                double *out, int64_t *stats_out, int nthreads) {
+    double a0r = 0, a0i = 0, aur = 0, aui = 0, avr = 0, avi = 0, l1 = 0;
+    int64_t ng = 0, noob = 0, nzero = 0, nclamp = 0, nupd = 0;
+    if (nthreads < 1) nthreads = 1;
+#pragma omp parallel for schedule(static) num_threads(nthreads) \
+    reduction(+ : a0r, a0i, aur, aui, avr, avi, l1, ng, noob, nzero, nclamp, nupd)
+    for (int64_t r = 0; r < nrow; ++r) {
+        for (int c = 0; c < nchan; ++c) {
+            double wt = (double)weight[r * nchan + c];
+            if (wt == 0.0) { nzero++; continue; }
+            double f = freq[c] / C0;
+            double u = uvw[3 * r + 0] * f, v = uvw[3 * r + 1] * f, w = uvw[3 * r + 2] * f;
+            int clamped;
+            int p = oracle_plane(w, w_max, Nw, &clamped);
+            int S = support[p];
+            int64_t j0u, j0v; int ou, ov;
+            oracle_index_map(u, N, cell, S, Q, &j0u, &ou);
+            oracle_index_map(v, N, cell, S, Q, &j0v, &ov);
+            if (j0u < 0 || j0v < 0 || j0u + S > N || j0v + S > N) { noob++; continue; }
+            if (clamped) nclamp++;
+            double vr = wt * (double)vis[2 * (r * nchan + c) + 0];
+            double vi = wt * (double)vis[2 * (r * nchan + c) + 1];
+            const double *sg = sig + 6 * (((int64_t)p * Q + ov) * Q + ou);
+            double s0r = sg[0], s0i = sg[1];
+            double sur = (double)j0u * s0r + sg[2], sui = (double)j0u * s0i + sg[3];
+            double svr = (double)j0v * s0r + sg[4], svi = (double)j0v * s0i + sg[5];
+            a0r += vr * s0r - vi * s0i; a0i += vr * s0i + vi * s0r;
+            aur += vr * sur - vi * sui; aui += vr * sui + vi * sur;
+            avr += vr * svr - vi * svi; avi += vr * svi + vi * svr;
+            l1 += sqrt(vr * vr + vi * vi) * sqrt(s0r * s0r + s0i * s0i);
+            ng++; nupd += (int64_t)S * S;
+        }
+    }
+    out[0] = a0r; out[1] = a0i; out[2] = aur; out[3] = aui; out[4] = avr; out[5] = avi; out[6] = l1; out[7] = 0.0;
+    stats_out[0] = ng; stats_out[1] = noob; stats_out[2] = nzero; stats_out[3] = nclamp; stats_out[4] = nupd;
+    return 0;
+}
+
 int oracle_max_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -43,6 +43,8 @@ def _load():
         lib.oracle_grid.restype = cint
         lib.oracle_degrid.argtypes = [vp, vp, i64, cint, vp, vp, vp, cint, cint, cint, dbl, dbl, vp, vp, vp]
         lib.oracle_degrid.restype = cint
+        lib.oracle_flux.argtypes = [vp, vp, vp, vp, i64, cint, vp, vp, cint, cint, cint, dbl, dbl, vp, vp, cint]
+        lib.oracle_flux.restype = cint
         lib.oracle_max_threads.restype = cint
         _lib = lib
     return _lib
@@ -116,3 +118,41 @@ def degrid(uvw, freq, stack, grid):
     if rc != 0:
         raise RuntimeError("oracle_degrid failed rc=%d" % rc)
     return out, {"n_predicted": int(cnt[0]), "n_outside": int(cnt[1])}
+
+
+def slice_moments(stack):
+    """[Nw * Q * Q][3] complex128: (sigma, sigma_u, sigma_v) of every slice K[p][ov][ou] — its sum and its first
+    moments over the window columns iu and rows iv (P11)."""
+    Q = stack.oversample
+    out = np.empty((stack.Nw * Q * Q, 3), dtype=np.complex128)
+    for p in range(stack.Nw):
+        Kp = stack.plane(p)                                  # [Q][Q][S][S]
+        S = Kp.shape[-1]
+        i = np.arange(S, dtype=np.float64)
+        blk = out[p * Q * Q:(p + 1) * Q * Q].reshape(Q, Q, 3)
+        blk[..., 0] = Kp.sum(axis=(2, 3))
+        blk[..., 1] = (Kp * i[None, None, None, :]).sum(axis=(2, 3))
+        blk[..., 2] = (Kp * i[None, None, :, None]).sum(axis=(2, 3))
+    return out
+
+
+def flux(uvw, vis, weight, freq, stack, threads=1):
+    """P11 without a grid, O(nvis) (oracle_flux in grid_oracle.c): what sum(grid), sum(grid * ju) and sum(grid * jv)
+    of the gridded result must be.  Returns ({"sum", "mom_u", "mom_v": complex, "l1": float}, stats dict)."""
+    uvw = np.ascontiguousarray(uvw, dtype=np.float64)
+    vis = np.ascontiguousarray(vis, dtype=np.complex64)
+    weight = np.ascontiguousarray(weight, dtype=np.float32)
+    freq = np.ascontiguousarray(freq, dtype=np.float64)
+    nrow, nchan = uvw.shape[0], freq.shape[0]
+    assert vis.size == nrow * nchan and weight.size == nrow * nchan
+    sig = np.ascontiguousarray(slice_moments(stack))
+    sup = np.ascontiguousarray(stack.support, dtype=np.int32)
+    out = np.zeros(8, dtype=np.float64)
+    st = np.zeros(5, dtype=np.int64)
+    rc = _load().oracle_flux(uvw.ctypes.data, vis.ctypes.data, weight.ctypes.data, freq.ctypes.data, nrow, nchan,
+                             sig.ctypes.data, sup.ctypes.data, stack.Nw, stack.oversample, stack.grid_N,
+                             stack.cell, stack.w_max, out.ctypes.data, st.ctypes.data, int(threads))
+    if rc != 0:
+        raise RuntimeError("oracle_flux failed rc=%d" % rc)
+    return ({"sum": complex(out[0], out[1]), "mom_u": complex(out[2], out[3]), "mom_v": complex(out[4], out[5]),
+             "l1": float(out[6])}, dict(zip(STAT_NAMES, (int(x) for x in st))))

@@ -332,12 +332,8 @@ def test_config3_large_grid_uniform(ctx):
 
 
 # ------------------------------------------------------------------ code paths added with the pair / cell gridders
-@pytest.mark.parametrize("S", [2, 4, 6, 8, 10, 16, 22, 24, 28, 32])
-def test_even_supports_segments_and_tails(ctx, S):
-    """Every instantiation of the pair gridder (lane groups at S = 4, power-of-two and generic supports, the
-    window split over two to four work items above S = 16) and of the fp64 cell gridder, with work-item lengths that leave ragged
-    tails in the look-ahead ring (1, 5, 17 records) and one item for everything."""
-    rng = np.random.default_rng(100 + S)
+def _support_case(S, seed):
+    rng = np.random.default_rng(seed)
     N, cell, Q, Nw, w_max, n = 128, 0.06 / 128, 4, 6, 80.0, 6000
     du = 1.0 / 0.06
     uvw = np.stack([rng.uniform(-40, 40, n) * du, rng.uniform(-40, 40, n) * du, rng.uniform(-90, 90, n)], 1)
@@ -348,9 +344,32 @@ def test_even_supports_segments_and_tails(ctx, S):
     st = owk.build_stack(Nw, w_max, S, Q, N, cell)
     ref, rstats = ogrid.grid(uvw, vis, wt, freq, st)
     assert rstats["n_gridded"] > 5000
-    wl = synth.Workload("even%d" % S, uvw, freq, vis, wt, N, cell, Nw, w_max, S, Q)
+    return synth.Workload("S%d" % S, uvw, freq, vis, wt, N, cell, Nw, w_max, S, Q), st, ref, rstats
+
+
+@pytest.mark.parametrize("S", [2, 4, 6, 8, 10, 12, 14, 16, 18, 20, 22, 24, 26, 28, 30, 32])
+def test_even_supports_segments_and_tails(ctx, S):
+    """Every instantiation of the pair gridder (lane groups at S = 4 and 8, power-of-two and generic supports with
+    1..4 lane-slot sets, the window split over two to four work items from S = 16 up) and of the fp64 cell gridder
+    (window split over 2..8 work items), with work-item lengths that leave ragged tails in the look-ahead ring
+    (1, 5, 17 records) and one item for everything.  launch_class (csrc/wpg_grid.cu) picks the instantiation from S
+    alone for a uniform stack, so this list reaches every even-support line of it in both precisions."""
+    wl, st, ref, rstats = _support_case(S, 100 + S)
     check_all_paths(ctx, wl, st, ref, rstats, segments=(0, 1, 5, 17, 100000))
     ctx.set_option("no_pairs", 1)                                       # the run gridder on the same input
+    check_all_paths(ctx, wl, st, ref, rstats)
+    ctx.set_option("no_pairs", 0)
+
+
+@pytest.mark.parametrize("S", [3, 5, 7, 9, 11, 13, 15, 17, 19, 21, 23, 27, 31])
+def test_odd_supports_segments_and_tails(ctx, S):
+    """Odd supports (the paper's own experiments use full support 9): fp32 goes through the cell
+    gridder with one cell per lane-slot (2 slot sets up to S = 7, 4 at S = 9 / 11, the window split over 2 / 4 / 8
+    work items at S = 13-15 / 17-21 / 23-31), fp64 through its 5-slot and window-split lines (S = 9 ... 27).  Same
+    ragged work-item lengths as the even supports, and the run gridder on the same input."""
+    wl, st, ref, rstats = _support_case(S, 300 + S)
+    check_all_paths(ctx, wl, st, ref, rstats, segments=(0, 1, 5, 17, 100000))
+    ctx.set_option("no_pairs", 1)
     check_all_paths(ctx, wl, st, ref, rstats)
     ctx.set_option("no_pairs", 0)
 

@@ -160,3 +160,59 @@ def test_ragged_stack_gridding_matches_per_plane_uniform():
         upd += S * S
     assert s["n_updates"] == upd and s["n_gridded"] == n
     assert np.max(np.abs(g - exp)) <= 1e-13 * np.max(np.abs(exp))
+
+
+# ---------------------------------------------------------------- P11 without a grid (oracle_flux)
+def test_flux_matches_python_p11_on_config1(cfg1_small):
+    """oracle_flux (the O(nvis) C loop used to check full-size GPU runs) against the Python P11 sum written out
+    here from index_map / plane_of and the stack's slice sums, and against the gridded result itself."""
+    wl, st = cfg1_small
+    K = st.as_array()
+    sig = K.sum(axis=(3, 4))
+    i = np.arange(7, dtype=np.float64)
+    sig_u = (K * i).sum(axis=(3, 4)); sig_v = (K * i[:, None]).sum(axis=(3, 4))
+    tot = mu = mv = 0j
+    for k in range(wl.uvw.shape[0]):
+        j0u, ou = gridder.index_map(wl.uvw[k, 0], wl.grid_N, wl.cell, 7, 8)
+        j0v, ov = gridder.index_map(wl.uvw[k, 1], wl.grid_N, wl.cell, 7, 8)
+        p, _ = gridder.plane_of(wl.uvw[k, 2], wl.w_max, wl.Nw)
+        v = complex(wl.vis[k, 0])
+        tot += v * sig[p, ov, ou]
+        mu += v * (j0u * sig[p, ov, ou] + sig_u[p, ov, ou])
+        mv += v * (j0v * sig[p, ov, ou] + sig_v[p, ov, ou])
+    fl, fstats = gridder.flux(wl.uvw, wl.vis, wl.weight, wl.freq, st)
+    assert abs(fl["sum"] - tot) <= 1e-13 * fl["l1"]
+    assert abs(fl["mom_u"] - mu) <= 1e-13 * fl["l1"] * wl.grid_N
+    assert abs(fl["mom_v"] - mv) <= 1e-13 * fl["l1"] * wl.grid_N
+    g, stats = gridder.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st)
+    assert fstats == stats
+    ju = np.arange(wl.grid_N, dtype=np.float64)
+    assert abs(g.sum() - fl["sum"]) <= 1e-13 * fl["l1"]
+    assert abs((g * ju[None, :]).sum() - fl["mom_u"]) <= 1e-13 * fl["l1"] * wl.grid_N
+    assert abs((g * ju[:, None]).sum() - fl["mom_v"]) <= 1e-13 * fl["l1"] * wl.grid_N
+    # a window placed one cell off, or a dropped visibility, is far outside these bounds
+    assert abs(fl["sum"]) > 1e-6 * fl["l1"] and 1e-13 * fl["l1"] * wl.grid_N < 1e-3 * abs(sig[0, 0, 0])
+
+
+def test_flux_ragged_multichannel_flags_and_threads():
+    """oracle_flux on a ragged stack with several channels, zero weights, clamped w and off-grid windows: counters
+    equal oracle_grid's, sums and first moments equal those of the gridded result; threads change nothing."""
+    N, cell, Q, Nw, w_max = 128, 0.2 / 128, 4, 4, 400.0
+    sup = wkernel.ragged_support(Nw, w_max, N, cell, 8, 32)
+    st = wkernel.build_stack(Nw, w_max, sup, Q, N, cell)
+    rng = np.random.default_rng(11)
+    n, nchan = 500, 3
+    uvw = np.stack([rng.uniform(-330, 330, n), rng.uniform(-330, 330, n), rng.uniform(-450, 450, n)], 1)
+    freq = np.array([0.9, 1.0, 1.1]) * synth.C0
+    vis = (rng.standard_normal((n, nchan)) + 1j * rng.standard_normal((n, nchan))).astype(np.complex64)
+    wt = rng.uniform(0.0, 2.0, (n, nchan)).astype(np.float32)
+    wt[rng.uniform(size=wt.shape) < 0.1] = 0.0
+    g, stats = gridder.grid(uvw, vis, wt, freq, st)
+    assert stats["n_skipped_oob"] > 0 and stats["n_skipped_zero_weight"] > 0 and stats["n_clamped_w"] > 0
+    ju = np.arange(N, dtype=np.float64)
+    for threads in (1, 3):
+        fl, fstats = gridder.flux(uvw, vis, wt, freq, st, threads=threads)
+        assert fstats == stats
+        assert abs(g.sum() - fl["sum"]) <= 1e-13 * fl["l1"]
+        assert abs((g * ju[None, :]).sum() - fl["mom_u"]) <= 1e-13 * fl["l1"] * N
+        assert abs((g * ju[:, None]).sum() - fl["mom_v"]) <= 1e-13 * fl["l1"] * N
