@@ -33,7 +33,8 @@ extern "C" int wpg_create(wpg_ctx **out, int device, void *cuda_stream) {
     wpg_ctx *ctx = new wpg_ctx();
     ctx->device = device;
     ctx->stream = (cudaStream_t)cuda_stream;
-    if (cudaSetDevice(device) != cudaSuccess ||
+    DeviceGuard guard(device);             // the caller's current device is restored on return
+    if (guard.err != cudaSuccess ||
         cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
         delete ctx;
         return wpg_fail(nullptr, WPG_ECUDA, "wpg_create: cannot select device %d", device);
@@ -44,7 +45,7 @@ extern "C" int wpg_create(wpg_ctx **out, int device, void *cuda_stream) {
 
 extern "C" void wpg_destroy(wpg_ctx *ctx) {
     if (!ctx) return;
-    cudaSetDevice(ctx->device);
+    DeviceGuard guard(ctx->device);
     for (auto &e : ctx->ev) cudaEventDestroy(e);
     for (int i = 0; i < 3; ++i) {
         if (ctx->side[i]) cudaStreamDestroy(ctx->side[i]);
@@ -264,7 +265,6 @@ static int bin_common(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, cons
     if (rc) return rc;
     if (!d_workspace || workspace_bytes < ws->total)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, ws->total);
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
     if ((rc = wpg_mark(ctx, 0))) return rc;
     char *w = (char *)d_workspace;
     // counters + histogram are contiguous at the head of the workspace
@@ -275,6 +275,8 @@ static int bin_common(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, cons
 extern "C" int wpg_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
                        const double *d_freq, int64_t nrow, int nchan, const wpg_kdesc *desc, wpg_prec prec,
                        void *d_workspace, size_t workspace_bytes, wpg_bin_info *info, wpg_stats *h_stats) {
+    if (!ctx) return WPG_EINVAL;
+    WPG_DEVICE(ctx);
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     int rc = bin_common(ctx, d_vis, d_uvw, d_weight, d_freq, nrow, nchan, desc, prec, d_workspace, workspace_bytes, &tab, &bp, &ws);
     if (rc) return rc;
@@ -296,6 +298,7 @@ extern "C" int wpg_grid(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, co
                         void *d_workspace, size_t workspace_bytes, wpg_stats *h_stats) {
     if (!ctx) return WPG_EINVAL;
     if (!d_kernels || !d_grid) return wpg_fail(ctx, WPG_EINVAL, "kernels or grid pointer is NULL");
+    WPG_DEVICE(ctx);
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     int rc = bin_common(ctx, d_vis, d_uvw, d_weight, d_freq, nrow, nchan, desc, prec, d_workspace, workspace_bytes, &tab, &bp, &ws);
     if (rc) return rc;
@@ -340,7 +343,7 @@ extern "C" int wpg_grid_pol(wpg_ctx *ctx, const void *d_vis, const double *d_uvw
     if (rc) return rc;
     if (!d_workspace || workspace_bytes < ws.total)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, ws.total);
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     char *w = (char *)d_workspace;
     if ((rc = wpg_mark(ctx, 0))) return rc;
     WPG_CUDA(ctx, cudaMemsetAsync(w, 0, ws.off_blocksum, ctx->stream));
@@ -363,7 +366,7 @@ extern "C" int wpg_grid_naive(wpg_ctx *ctx, const void *d_vis, const double *d_u
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     rc = wpg_make_plan(ctx, desc, nrow, nchan, prec, &tab, &bp, &ws);
     if (rc) return rc;
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     Counters *d_c = nullptr;
     WPG_CUDA(ctx, cudaMallocAsync((void **)&d_c, sizeof(Counters), ctx->stream));
     WPG_CUDA(ctx, cudaMemsetAsync(d_c, 0, sizeof(Counters), ctx->stream));
@@ -383,7 +386,7 @@ extern "C" int wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uv
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     rc = wpg_make_plan(ctx, desc, nrow, nchan, prec, &tab, &bp, &ws);
     if (rc) return rc;
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     int64_t nvis = nrow * nchan;
     size_t cplx = prec == WPG_F32 ? 8 : 16;
     size_t b_vis = align_up((size_t)nvis * 8), b_uvw = align_up((size_t)nrow * 24), b_wt = align_up((size_t)nvis * 4),

@@ -105,9 +105,9 @@ bl_build_records_kernel(const float2 *__restrict__ vis, const double *__restrict
         else { c_grid = 1; c_clamp = r.clamped; c_upd = r.S * r.S; }
         const int j0u = min(max(r.j0u, 0), P.N - r.S), j0v = min(max(r.j0v, 0), P.N - r.S);
         const float2 v = __ldg(vis + i);
-        const TT w = ok ? (TT)wt : (TT)0;
+        // literal zeros for a flagged / off-grid sample: its value may be NaN or Inf (RFI), and 0 * NaN = NaN
         Rec<TT> out;
-        out.re = w * (TT)v.x; out.im = w * (TT)v.y;
+        out.re = ok ? (TT)wt * (TT)v.x : (TT)0; out.im = ok ? (TT)wt * (TT)v.y : (TT)0;
         out.pos = (unsigned)j0u | ((unsigned)j0v << 16);
         out.koff = ok ? wpg_koff(r, P, ST) : (unsigned)ST.off(r.p);
         rec[idx] = out;
@@ -195,7 +195,7 @@ extern "C" int wpg_baseline_reorder(wpg_ctx *ctx, const int *d_ant1, const int *
     if (!d_workspace || workspace_bytes < L.total)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, L.total);
     if (!d_bstart_out || !d_perm_out) return wpg_fail(ctx, WPG_EINVAL, "output pointer is NULL");
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     char *w = (char *)d_workspace;
     rc = bl_reorder(ctx, d_ant1, d_ant2, n_ant, nrow, w, L);
     if (rc) return rc;
@@ -222,7 +222,7 @@ extern "C" int wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const do
     const BlLayout L = bl_layout(nrow, nchan, n_ant, recb);
     if (!d_workspace || workspace_bytes < L.total)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, L.total);
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     char *w = (char *)d_workspace;
     cudaStream_t s = ctx->stream;
     if ((rc = wpg_mark(ctx, 0))) return rc;

@@ -92,6 +92,7 @@ struct wpg_ctx {
     // side streams for the gridder launches of ragged stacks (one launch per support class; created lazily)
     cudaStream_t side[3] = {nullptr, nullptr, nullptr};
     cudaEvent_t ev_fork = nullptr, ev_join[3] = {nullptr, nullptr, nullptr};
+    bool side_ready = false;
     // copy stream and events of the host-buffer pipeline (wpg_grid_host; created lazily)
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_start = nullptr, ev_chunk[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -104,6 +105,23 @@ struct wpg_ctx {
 };
 
 int wpg_fail(wpg_ctx *ctx, int code, const char *fmt, ...);
+
+// Selects the context's device for the duration of an entry point and restores the caller's current device on
+// return (the caller may drive several GPUs from one thread; torch's current device must not change under it).
+struct DeviceGuard {
+    int prev = -1; cudaError_t err;
+    explicit DeviceGuard(int device) {
+        err = cudaGetDevice(&prev);
+        if (err == cudaSuccess && prev != device) err = cudaSetDevice(device); else if (err == cudaSuccess) prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
+};
+#define WPG_DEVICE(ctx)                                                                          \
+    DeviceGuard dev_guard_((ctx)->device);                                                       \
+    if (dev_guard_.err != cudaSuccess)                                                           \
+        return wpg_fail(ctx, WPG_ECUDA, "cannot select device %d: %s", (ctx)->device, cudaGetErrorString(dev_guard_.err))
 #define WPG_CUDA(ctx, call)                                                                   \
     do {                                                                                      \
         cudaError_t e_ = (call);                                                              \

@@ -112,7 +112,7 @@ extern "C" int wpg_degrid(wpg_ctx *ctx, const void *d_grid, const double *d_uvw,
     const size_t need = wpg_degrid_workspace_bytes(nchan);
     if (!d_workspace || workspace_bytes < need)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, need);
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     cudaStream_t s = ctx->stream;
     char *w = (char *)d_workspace;
     unsigned long long *counts = (unsigned long long *)w;             // kStatSlots x {predicted, outside}

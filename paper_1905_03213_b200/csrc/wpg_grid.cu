@@ -530,14 +530,14 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
 }
 
 template <int SCT, int NSLOT, int DEPTH, int MINB, int G = 1, int RPS = 0, bool ST = false, int WS = 1>
-int launch_pairs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+int launch_pairs(wpg_ctx *ctx, cudaStream_t strm, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                  int cls, int S) {
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
     int blocks = ctx->sm_count * per_sm;
     unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;         // (x * magicS) >> 20 == x / S for x < 2^13, S <= 32
-    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB, G, RPS, ST, WS><<<blocks, kRunThreads, 0, ctx->stream>>>(
+    grid_pairs_kernel<SCT, NSLOT, DEPTH, MINB, G, RPS, ST, WS><<<blocks, kRunThreads, 0, strm>>>(
         (const Rec<float> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
         bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
         (const float2 *)K, (float2 *)grid, bp.N, seg);
@@ -872,14 +872,14 @@ grid_cells_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ b
 }
 
 template <typename T, int SCT, int NSLOT, int DEPTH, int MINB, int WS = 1>
-int launch_cells(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+int launch_cells(wpg_ctx *ctx, cudaStream_t strm, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                    int cls, int S) {
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
     int blocks = ctx->sm_count * per_sm;
     unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     unsigned magicS = (1u << 20) / (unsigned)S + 1u;
-    grid_cells_kernel<T, SCT, NSLOT, DEPTH, MINB, WS><<<blocks, kRunThreads, 0, ctx->stream>>>(
+    grid_cells_kernel<T, SCT, NSLOT, DEPTH, MINB, WS><<<blocks, kRunThreads, 0, strm>>>(
         (const Rec<T> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
         bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, &ctr->cursor[cls],
         (const typename Cplx<T>::type *)K, (typename Cplx<T>::type *)grid, bp.N, seg);
@@ -889,14 +889,14 @@ int launch_cells(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, c
 }
 
 template <typename T, int SCT, int NSLOT, int MINB>
-int launch_runs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+int launch_runs(wpg_ctx *ctx, cudaStream_t strm, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                 int cls, int S) {
     using C = typename Cplx<T>::type;
     int per_sm = ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MINB;
     int blocks = ctx->sm_count * per_sm;
     unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     Counters *ctr = (Counters *)(w + ws.off_counters);
-    grid_runs_kernel<T, SCT, NSLOT, MINB><<<blocks, kRunThreads, 0, ctx->stream>>>(
+    grid_runs_kernel<T, SCT, NSLOT, MINB><<<blocks, kRunThreads, 0, strm>>>(
         (const Rec<T> *)(w + ws.off_records), (const unsigned *)(w + ws.off_hist),
         bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class, (unsigned)(cls + 1) * bp.keys_per_class, S, &ctr->cursor[cls],
         (const C *)K, (C *)grid, bp.N, seg);
@@ -906,59 +906,59 @@ int launch_runs(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, co
 }
 
 template <typename T>
-int launch_class(wpg_ctx *ctx, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
+int launch_class(wpg_ctx *ctx, cudaStream_t strm, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                  int cls, int S) {
     constexpr bool F = sizeof(T) == 4;
     if (F && S % 2 == 0 && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp32, even support: the pair gridder (S*S/2 pairs over 32 lanes)
         const int np = S * S / 2, nslot = (np + 31) / 32;
-        if (S == 8) return launch_pairs<8, 2, 4, 3, 2>(ctx, bp, ws, K, grid, w, cls, S);        // two half-warps, two pairs per lane
-        if (S == 16) return launch_pairs<16, 2, 4, 3, 1, 0, false, 2>(ctx, bp, ws, K, grid, w, cls, S);   // window split over two work items
-        if (S == 4) return launch_pairs<4, 1, 4, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);        // 8 pairs: 4 records per step
-        if (S == 12) return launch_pairs<12, 3, 2, 3, 1, 4, true>(ctx, bp, ws, K, grid, w, cls, S);     // 4 rows per slot
-        if (nslot <= 1) return launch_pairs<0, 1, 4, 4, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 2) return launch_pairs<0, 2, 4, 3, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 3) return launch_pairs<0, 3, 2, 3, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 4) return launch_pairs<0, 4, 2, 2, 1, 0, true>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 6) return launch_pairs<0, 3, 2, 3, 1, 0, true, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 3 slot sets
-        if (nslot <= 8) return launch_pairs<0, 4, 2, 2, 1, 0, true, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
-        if (nslot <= 12) return launch_pairs<0, 4, 2, 2, 1, 0, true, 3>(ctx, bp, ws, K, grid, w, cls, S);   // three (S = 24)
-        if (nslot <= 16) return launch_pairs<0, 4, 2, 2, 1, 0, true, 4>(ctx, bp, ws, K, grid, w, cls, S);   // four (S = 26 .. 32)
+        if (S == 8) return launch_pairs<8, 2, 4, 3, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);        // two half-warps, two pairs per lane
+        if (S == 16) return launch_pairs<16, 2, 4, 3, 1, 0, false, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);   // window split over two work items
+        if (S == 4) return launch_pairs<4, 1, 4, 4, 4>(ctx, strm, bp, ws, K, grid, w, cls, S);        // 8 pairs: 4 records per step
+        if (S == 12) return launch_pairs<12, 3, 2, 3, 1, 4, true>(ctx, strm, bp, ws, K, grid, w, cls, S);     // 4 rows per slot
+        if (nslot <= 1) return launch_pairs<0, 1, 4, 4, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 2) return launch_pairs<0, 2, 4, 3, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 3) return launch_pairs<0, 3, 2, 3, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 4) return launch_pairs<0, 4, 2, 2, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 6) return launch_pairs<0, 3, 2, 3, 1, 0, true, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);    // two work items of 3 slot sets
+        if (nslot <= 8) return launch_pairs<0, 4, 2, 2, 1, 0, true, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
+        if (nslot <= 12) return launch_pairs<0, 4, 2, 2, 1, 0, true, 3>(ctx, strm, bp, ws, K, grid, w, cls, S);   // three (S = 24)
+        if (nslot <= 16) return launch_pairs<0, 4, 2, 2, 1, 0, true, 4>(ctx, strm, bp, ws, K, grid, w, cls, S);   // four (S = 26 .. 32)
     }
     if (!F && !ctx->opt_no_pairs && ((uintptr_t)K & 15) == 0) {
         // fp64: one cell per lane-slot, S*S cells over 32 lanes
         const int nslot = (S * S + 31) / 32;
-        if (S == 8) return launch_cells<double, 8, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
-        if (S == 16) return launch_cells<double, 16, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);       // window split over two work items
-        if (S == 4) return launch_cells<double, 4, 1, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 2) return launch_cells<double, 0, 2, 4, 3>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 5) return launch_cells<double, 0, 5, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 8) return launch_cells<double, 0, 4, 2, 2, 2>(ctx, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
-        if (nslot <= 12) return launch_cells<double, 0, 4, 2, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 16) return launch_cells<double, 0, 4, 2, 2, 4>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 20) return launch_cells<double, 0, 4, 2, 2, 5>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 24) return launch_cells<double, 0, 4, 2, 2, 6>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 28) return launch_cells<double, 0, 4, 2, 2, 7>(ctx, bp, ws, K, grid, w, cls, S);
-        if (nslot <= 32) return launch_cells<double, 0, 4, 2, 2, 8>(ctx, bp, ws, K, grid, w, cls, S);    // S = 32: eight work items
+        if (S == 8) return launch_cells<double, 8, 2, 4, 3>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (S == 16) return launch_cells<double, 16, 4, 2, 2, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);       // window split over two work items
+        if (S == 4) return launch_cells<double, 4, 1, 4, 4>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 2) return launch_cells<double, 0, 2, 4, 3>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 5) return launch_cells<double, 0, 5, 2, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 8) return launch_cells<double, 0, 4, 2, 2, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);    // two work items of 4 slot sets
+        if (nslot <= 12) return launch_cells<double, 0, 4, 2, 2, 3>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 16) return launch_cells<double, 0, 4, 2, 2, 4>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 20) return launch_cells<double, 0, 4, 2, 2, 5>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 24) return launch_cells<double, 0, 4, 2, 2, 6>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 28) return launch_cells<double, 0, 4, 2, 2, 7>(ctx, strm, bp, ws, K, grid, w, cls, S);
+        if (nslot <= 32) return launch_cells<double, 0, 4, 2, 2, 8>(ctx, strm, bp, ws, K, grid, w, cls, S);    // S = 32: eight work items
     }
     if (F && !ctx->opt_no_pairs) {
         // fp32, odd support (the paper's own experiments use full support 9): one cell per lane-slot
         const int nslot = (S * S + 31) / 32;
-        if (nslot <= 2) return launch_cells<float, 0, 2, 4, 4>(ctx, bp, ws, K, grid, w, cls, S);            // S <= 7
-        if (nslot <= 4) return launch_cells<float, 0, 4, 2, 3>(ctx, bp, ws, K, grid, w, cls, S);            // S = 9, 11
-        if (nslot <= 8) return launch_cells<float, 0, 4, 2, 3, 2>(ctx, bp, ws, K, grid, w, cls, S);         // S = 13, 15
-        if (nslot <= 16) return launch_cells<float, 0, 4, 2, 3, 4>(ctx, bp, ws, K, grid, w, cls, S);        // S = 17 .. 21
-        if (nslot <= 32) return launch_cells<float, 0, 4, 2, 3, 8>(ctx, bp, ws, K, grid, w, cls, S);        // S = 23 .. 31
+        if (nslot <= 2) return launch_cells<float, 0, 2, 4, 4>(ctx, strm, bp, ws, K, grid, w, cls, S);            // S <= 7
+        if (nslot <= 4) return launch_cells<float, 0, 4, 2, 3>(ctx, strm, bp, ws, K, grid, w, cls, S);            // S = 9, 11
+        if (nslot <= 8) return launch_cells<float, 0, 4, 2, 3, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);         // S = 13, 15
+        if (nslot <= 16) return launch_cells<float, 0, 4, 2, 3, 4>(ctx, strm, bp, ws, K, grid, w, cls, S);        // S = 17 .. 21
+        if (nslot <= 32) return launch_cells<float, 0, 4, 2, 3, 8>(ctx, strm, bp, ws, K, grid, w, cls, S);        // S = 23 .. 31
     }
-    if (S == 8) return launch_runs<T, 8, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
-    if (S == 16) return launch_runs<T, 16, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
-    if (S == 4) return launch_runs<T, 4, 1, F ? 6 : 4>(ctx, bp, ws, K, grid, w, cls, S);
+    if (S == 8) return launch_runs<T, 8, 2, F ? 4 : 3>(ctx, strm, bp, ws, K, grid, w, cls, S);
+    if (S == 16) return launch_runs<T, 16, 8, F ? 2 : 1>(ctx, strm, bp, ws, K, grid, w, cls, S);
+    if (S == 4) return launch_runs<T, 4, 1, F ? 6 : 4>(ctx, strm, bp, ws, K, grid, w, cls, S);
     int nslot = (S * S + 31) / 32;
-    if (nslot <= 2) return launch_runs<T, 0, 2, F ? 4 : 3>(ctx, bp, ws, K, grid, w, cls, S);
-    if (nslot <= 5) return launch_runs<T, 0, 5, F ? 3 : 2>(ctx, bp, ws, K, grid, w, cls, S);
-    if (nslot <= 8) return launch_runs<T, 0, 8, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
-    if (nslot <= 18) return launch_runs<T, 0, 18, F ? 2 : 1>(ctx, bp, ws, K, grid, w, cls, S);
-    return launch_runs<T, 0, 32, 1>(ctx, bp, ws, K, grid, w, cls, S);
+    if (nslot <= 2) return launch_runs<T, 0, 2, F ? 4 : 3>(ctx, strm, bp, ws, K, grid, w, cls, S);
+    if (nslot <= 5) return launch_runs<T, 0, 5, F ? 3 : 2>(ctx, strm, bp, ws, K, grid, w, cls, S);
+    if (nslot <= 8) return launch_runs<T, 0, 8, F ? 2 : 1>(ctx, strm, bp, ws, K, grid, w, cls, S);
+    if (nslot <= 18) return launch_runs<T, 0, 18, F ? 2 : 1>(ctx, strm, bp, ws, K, grid, w, cls, S);
+    return launch_runs<T, 0, 32, 1>(ctx, strm, bp, ws, K, grid, w, cls, S);
 }
 
 }  // namespace
@@ -967,30 +967,40 @@ int wpg_launch_grid(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, cons
                     wpg_prec prec, const void *K, void *grid, char *w) {
     if (bp.nrow == 0) return WPG_OK;
     if (bp.ncls == 1) {
-        return prec == WPG_F32 ? launch_class<float>(ctx, bp, ws, K, grid, w, 0, tab.clsS[0])
-                               : launch_class<double>(ctx, bp, ws, K, grid, w, 0, tab.clsS[0]);
+        return prec == WPG_F32 ? launch_class<float>(ctx, ctx->stream, bp, ws, K, grid, w, 0, tab.clsS[0])
+                               : launch_class<double>(ctx, ctx->stream, bp, ws, K, grid, w, 0, tab.clsS[0]);
     }
     // Ragged stack: one launch per support class, independent of each other (they only meet in the grid's
     // reductions).  Most classes hold few visibilities and cannot fill the machine on their own, so the
     // launches are spread over the context's stream and three side streams, large supports first.
     cudaStream_t main_stream = ctx->stream;
-    if (!ctx->ev_fork) {
-        WPG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
-        for (int i = 0; i < 3; ++i) {
-            WPG_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->side[i], cudaStreamNonBlocking));
-            WPG_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming));
+    if (!ctx->side_ready) {             // all or nothing: a partial failure leaves no half-built set behind
+        cudaError_t e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+        for (int i = 0; i < 3 && e == cudaSuccess; ++i) {
+            e = cudaStreamCreateWithFlags(&ctx->side[i], cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join[i], cudaEventDisableTiming);
         }
+        if (e != cudaSuccess) {
+            for (int i = 0; i < 3; ++i) {
+                if (ctx->side[i]) cudaStreamDestroy(ctx->side[i]);
+                if (ctx->ev_join[i]) cudaEventDestroy(ctx->ev_join[i]);
+                ctx->side[i] = nullptr; ctx->ev_join[i] = nullptr;
+            }
+            if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+            ctx->ev_fork = nullptr;
+            return wpg_fail(ctx, WPG_ECUDA, "cannot create the side streams of the ragged-stack gridder: %s", cudaGetErrorString(e));
+        }
+        ctx->side_ready = true;
     }
     WPG_CUDA(ctx, cudaEventRecord(ctx->ev_fork, main_stream));
     for (int i = 0; i < 3; ++i) WPG_CUDA(ctx, cudaStreamWaitEvent(ctx->side[i], ctx->ev_fork, 0));
     int rc = WPG_OK;
     for (int cls = bp.ncls - 1; cls >= 0 && rc == WPG_OK; --cls) {
         const int S = tab.clsS[cls];
-        ctx->stream = cls % 4 == 0 ? main_stream : ctx->side[cls % 4 - 1];
-        rc = prec == WPG_F32 ? launch_class<float>(ctx, bp, ws, K, grid, w, cls, S)
-                             : launch_class<double>(ctx, bp, ws, K, grid, w, cls, S);
+        cudaStream_t strm = cls % 4 == 0 ? main_stream : ctx->side[cls % 4 - 1];
+        rc = prec == WPG_F32 ? launch_class<float>(ctx, strm, bp, ws, K, grid, w, cls, S)
+                             : launch_class<double>(ctx, strm, bp, ws, K, grid, w, cls, S);
     }
-    ctx->stream = main_stream;
     for (int i = 0; i < 3; ++i) {
         WPG_CUDA(ctx, cudaEventRecord(ctx->ev_join[i], ctx->side[i]));
         WPG_CUDA(ctx, cudaStreamWaitEvent(main_stream, ctx->ev_join[i], 0));

@@ -58,7 +58,7 @@ extern "C" int wpg_dirty_image(wpg_ctx *ctx, const void *d_grid, const wpg_kdesc
     size_t need = wpg_dirty_image_workspace_bytes(N, prec);
     if (!d_workspace || workspace_bytes < need)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, need);
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     if (ctx->plan_N != N || ctx->plan_prec != (int)prec) {
         if (ctx->plan) { cufftDestroy(ctx->plan); ctx->plan = 0; ctx->plan_N = 0; }
         cufftResult r = cufftPlan2d(&ctx->plan, N, N, prec == WPG_F32 ? CUFFT_C2C : CUFFT_Z2Z);

@@ -83,7 +83,7 @@ extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, s
     if (!ctx || !h_out || !d_buf) return WPG_EINVAL;
     if (which < 0 || which > 4 || iters < 1 || buf_bytes < ((size_t)1 << 20))
         return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which 0..4, iters >= 1, buffer >= 1 MiB");
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     size_t ncell = 1;
     while (ncell * 2 * sizeof(float2) <= buf_bytes) ncell *= 2;
     if (which == 2 && buf_bytes < ((size_t)16 << 20)) return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which = 2 needs a 16 MiB buffer");

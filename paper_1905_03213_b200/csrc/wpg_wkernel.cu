@@ -218,7 +218,7 @@ extern "C" int wpg_wkernel_build(wpg_ctx *ctx, const wpg_kdesc *desc, wpg_prec p
     if (rc) return rc;
     if (!d_out) return wpg_fail(ctx, WPG_EINVAL, "output pointer is NULL");
     if (prec != WPG_F32 && prec != WPG_F64) return wpg_fail(ctx, WPG_EINVAL, "bad precision");
-    WPG_CUDA(ctx, cudaSetDevice(ctx->device));
+    WPG_DEVICE(ctx);
     const int Nw = desc->Nw, Q = desc->oversample;
     const double fov = (double)desc->grid_N * desc->cell, dw = 2.0 * desc->w_max / Nw;
     std::map<int, std::vector<int>> groups;                 // support -> planes

@@ -219,26 +219,53 @@ def ska_low_layout(rng):
     return E, Nn
 
 
+def _fill_vis_blocks(seed, uvw, freq, src, device, noise=True, block_rows=1 << 20):
+    """vis[row][chan] = O1 model + noise, generated in row blocks with the noise drawn row-major from its own
+    stream, so that the first k rows of a workload are the same whatever the total row count (a prefix of the
+    workload can be generated on its own)."""
+    nrow, nchan = uvw.shape[0], freq.size
+    vis = np.empty((nrow, nchan), dtype=np.complex64)
+    f = freq / C0
+    nrng = np.random.default_rng([seed, 7])
+    for r0 in range(0, nrow, block_rows):
+        blk = uvw[r0:r0 + block_rows]
+        v = predict_vis(blk[:, 0:1] * f[None, :], blk[:, 1:2] * f[None, :], blk[:, 2:3] * f[None, :],
+                        src["flux"], src["l"], src["m"], device=device)
+        if noise:
+            nz = nrng.normal(0.0, 0.1, (blk.shape[0], nchan, 2))        # R16: sigma 0.1 on re and im
+            v = v + (nz[..., 0] + 1j * nz[..., 1])
+        vis[r0:r0 + block_rows] = v.astype(np.complex64)
+    return vis
+
+
 def config4(n_dump=360, nchan=8, seed=SEED0 + 4, device=None, max_rows=None, noise=True,
-            values="model"):
+            values="model", prefix_rows=None):
     """SKA1-low-like: 512 stations, 130 816 baselines x n_dump x nchan (150-160 MHz),
     N=8192, Nw=128, ragged support 8..32 (rule K6), Q=8, fp32.
-    values="model": 50 sources + noise; values="random": N(0,1) (same throughput, cheap)."""
+    values="model": 50 sources + noise; values="random": N(0,1) (same throughput, cheap).
+    prefix_rows: keep only the first rows of the workload (cell, w_max and every value are those of the full
+    n_dump workload: a bounded sample of the same workload for the CPU legs)."""
     rng = np.random.default_rng(seed)
     E, Nn = ska_low_layout(rng)
     uvw = earth_rotation_uvw(E, Nn, n_dump, max_rows=max_rows)
     freq = np.linspace(150e6, 160e6, nchan)
     cell, w_max = _cell_and_wmax(uvw, freq)
+    if prefix_rows is not None:
+        uvw = np.ascontiguousarray(uvw[:prefix_rows])
     N, Nw = 8192, 128
     src = _sources(rng, 50, 0.3 * N * cell)
     if values == "model":
-        vis = _fill_vis(rng, uvw, freq, src, device, noise)
+        vis = _fill_vis_blocks(seed, uvw, freq, src, device, noise)
     else:
         vis = np.empty((uvw.shape[0], nchan), np.complex64)
-        vis.real[...] = rng.standard_normal(vis.shape, dtype=np.float32)
-        vis.imag[...] = rng.standard_normal(vis.shape, dtype=np.float32)
+        for part, sub in ((vis.real, 1), (vis.imag, 2)):
+            prng = np.random.default_rng([seed, sub])
+            for r0 in range(0, uvw.shape[0], 1 << 22):
+                part[r0:r0 + (1 << 22)] = prng.standard_normal((min(1 << 22, uvw.shape[0] - r0), nchan), dtype=np.float32)
     return Workload("config4", uvw, freq, vis, np.ones(vis.shape, np.float32),
-                    N, cell, Nw, w_max, ("ragged", 8, 32), 8, src, notes={"row_block": E.size * (E.size - 1) // 2, "n_ant": int(E.size)})
+                    N, cell, Nw, w_max, ("ragged", 8, 32), 8, src,
+                    notes={"row_block": E.size * (E.size - 1) // 2, "n_ant": int(E.size), "n_dump": int(n_dump),
+                           "full_rows": int(n_dump * (E.size * (E.size - 1) // 2)) if max_rows is None else int(max_rows)})
 
 
 def config5(nvis=100_000_000, seed=SEED0 + 5, device=None, n_dump=3064, noise=True):

@@ -241,6 +241,25 @@ class Context:
         assert vis.numel() == nrow * nchan and weight.numel() == nrow * nchan and uvw.shape[1] == 3
         return nrow, nchan
 
+    def _check_grid(self, grid, stack, lead=()):
+        """A caller-supplied grid goes to the C ABI as a raw pointer: refuse anything but a contiguous device
+        tensor of the stack's precision and shape."""
+        t = self.torch
+        N = stack.desc.grid_N
+        want = t.complex64 if stack.prec == F32 else t.complex128
+        if not (grid.is_cuda and grid.device == self.device and grid.is_contiguous()
+                and grid.dtype == want and tuple(grid.shape) == tuple(lead) + (N, N)):
+            raise WpgError(EINVAL, "grid must be a contiguous %s tensor of shape %s on %s (got %s %s on %s)"
+                           % (want, tuple(lead) + (N, N), self.device, grid.dtype, tuple(grid.shape), grid.device))
+
+    def _temp(self, nbytes):
+        """Temporary workspace, allocated on the context's stream (torch's caching allocator ties a block to the
+        stream it was allocated on: a block from another stream could be handed out again while the library's
+        kernels are still queued)."""
+        t = self.torch
+        with t.cuda.stream(self.stream):
+            return t.empty(int(nbytes), dtype=t.uint8, device=self.device)
+
     def new_grid(self, stack):
         t = self.torch
         N = stack.desc.grid_N
@@ -252,8 +271,9 @@ class Context:
         nrow, nchan = self._inputs(vis, uvw, weight, freq)
         if grid is None:
             grid = self.new_grid(stack)
+        self._check_grid(grid, stack)
         if workspace is None:
-            workspace = t.empty(self.grid_workspace_bytes(nrow, nchan, stack), dtype=t.uint8, device=self.device)
+            workspace = self._temp(self.grid_workspace_bytes(nrow, nchan, stack))
         st = Stats()
         self._check(self.lib.wpg_grid(self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(),
                                       nrow, nchan, stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec,
@@ -265,6 +285,7 @@ class Context:
         nrow, nchan = self._inputs(vis, uvw, weight, freq)
         if grid is None:
             grid = self.new_grid(stack)
+        self._check_grid(grid, stack)
         st = Stats()
         self._check(self.lib.wpg_grid_naive(self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(),
                                             freq.data_ptr(), nrow, nchan, stack.data.data_ptr(),
@@ -279,8 +300,25 @@ class Context:
             return x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data
         nrow, nchan = int(uvw.shape[0]), int(freq.shape[0])
         N = stack.desc.grid_N
+        cdt = np.complex64 if stack.prec == F32 else np.complex128
         if out is None:
-            out = np.empty((N, N), dtype=np.complex64 if stack.prec == F32 else np.complex128)
+            out = np.empty((N, N), dtype=cdt)
+
+        def host_ok(x, dtype, size):
+            """C-contiguous host array (numpy or CPU torch) of the given element type and size"""
+            if hasattr(x, "data_ptr"):
+                return (not x.is_cuda) and x.is_contiguous() and x.numel() == size and \
+                    np.dtype(str(x.dtype).replace("torch.", "")) == np.dtype(dtype)
+            return isinstance(x, np.ndarray) and x.flags.c_contiguous and x.size == size and x.dtype == np.dtype(dtype)
+
+        checks = [(vis, np.complex64, nrow * nchan, "vis"), (uvw, np.float64, nrow * 3, "uvw"),
+                  (weight, np.float32, nrow * nchan, "weight"), (freq, np.float64, nchan, "freq"), (out, cdt, N * N, "out")]
+        if image_out is not None:
+            checks.append((image_out, np.float32 if stack.prec == F32 else np.float64, N * N, "image_out"))
+        for x, dtype, size, name in checks:
+            if not host_ok(x, dtype, size):
+                raise WpgError(EINVAL, "grid_host: %s must be a C-contiguous host array of %d %s elements"
+                               % (name, size, np.dtype(dtype).name))
         st = Stats()
         self._check(self.lib.wpg_grid_host(self.h, ptr(vis), ptr(uvw), ptr(weight), ptr(freq), nrow, nchan,
                                            stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec,
@@ -298,7 +336,7 @@ class Context:
         bstart = t.empty(nb + 1, dtype=t.int32, device=self.device)
         perm = t.empty(max(nrow, 1), dtype=t.int32, device=self.device)
         need = int(self.lib.wpg_baseline_workspace_bytes(nrow, 1, n_ant, F32))
-        ws = t.empty(need, dtype=t.uint8, device=self.device)
+        ws = self._temp(need)
         self._check(self.lib.wpg_baseline_reorder(self.h, ant1.data_ptr(), ant2.data_ptr(), n_ant, nrow,
                                                   bstart.data_ptr(), perm.data_ptr(), ws.data_ptr(), ws.numel()))
         return bstart, perm[:nrow]
@@ -310,9 +348,9 @@ class Context:
         assert ant1.dtype == t.int32 and ant2.dtype == t.int32 and ant1.numel() == nrow and ant2.numel() == nrow
         if grid is None:
             grid = self.new_grid(stack)
+        self._check_grid(grid, stack)
         if workspace is None:
-            need = int(self.lib.wpg_baseline_workspace_bytes(nrow, nchan, n_ant, stack.prec))
-            workspace = t.empty(need, dtype=t.uint8, device=self.device)
+            workspace = self._temp(self.lib.wpg_baseline_workspace_bytes(nrow, nchan, n_ant, stack.prec))
         st = Stats()
         self._check(self.lib.wpg_grid_baseline_order(
             self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(), ant1.data_ptr(), ant2.data_ptr(),
@@ -334,7 +372,8 @@ class Context:
             need = int(self.lib.wpg_grid_pol_workspace_bytes(self.h, nrow, nchan, npol, ctypes.byref(stack.desc)))
             if need == 0:
                 raise WpgError(EINVAL, "wpg_grid_pol_workspace_bytes: bad arguments (npol 2|4, uniform support 8|16)")
-            workspace = t.empty(need, dtype=t.uint8, device=self.device)
+            workspace = self._temp(need)
+        self._check_grid(grid, stack, lead=(npol,))
         st = Stats()
         self._check(self.lib.wpg_grid_pol(self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(),
                                           nrow, nchan, npol, stack.data.data_ptr(), ctypes.byref(stack.desc),
@@ -353,7 +392,7 @@ class Context:
         nrow, nchan = uvw.shape[0], freq.shape[0]
         if out is None:
             out = t.empty((nrow, nchan), dtype=cdt, device=self.device)
-        ws = t.empty(int(self.lib.wpg_degrid_workspace_bytes(nchan)), dtype=t.uint8, device=self.device)
+        ws = self._temp(self.lib.wpg_degrid_workspace_bytes(nchan))
         c2 = (ctypes.c_int64 * 2)()
         self._check(self.lib.wpg_degrid(self.h, grid.data_ptr(), uvw.data_ptr(), freq.data_ptr(), nrow, nchan,
                                         stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec, out.data_ptr(),
@@ -365,7 +404,7 @@ class Context:
         t = self.torch
         nrow, nchan = self._inputs(vis, uvw, weight, freq)
         if workspace is None:
-            workspace = t.empty(self.grid_workspace_bytes(nrow, nchan, stack), dtype=t.uint8, device=self.device)
+            workspace = self._temp(self.grid_workspace_bytes(nrow, nchan, stack))
         info, st = BinInfo(), Stats()
         self._check(self.lib.wpg_bin(self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(),
                                      nrow, nchan, ctypes.byref(stack.desc), stack.prec, workspace.data_ptr(),
@@ -379,7 +418,7 @@ class Context:
         assert grid.is_cuda and grid.is_contiguous() and grid.shape == (N, N)
         need = int(self.lib.wpg_dirty_image_workspace_bytes(N, stack.prec))
         if workspace is None:
-            workspace = t.empty(need, dtype=t.uint8, device=self.device)
+            workspace = self._temp(need)
         img = t.empty((N, N), dtype=t.float32 if stack.prec == F32 else t.float64, device=self.device)
         self._check(self.lib.wpg_dirty_image(self.h, grid.data_ptr(), ctypes.byref(stack.desc), float(weight_sum),
                                              stack.prec, img.data_ptr(), workspace.data_ptr(), workspace.numel()))

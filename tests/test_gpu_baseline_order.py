@@ -94,6 +94,32 @@ def test_grid_in_baseline_order_matches_oracle(ctx):
         assert s == rstats
         err = float(np.max(np.abs(g.cpu().numpy() - ref)) / np.max(np.abs(ref)))
         assert err <= TOL[prec], (prec, err)
+    # NaN / Inf values under zero weight (RFI-flagged samples) and in samples off the grid: skipped
+    # outright by the oracle and by wpg_grid, and they must not leak through the zero-valued place-holder records
+    vis_bad = vis.copy()
+    flagged = wt == 0.0
+    vis_bad[flagged] = np.complex64(complex(np.nan, np.inf))
+    fscale = freq / synth.C0
+    off_grid = np.zeros_like(flagged)
+    for c in range(nchan):
+        for k in range(nrow):
+            j0u, _ = ogrid.index_map(uvw[k, 0] * fscale[c], N, cell, S, Q)
+            j0v, _ = ogrid.index_map(uvw[k, 1] * fscale[c], N, cell, S, Q)
+            off_grid[k, c] = j0u < 0 or j0v < 0 or j0u + S > N or j0v + S > N
+    assert off_grid.sum() == rstats["n_skipped_oob"] + (off_grid & flagged).sum()
+    vis_bad[off_grid] = np.complex64(complex(-np.inf, np.nan))
+    ref_bad, rstats_bad = ogrid.grid(uvw, vis_bad, wt, freq, st)
+    assert rstats_bad == rstats and np.array_equal(ref_bad, ref)
+    d_bad = [torch.from_numpy(vis_bad).cuda()] + d[1:]
+    for prec in (wpgrid.F32, wpgrid.F64):
+        ks = ctx.stack_from_host(st.data, Nw, w_max, S, Q, N, cell, prec)
+        g, s = ctx.grid_baseline_order(*d_bad, n_ant, ks, stats=True)
+        g2, s2 = ctx.grid(*d_bad[:4], ks, stats=True)
+        assert s == rstats and s2 == rstats
+        for gg in (g, g2):
+            gh = gg.cpu().numpy()
+            assert np.isfinite(gh).all()
+            assert float(np.max(np.abs(gh - ref)) / np.max(np.abs(ref))) <= TOL[prec]
     # ragged stacks are refused
     sup = np.array([8, 8, 10, 10, 12, 12, 8, 8], np.int32)
     ks = ctx.wkernel_build(Nw, w_max, sup, Q, N, cell, wpgrid.F32)

@@ -37,6 +37,15 @@ def oracle_stack(wl):
     return owk.build_stack(wl.Nw, wl.w_max, sup, wl.oversample, wl.grid_N, wl.cell)
 
 
+def classes_exercised(wl, st):
+    """{support: number of visibilities whose plane has that support} (which gridder instantiations a ragged stack
+    reaches; w -> plane as in G2, used only for this coverage assertion)."""
+    w = (wl.uvw[:, 2:3] * (wl.freq / synth.C0)[None, :]).ravel()
+    p = np.clip(np.floor((w + wl.w_max) / (2.0 * wl.w_max / wl.Nw)), 0, wl.Nw - 1).astype(np.int64)
+    cls, cnt = np.unique(st.support[p], return_counts=True)
+    return dict(zip(cls.tolist(), cnt.tolist()))
+
+
 def upload(ctx, st, prec):
     sup = int(st.support[0]) if st.uniform else st.support
     return ctx.stack_from_host(st.data, st.Nw, st.w_max, sup, st.oversample, st.grid_N, st.cell, prec)
@@ -92,10 +101,10 @@ def test_config1_end_to_end_image(ctx, cfg1):
     d = dev(wl)
     wsum = float(wl.weight.sum())
     ref_img = oimage.dirty_image(ref, wl.cell, wsum)
-    for prec, tol in ((wpgrid.F32, 1e-4), (wpgrid.F64, 1e-9)):
+    for prec, tol in ((wpgrid.F32, 1e-4), (wpgrid.F64, 1e-10)):           # north_star's bounds, end to end
         ks = ctx.wkernel_build(wl.Nw, wl.w_max, wl.support, wl.oversample, wl.grid_N, wl.cell, prec)
         g, _ = ctx.grid(*d, ks)
-        assert relerr(g.cpu().numpy(), ref) <= (2e-4 if prec == wpgrid.F32 else 1e-9)
+        assert relerr(g.cpu().numpy(), ref) <= tol
         img = ctx.dirty_image(g, ks, wsum).cpu().numpy().astype(np.float64)
         assert np.max(np.abs(img - ref_img)) <= tol * np.max(np.abs(ref_img))
         # the image step alone, fed the oracle's grid
@@ -240,7 +249,8 @@ def test_config4_ragged_scaled(ctx):
     """SKA-low-like layout, ragged support 8..32, 8 channels, N = 8192; 2 dumps (2.1e6 visibilities)."""
     wl = synth.config4(n_dump=2, values="random")
     st = oracle_stack(wl)
-    assert st.support.min() >= 8 and len(set(st.support.tolist())) >= 4
+    # the support classes this input sends visibilities to (each is one gridder launch of its own instantiation)
+    assert sorted(classes_exercised(wl, st)) == [8, 10, 12, 14, 16, 18]
     ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
     sup, off = wpgrid.ragged_support(wl.Nw, wl.w_max, wl.grid_N, wl.cell, wl.oversample, 8, 32)
     assert np.array_equal(sup, st.support) and np.array_equal(off, st.plane_offset)
@@ -293,7 +303,9 @@ def test_config2_full_size_as_benchmarked(ctx):
     wsum = float(wl.weight.sum())
     img = ctx.dirty_image(g, ks, wsum).cpu().numpy().astype(np.float64)
     ref_img = oimage.dirty_image(ref, wl.cell, wsum)
-    assert np.max(np.abs(img - ref_img)) <= 2e-4 * np.max(np.abs(ref_img))
+    ierr = float(np.max(np.abs(img - ref_img)) / np.max(np.abs(ref_img)))
+    print("config2 full size fp32 dirty image relerr %.3e" % ierr)
+    assert ierr <= 1e-4
 
 
 def test_config5_1e7_both_precisions_full_grid(ctx):
@@ -381,7 +393,7 @@ def test_ragged_stack_key_budgets_both_precisions(ctx):
     wl = synth.config4(n_dump=1, nchan=2, values="random")
     st = oracle_stack(wl)
     ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
-    assert len(set(st.support.tolist())) >= 4
+    assert sorted(classes_exercised(wl, st)) == [8, 10, 12, 14, 16, 18]
     check_all_paths(ctx, wl, st, ref, rstats, key_bits=(0, 8, 20, 27))
 
 
