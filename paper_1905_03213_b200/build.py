@@ -29,15 +29,30 @@ def stale():
 
 
 def build(force=False, verbose=False):
+    """One nvcc -c per source, in parallel, objects cached under build/ (git-ignored), then one link."""
     if not force and not stale():
         return LIB
-    tmp = LIB + ".%d.tmp" % os.getpid()
-    cmd = [NVCC, "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-           "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall", "-shared", "-I", INCLUDE,
-           "-o", tmp] + sources() + ["-lcufft", "-Xlinker", "-rpath,/usr/local/cuda/lib64"]
+    from concurrent.futures import ThreadPoolExecutor
+    objdir = os.path.join(HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    headers = glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(INCLUDE, "*.h"))
+    newest_header = max(os.path.getmtime(h) for h in headers)
+    flags = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+             "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall", "-I", INCLUDE]
     if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-    subprocess.check_call(cmd)
+        flags.insert(0, "-Xptxas=-v")
+
+    def compile_one(src):
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        if force or verbose or not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(src), newest_header):
+            subprocess.check_call([NVCC] + flags + ["-c", src, "-o", obj])
+        return obj
+
+    with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
+        objs = list(ex.map(compile_one, sources()))
+    tmp = LIB + ".%d.tmp" % os.getpid()
+    subprocess.check_call([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs +
+                          ["-lcufft", "-Xlinker", "-rpath,/usr/local/cuda/lib64"])
     os.replace(tmp, LIB)
     return LIB
 

@@ -72,6 +72,7 @@ extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
     else if (!strcmp(name, "key_bits")) { if (value != 0 && (value < 8 || value > 28)) return wpg_fail(ctx, WPG_EINVAL, "key_bits must be 0 or 8..28"); ctx->opt_key_bits = (int)value; }
     else if (!strcmp(name, "timing")) { ctx->opt_timing = value != 0; }
     else if (!strcmp(name, "no_pairs")) { ctx->opt_no_pairs = value != 0; }
+    else if (!strcmp(name, "compress")) { ctx->opt_compress = value != 0; }
     else if (!strcmp(name, "row_block")) { if (value < 0) return wpg_fail(ctx, WPG_EINVAL, "row_block must be >= 0"); ctx->opt_row_block = value; }
     else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
     return WPG_OK;
@@ -149,6 +150,8 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     bp->qshift = -1;
     for (int sft = 0; sft < 7; ++sft) if ((1 << sft) == d->oversample) bp->qshift = sft;
     bp->ncls = (int)distinct.size();
+    bp->compress = ctx->opt_compress;
+    bp->S0 = distinct[0];
     // sort key = (class, j0u, j0v >> kshift): the visibilities are swept column by column of window starts,
     // down the v axis, so a window that moves on leaves whole grid-row segments behind (contiguous write-outs)
     // and keeps its column ownership (the parity of j0u is fixed within a sweep); full resolution unless the

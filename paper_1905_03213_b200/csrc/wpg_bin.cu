@@ -13,17 +13,20 @@ namespace {
 
 constexpr int kScanBlock = 4096;   // keys per scan block (1024 threads x 4)
 
-// Block totals of the five wpg_stats counters: warp sums, shared memory, one reduction per counter and block.
-__device__ __forceinline__ void block_count(Counters *ctr, unsigned c_grid, unsigned c_oob, unsigned c_zero,
-                                            unsigned c_clamp, unsigned c_upd) {
+// Block totals of the wpg_stats counters.  The four per-visibility flags travel as 8-bit fields of one word (a
+// warp holds 32 * kVpt = 128 visibilities), the update count on its own: two warp reductions per block.
+constexpr unsigned kFlagGridded = 1u, kFlagOob = 1u << 8, kFlagZero = 1u << 16, kFlagClamped = 1u << 24;
+__device__ __forceinline__ void block_count(Counters *ctr, unsigned flags, unsigned c_upd) {
     __shared__ unsigned s_cnt[5];
     if (threadIdx.x < 5) s_cnt[threadIdx.x] = 0;
     __syncthreads();
-    unsigned v[5] = {c_grid, c_oob, c_zero, c_clamp, c_upd};
-#pragma unroll
-    for (int k = 0; k < 5; ++k) {
-        const unsigned t = __reduce_add_sync(0xffffffffu, v[k]);
-        if ((threadIdx.x & 31) == 0 && t) atomicAdd(&s_cnt[k], t);
+    const unsigned f = __reduce_add_sync(0xffffffffu, flags), u = __reduce_add_sync(0xffffffffu, c_upd);
+    if ((threadIdx.x & 31) == 0) {
+        if (f & 0xFFu) atomicAdd(&s_cnt[0], f & 0xFFu);
+        if ((f >> 8) & 0xFFu) atomicAdd(&s_cnt[1], (f >> 8) & 0xFFu);
+        if ((f >> 16) & 0xFFu) atomicAdd(&s_cnt[2], (f >> 16) & 0xFFu);
+        if (f >> 24) atomicAdd(&s_cnt[3], f >> 24);
+        if (u) atomicAdd(&s_cnt[4], u);
     }
     __syncthreads();
     if (threadIdx.x < 5 && s_cnt[threadIdx.x]) {
@@ -52,7 +55,9 @@ __global__ void chan_scale_kernel(const double *__restrict__ freq, int nchan, do
 }
 
 // Ragged stacks, pass 0b: census of the support classes (w -> plane -> class; weights and grid edges are
-// ignored — the census only steers the key resolution).  One thread per row, all channels.
+// ignored — the census only steers the key resolution, the result of the binning does not depend on it, so every
+// kCensusStride-th row is enough).  One thread per sampled row, all channels.
+constexpr int kCensusStride = 16;
 __global__ void __launch_bounds__(256)
 census_kernel(const double *__restrict__ uvw, const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
               const __grid_constant__ BinParams P, Counters *__restrict__ ctr) {
@@ -62,7 +67,8 @@ census_kernel(const double *__restrict__ uvw, const double *__restrict__ fscale,
     wpg_stage_planetab(s_tab, T, P.Nw);
     __syncthreads();
     unsigned *mine = s_cnt[threadIdx.x >> 5];
-    for (long long row = (long long)blockIdx.x * 256 + threadIdx.x; row < P.nrow; row += (long long)gridDim.x * 256) {
+    const long long stride = P.nrow >= 65536 ? kCensusStride : 1;
+    for (long long row = ((long long)blockIdx.x * 256 + threadIdx.x) * stride; row < P.nrow; row += (long long)gridDim.x * 256 * stride) {
         const double wm = __ldg(uvw + 3 * row + 2);
         for (int ch = 0; ch < P.nchan; ++ch) {
             const double w = __dmul_rn(wm, __ldg(fscale + ch));
@@ -71,7 +77,7 @@ census_kernel(const double *__restrict__ uvw, const double *__restrict__ fscale,
                 const double fp = floor(wpg_div_const(__dadd_rn(w, P.w_max), P.dw, P.rdw));
                 p = fp < 0.0 ? 0 : (fp > (double)(P.Nw - 1) ? P.Nw - 1 : (int)fp);
             }
-            atomicAdd(&mine[s_tab[p].y >> 8], 1u);
+            atomicAdd(&mine[s_tab[p].y >> 8], (unsigned)stride);
         }
     }
     __syncthreads();
@@ -115,117 +121,192 @@ __global__ void plan_keys_kernel(Counters *__restrict__ ctr, int ncls, int N, un
 constexpr int kVpt = 4;            // visibilities per thread: four independent atomics in flight per thread
 
 // The kVpt visibilities of a thread.  Default: a block takes 256 * kVpt consecutive visibilities, thread t the
-// ones at t, t + 256, ...  With the "row_block" hint (P.vis_block = visibilities per time step): thread
-// (dg, x) takes visibility x of the time steps dg * kVpt + j — the same baseline and channel at consecutive
-// times, whose window starts (and so sort keys) mostly coincide, so that the bucket counter is
-// touched once per run of equal keys.  Loads stay coalesced either way (consecutive lanes, consecutive x).
-__device__ __forceinline__ void vis_indices(const BinParams &P, unsigned (&idx)[kVpt]) {
-    const unsigned long long nvis = (unsigned long long)(P.nrow * P.nchan);     // < 2^32 - 1 (wpg_make_plan)
+// ones at t, t + 256, ...  With the "row_block" hint (P.vis_block = visibilities per time step; the blocks of a group
+// of kVpt time steps are consecutive): thread x of group dg takes visibility x of the time steps dg * kVpt + j — the same baseline and
+// channel at consecutive times, whose window starts (and so sort keys) mostly coincide, so that the
+// bucket counter is touched once per run of equal keys, and equal records are merged (compression).  Loads stay
+// coalesced either way (consecutive lanes, consecutive x).  idx = 0xFFFFFFFF: no visibility.
+struct VisIdx { unsigned i[kVpt], row[kVpt]; int ch[kVpt]; };
+__device__ __forceinline__ VisIdx vis_indices(const BinParams &P) {
+    VisIdx V;
+    const unsigned nvis = (unsigned)(P.nrow * P.nchan);             // < 2^32 - 2 (wpg_make_plan)
     if (P.vis_block) {
-        const unsigned t = blockIdx.x * 256u + threadIdx.x;
-        const unsigned dg = t / P.vis_block, x = t - dg * P.vis_block;
+        const unsigned nbx = (P.vis_block + 255u) / 256u, dg = blockIdx.x / nbx;      // (uniform: one division per block)
+        const unsigned x = (blockIdx.x - dg * nbx) * 256u + threadIdx.x;
+        const unsigned xr = P.nchan > 1 ? x / (unsigned)P.nchan : x;      // one division per thread, not per visibility
+        const int ch = (int)(x - xr * (unsigned)P.nchan);
+        const unsigned rows_per_step = P.vis_block / (unsigned)P.nchan;
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) {
-            const unsigned long long i = (unsigned long long)(dg * kVpt + j) * P.vis_block + x;
-            idx[j] = i < nvis ? (unsigned)i : 0xFFFFFFFFu;
+            const unsigned long long step = (unsigned long long)dg * kVpt + j;
+            const unsigned long long i = step * P.vis_block + x;
+            const bool ok = x < P.vis_block && i < nvis;
+            V.i[j] = ok ? (unsigned)i : 0xFFFFFFFFu;
+            V.row[j] = (unsigned)(step * rows_per_step) + xr;
+            V.ch[j] = ch;
         }
     } else {
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) {
             const unsigned long long i = (unsigned long long)blockIdx.x * (256 * kVpt) + j * 256 + threadIdx.x;
-            idx[j] = i < nvis ? (unsigned)i : 0xFFFFFFFFu;
+            const bool ok = i < nvis;
+            V.i[j] = ok ? (unsigned)i : 0xFFFFFFFFu;
+            const unsigned r = P.nchan > 1 ? (unsigned)i / (unsigned)P.nchan : (unsigned)i;
+            V.row[j] = r; V.ch[j] = (int)((unsigned)i - r * (unsigned)P.nchan);
         }
     }
+    return V;
 }
-// run structure of a thread's keys: head[j] = first of a run of equal valid keys, len[j] = length of the run from j
-__device__ __forceinline__ void key_runs(const unsigned (&key)[kVpt], bool (&head)[kVpt], unsigned (&len)[kVpt]) {
+
+// Run structure of a thread's visibilities.  head[j]: first of a run of equal valid keys; rhead[j]: starts a
+// record — with record compression ("compression": samples that fall on the
+// same point are merged before gridding) a visibility whose window start AND coefficient slice equal its
+// predecessor's is summed into the predecessor's record instead of getting its own; nrec[j]: records in the key
+// run that starts at j.  Without compression every valid visibility is its own record.
+__device__ __forceinline__ void key_runs(const unsigned (&key)[kVpt], const unsigned (&pos)[kVpt], const unsigned (&koff)[kVpt],
+                                         bool compress, bool (&head)[kVpt], bool (&rhead)[kVpt], unsigned (&nrec)[kVpt]) {
 #pragma unroll
-    for (int j = kVpt - 1; j >= 0; --j) {
-        len[j] = 1u + ((j + 1 < kVpt && key[j + 1] == key[j]) ? len[j + 1 < kVpt ? j + 1 : j] : 0u);
-        head[j] = key[j] != WPG_NO_KEY && (j == 0 || key[j] != key[j - 1]);
+    for (int j = 0; j < kVpt; ++j) {
+        const bool valid = key[j] != WPG_NO_KEY;
+        const bool same_key = j > 0 && key[j] == key[j - 1];
+        head[j] = valid && !same_key;
+        rhead[j] = valid && !(compress && same_key && pos[j] == pos[j > 0 ? j - 1 : 0] && koff[j] == koff[j > 0 ? j - 1 : 0]);
     }
+#pragma unroll
+    for (int j = kVpt - 1; j >= 0; --j)
+        nrec[j] = (rhead[j] ? 1u : 0u) + ((j + 1 < kVpt && key[j + 1] == key[j]) ? nrec[j + 1 < kVpt ? j + 1 : j] : 0u);
 }
 
-// Position math (fp64, G1-G3) and validity (G4, R9) of visibility i; returns the sort key or WPG_NO_KEY.
-// The two passes below both evaluate it: recomputing is cheaper than a round trip of (key, position,
-// coefficient offset) through HBM, and the workspace holds nothing per visibility but the records.
-struct Located { unsigned key, pos, koff; int S; bool clamped, zero_weight; };
-struct RawVis { double um, vm, wm, f; float wt; bool valid; };
+// ---------------------------------------------------------------------------------------------
+// Position math (fp64, G1-G3) and validity (G4, R9).  Both passes evaluate it: recomputing is cheaper than a round
+// trip of (key, position, coefficient offset) through HBM (measured in round 2: an 8-byte intermediate per visibility
+// made the pair of passes slower on every workload), and the workspace holds nothing per visibility but the records.
+//
+// The fast path is straight-line code: quotients by Markstein's sequence (wpg_div_const), floor() through the
+// 2^52 + 2^51 rounding constant instead of the conversion pipe, and ONE flag that says whether any of the three
+// values whose floor is taken lies within 1e-6 of an integer (or outside the range where the trick is valid).  Only
+// then — a few visibilities in a million — the written form with IEEE divisions is evaluated out of line
+// (wpg_locate), so that G6 holds whatever the constant-divisor sequence does in its last bit.
+struct RawVis { double um, vm, wm, f; float wt; };
+struct Located { unsigned key, pos, koff; int S; bool clamped; };
 
-// All global loads of one visibility, issued before any arithmetic so that a thread has the inputs of
-// its kVpt visibilities in flight at once (the passes are latency-bound otherwise).
-__device__ __forceinline__ RawVis load_vis(long long i, long long nvis, const double *__restrict__ uvw,
-                                           const float *__restrict__ weight, const double *__restrict__ fscale,
-                                           const BinParams &P) {
-    RawVis r; r.valid = i < nvis; r.um = r.vm = r.wm = 0.0; r.f = 0.0; r.wt = 0.f;
-    if (r.valid) {
-        long long row = i; int ch = 0;
-        if (P.nchan > 1) {             // nrow * nchan < 2^32 (wpg_make_plan): 32-bit division
-            const unsigned r32 = (unsigned)i / (unsigned)P.nchan;
-            row = r32; ch = (int)((unsigned)i - r32 * (unsigned)P.nchan);
-        }
-        r.wt = __ldg(weight + i);
-        r.um = __ldg(uvw + 3 * row); r.vm = __ldg(uvw + 3 * row + 1); r.wm = __ldg(uvw + 3 * row + 2);
-        r.f = __ldg(fscale + ch);
-    }
-    return r;
-}
-// Keeps the compiler from consuming a loaded value (and so waiting for it) before the loads that
-// follow in program order have been issued.
-__device__ __forceinline__ void use_after_here(RawVis &r) {
-    asm volatile("" : "+f"(r.wt), "+d"(r.um), "+d"(r.vm), "+d"(r.wm));
+__device__ __forceinline__ int floor_magic(double t, double lim, bool &risk) {
+    // |t| < lim <= 2^30: t + M holds rint(t) in its low word; t - rint(t) is exact.  One ulp of t is below 2.4e-7 there.
+    // Outside the range (also NaN) the flag is raised and the value returned is not used.
+    const double M = 6755399441055744.0;
+    const double tm = __dadd_rn(t, M);
+    const double d = __dadd_rn(t, -__dadd_rn(tm, -M));           // in [-0.5, 0.5]
+    risk |= !(fabs(d) >= 1e-6) | !(fabs(t) < lim);
+    return __double2loint(tm) - (d < 0.0 ? 1 : 0);
 }
 
-__device__ __forceinline__ Located locate_vis(const RawVis &v, const SmemPlaneTab &T, const BinParams &P) {
+// the rare exact path (IEEE divisions, the written order), out of line so that the fast path stays compact;
+// returns {p | S << 16 | inside << 24 | clamped << 25, j0u, j0v, ou | ov << 8}
+__device__ __noinline__ int4 locate_exact(double um, double vm, double wm, double f, const BinParams &P, const uint2 *s_tab) {
+    const SmemPlaneTab T{s_tab, nullptr};
+    const VisPos r = wpg_locate(um, vm, wm, f, P, T);
+    return make_int4(r.p | (r.S << 16) | (r.inside ? 1 << 24 : 0) | (r.clamped ? 1 << 25 : 0), r.j0u, r.j0v, r.ou | (r.ov << 8));
+}
+
+// QP2: the oversampling factor is a power of two (else the general form is used throughout)
+template <bool QP2>
+__device__ __forceinline__ Located locate_vis(const RawVis &v, const uint2 *s_tab, const uint4 *s_ck, const BinParams &P) {
     Located L; L.key = WPG_NO_KEY; L.pos = L.koff = 0; L.S = 0; L.clamped = false;
-    L.zero_weight = v.valid && v.wt == 0.0f;
-    if (!v.valid || L.zero_weight) return L;
-    VisPos r = wpg_locate(v.um, v.vm, v.wm, v.f, P, T);
-    if (!r.inside) return L;
-    L.S = r.S; L.clamped = r.clamped;
-    const uint4 ck = T.ck[T.cls(r.p)];
-    L.key = ck.x + (unsigned)r.j0u * ck.y + ((unsigned)r.j0v >> ck.z);
-    L.pos = (unsigned)r.j0u | ((unsigned)r.j0v << 16);
-    L.koff = wpg_koff(r, P, T);
+    int p, j0u, j0v, ou, ov, S;
+    bool inside, clamped, risk = !QP2;
+    if (QP2) {
+        const double u = __dmul_rn(v.um, v.f), vv = __dmul_rn(v.vm, v.f), w = __dmul_rn(v.wm, v.f);     // G1
+        clamped = fabs(w) > P.w_max;                                                                      // G2
+        p = 0;
+        if (P.dw > 0.0) {               // (uniform branch)
+            // (far outside [-w_max, w_max], and for NaN, the flag is raised: the exact path clamps)
+            const double qd = wpg_div_const(__dadd_rn(w, P.w_max), P.dw, P.rdw);
+            p = min(max(floor_magic(qd, 1048576.0, risk), 0), P.Nw - 1);
+        }
+        S = P.ncls == 1 ? P.S0 : (int)(s_tab[p].y & 0xFFu);
+        const int c = (S - 2) * P.Q / 2;
+        const double Qd = (double)P.Q, lim = 1073741824.0;
+        // G3.  x * Q is exact for Q = 2^k, so the fused form rounds once, like the written two-step form.  Far outside
+        // any grid (also NaN) the flag is raised and the exact path reports "outside".
+        const double tu = __fma_rn(__dadd_rn(wpg_div_const(u, P.du, P.rdu), P.halfN), Qd, 0.5);
+        const double tv = __fma_rn(__dadd_rn(wpg_div_const(vv, P.du, P.rdu), P.halfN), Qd, 0.5);
+        const int Yu = floor_magic(tu, lim, risk) - c;
+        const int Yv = floor_magic(tv, lim, risk) - c;
+        j0u = Yu >> P.qshift; ou = Yu & (P.Q - 1);
+        j0v = Yv >> P.qshift; ov = Yv & (P.Q - 1);
+        const unsigned lim_j = (unsigned)(P.N - S);
+        inside = (unsigned)j0u <= lim_j && (unsigned)j0v <= lim_j;                                       // G4
+    }
+    if (risk) {
+        const int4 o = locate_exact(v.um, v.vm, v.wm, v.f, P, s_tab);
+        p = o.x & 0xFFFF; S = (o.x >> 16) & 0xFF; inside = (o.x >> 24) & 1; clamped = (o.x >> 25) & 1;
+        j0u = o.y; j0v = o.z; ou = o.w & 0xFF; ov = o.w >> 8;
+    }
+    if (!inside) return L;
+    L.S = S; L.clamped = clamped;
+    if (P.ncls == 1) {
+        L.key = (unsigned)j0u * (unsigned)P.nkg + ((unsigned)j0v >> P.kshift);
+        L.koff = (unsigned)(((p * P.Q + ov) * P.Q + ou) * S * S);
+    } else {
+        const uint2 e = s_tab[p];
+        const uint4 ck = s_ck[e.y >> 8];
+        L.key = ck.x + (unsigned)j0u * ck.y + ((unsigned)j0v >> ck.z);
+        L.koff = e.x + (unsigned)((ov * P.Q + ou) * S * S);
+    }
+    L.pos = (unsigned)j0u | ((unsigned)j0v << 16);
     return L;
 }
 
+// The loads of a thread's kVpt visibilities, all issued before any arithmetic (the passes are latency-bound
+// otherwise).  wt = 0 for "no visibility".
+__device__ __forceinline__ void load_raw(const VisIdx &V, const double *__restrict__ uvw, const float *__restrict__ weight,
+                                         const double *__restrict__ fscale, RawVis (&raw)[kVpt]) {
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) {
+        const bool ok = V.i[j] != 0xFFFFFFFFu;
+        // the inputs stream through once per pass: evict-first, so that they do not push the bucket table out of L2
+        raw[j].wt = ok ? __ldcs(weight + V.i[j]) : 0.f;
+        const double *q = uvw + 3ull * (ok ? V.row[j] : 0u);
+        raw[j].um = ok ? __ldcs(q) : 0.0; raw[j].vm = ok ? __ldcs(q + 1) : 0.0; raw[j].wm = ok ? __ldcs(q + 2) : 0.0;
+        raw[j].f = __ldg(fscale + (ok ? V.ch[j] : 0));
+    }
+    // keeps the compiler from consuming a loaded value (and so waiting for it) before the loads that follow in
+    // program order have been issued
+#pragma unroll
+    for (int j = 0; j < kVpt; ++j) asm volatile("" : "+f"(raw[j].wt), "+d"(raw[j].um), "+d"(raw[j].vm), "+d"(raw[j].wm));
+}
+
 // Pass 1: histogram of the keys (reductions without return value) and the wpg_stats counters.
+template <bool QP2>
 __global__ void __launch_bounds__(256, 4)
 bin_count_kernel(const double *__restrict__ uvw, const float *__restrict__ weight,
                  const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
                  const __grid_constant__ BinParams P, Counters *__restrict__ ctr, unsigned *__restrict__ hist) {
-    const long long nvis = P.nrow * P.nchan;
-    unsigned idx[kVpt];
-    vis_indices(P, idx);
-    unsigned c_grid = 0, c_oob = 0, c_zero = 0, c_clamp = 0, c_upd = 0;
+    const VisIdx V = vis_indices(P);
     __shared__ uint2 s_tab[WPG_MAX_NW];
     __shared__ uint4 s_ck[WPG_MAX_CLS];
-    const SmemPlaneTab ST{s_tab, s_ck};
     RawVis raw[kVpt];
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) raw[j] = load_vis(idx[j], nvis, uvw, weight, fscale, P);
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
+    load_raw(V, uvw, weight, fscale, raw);
     wpg_stage_planetab(s_tab, T, P.Nw);
     wpg_stage_classkeys(s_ck, ctr, P);
     __syncthreads();
-    unsigned key[kVpt], len[kVpt];
-    bool head[kVpt];
+    unsigned key[kVpt], pos[kVpt], koff[kVpt], nrec[kVpt], flags = 0, c_upd = 0;
+    bool head[kVpt], rhead[kVpt];
 #pragma unroll
     for (int j = 0; j < kVpt; ++j) {
-        key[j] = WPG_NO_KEY;
-        if (!raw[j].valid) continue;
-        const Located L = locate_vis(raw[j], ST, P);
-        if (L.zero_weight) c_zero += 1;
-        else if (L.key == WPG_NO_KEY) c_oob += 1;
-        else { c_grid += 1; c_clamp += L.clamped; c_upd += L.S * L.S; key[j] = L.key; }
+        key[j] = WPG_NO_KEY; pos[j] = koff[j] = 0;
+        if (V.i[j] == 0xFFFFFFFFu) continue;
+        if (raw[j].wt == 0.0f) { flags += kFlagZero; continue; }                  // R19: zero weight is tested first
+        const Located L = locate_vis<QP2>(raw[j], s_tab, s_ck, P);
+        if (L.key == WPG_NO_KEY) { flags += kFlagOob; continue; }
+        flags += kFlagGridded + (L.clamped ? kFlagClamped : 0u); c_upd += L.S * L.S;
+        key[j] = L.key; pos[j] = L.pos; koff[j] = L.koff;
     }
-    key_runs(key, head, len);
+    key_runs(key, pos, koff, P.compress != 0, head, rhead, nrec);
 #pragma unroll
     for (int j = 0; j < kVpt; ++j)
-        if (head[j]) asm volatile("red.global.add.u32 [%0], %1;" ::"l"(hist + key[j]), "r"(len[j]) : "memory");
-    block_count(ctr, c_grid, c_oob, c_zero, c_clamp, c_upd);
+        if (head[j]) asm volatile("red.global.add.u32 [%0], %1;" ::"l"(hist + key[j]), "r"(nrec[j]) : "memory");
+    block_count(ctr, flags, c_upd);
 }
 
 // Block-wide inclusive scan of one unsigned per thread (1024 threads); returns the inclusive
@@ -318,108 +399,75 @@ __device__ __forceinline__ void store_rec(Rec<double> *dst, double re, double im
     *reinterpret_cast<uint2 *>(&dst->pos) = p;
 }
 
-// Pass 3: scatter into key order.  The slot of a visibility is the running cursor of its bucket
-// (bucket_start[key], advanced atomically: after this pass bucket_start[key] is the END of bucket key,
-// i.e. the array read one element earlier is the start array again — see wpg_launch_bin).  The record
-// carries weight*vis (R9, natural weighting).
-template <typename TT>
-__global__ void __launch_bounds__(256, 4)
+// Pass 3: scatter into key order.  The slot of a record is the running cursor of its bucket (bucket_start[key],
+// advanced atomically once per run of equal keys: after this pass bucket_start[key] is the END of bucket key, i.e.
+// the array read one element earlier is the start array again — see wpg_launch_bin).  The record carries
+// weight * vis (R9, natural weighting), summed over the visibilities merged into it (compression).
+// NPOL = 1: Rec<TT>;  NPOL = 2 | 4: vis[row][chan][pol], one RecP<NPOL> record carries all correlations (fp32).
+template <typename TT, int NPOL, bool QP2>
+__global__ void __launch_bounds__(256, NPOL == 1 ? 4 : 3)
 scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, const float *__restrict__ weight,
                const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
                const __grid_constant__ BinParams P, const Counters *__restrict__ ctr, unsigned *__restrict__ cursor,
-               Rec<TT> *__restrict__ rec) {
-    const long long nvis = P.nrow * P.nchan;
-    unsigned idx[kVpt];
-    vis_indices(P, idx);
-    Located L[kVpt];
-    float wt[kVpt];
-    unsigned dst[kVpt];
-    float2 v[kVpt];
+               void *__restrict__ rec_out) {
+    const VisIdx V = vis_indices(P);
     __shared__ uint2 s_tab[WPG_MAX_NW];
     __shared__ uint4 s_ck[WPG_MAX_CLS];
-    const SmemPlaneTab ST{s_tab, s_ck};
+    unsigned key[kVpt], pos[kVpt], koff[kVpt], nrec[kVpt], dst[kVpt];
+    bool head[kVpt], rhead[kVpt];
+    float wt[kVpt];
+    float2 v[kVpt];
     {
         RawVis raw[kVpt];
+#pragma unroll
+        for (int j = 0; j < kVpt; ++j) v[j] = NPOL == 1 && V.i[j] != 0xFFFFFFFFu ? __ldcs(vis + V.i[j]) : make_float2(0.f, 0.f);
+        load_raw(V, uvw, weight, fscale, raw);
+        wpg_stage_planetab(s_tab, T, P.Nw);
+        wpg_stage_classkeys(s_ck, ctr, P);
+        __syncthreads();
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) {
-            const long long i = idx[j];        // 0xFFFFFFFF = none (>= nvis)
-            raw[j] = load_vis(i, nvis, uvw, weight, fscale, P);
-            v[j] = i < nvis ? __ldg(vis + i) : make_float2(0.f, 0.f);
+            key[j] = WPG_NO_KEY; pos[j] = koff[j] = 0; wt[j] = raw[j].wt;
+            if (V.i[j] == 0xFFFFFFFFu || raw[j].wt == 0.0f) continue;
+            const Located L = locate_vis<QP2>(raw[j], s_tab, s_ck, P);
+            key[j] = L.key; pos[j] = L.pos; koff[j] = L.koff;
         }
-#pragma unroll
-        for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
-        wpg_stage_planetab(s_tab, T, P.Nw);
-        wpg_stage_classkeys(s_ck, ctr, P);
-        __syncthreads();
-#pragma unroll
-        for (int j = 0; j < kVpt; ++j) { L[j] = locate_vis(raw[j], ST, P); wt[j] = raw[j].wt; }
     }
-    // one returning atomic per run of equal keys (the slowest instruction of the pass: ~5 cycles per lane)
-    unsigned key[kVpt], len[kVpt];
-    bool head[kVpt];
+    // one returning atomic per run of equal keys (the slowest instruction of the pass: ~2 cycles per lane)
+    key_runs(key, pos, koff, P.compress != 0, head, rhead, nrec);
 #pragma unroll
-    for (int j = 0; j < kVpt; ++j) key[j] = L[j].key;
-    key_runs(key, head, len);
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) dst[j] = head[j] ? atomicAdd(cursor + key[j], len[j]) : 0u;
+    for (int j = 0; j < kVpt; ++j) dst[j] = head[j] ? atomicAdd(cursor + key[j], nrec[j]) : 0u;
 #pragma unroll
     for (int j = 1; j < kVpt; ++j)
-        if (key[j] != WPG_NO_KEY && !head[j]) dst[j] = dst[j - 1] + 1u;
+        if (key[j] != WPG_NO_KEY && !head[j]) dst[j] = dst[j - 1] + (rhead[j] ? 1u : 0u);
+    if (NPOL == 1) {
+        TT re[kVpt], im[kVpt];
 #pragma unroll
-    for (int j = 0; j < kVpt; ++j) {
-        if (L[j].key == WPG_NO_KEY) continue;
-        const TT w = (TT)wt[j];
-        store_rec(rec + dst[j], w * (TT)v[j].x, w * (TT)v[j].y, make_uint2(L[j].pos, L[j].koff));
-    }
-}
-
-// Pass 3 for NPOL correlations per (row, channel): vis[row][chan][pol]; one record carries all of them.
-template <int NPOL>
-__global__ void __launch_bounds__(256, 3)
-scatter_pol_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, const float *__restrict__ weight,
-                   const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
-                   const __grid_constant__ BinParams P, const Counters *__restrict__ ctr, unsigned *__restrict__ cursor,
-                   RecP<NPOL> *__restrict__ rec) {
-    const long long nvis = P.nrow * P.nchan;
-    unsigned idx[kVpt];
-    vis_indices(P, idx);
-    Located L[kVpt];
-    float wt[kVpt];
-    unsigned dst[kVpt];
-    __shared__ uint2 s_tab[WPG_MAX_NW];
-    __shared__ uint4 s_ck[WPG_MAX_CLS];
-    const SmemPlaneTab ST{s_tab, s_ck};
-    {
-        RawVis raw[kVpt];
+        for (int j = 0; j < kVpt; ++j) { const TT w = (TT)wt[j]; re[j] = w * (TT)v[j].x; im[j] = w * (TT)v[j].y; }
 #pragma unroll
-        for (int j = 0; j < kVpt; ++j) raw[j] = load_vis(idx[j], nvis, uvw, weight, fscale, P);
+        for (int j = kVpt - 1; j > 0; --j)
+            if (key[j] != WPG_NO_KEY && !rhead[j]) { re[j - 1] += re[j]; im[j - 1] += im[j]; }
 #pragma unroll
-        for (int j = 0; j < kVpt; ++j) use_after_here(raw[j]);
-        wpg_stage_planetab(s_tab, T, P.Nw);
-        wpg_stage_classkeys(s_ck, ctr, P);
-        __syncthreads();
+        for (int j = 0; j < kVpt; ++j)
+            if (rhead[j]) store_rec(reinterpret_cast<Rec<TT> *>(rec_out) + dst[j], re[j], im[j], make_uint2(pos[j], koff[j]));
+    } else {
+        // walk the thread's visibilities in order; a record is written when the next one starts a new record
+        constexpr int NP = NPOL > 1 ? NPOL : 2;
+        RecP<NP> out;
 #pragma unroll
-        for (int j = 0; j < kVpt; ++j) { L[j] = locate_vis(raw[j], ST, P); wt[j] = raw[j].wt; }
-    }
-    unsigned key[kVpt], len[kVpt];
-    bool head[kVpt];
+        for (int j = 0; j < kVpt; ++j) {
+            if (key[j] == WPG_NO_KEY) continue;
+            const float2 *src = vis + (size_t)V.i[j] * NP;
 #pragma unroll
-    for (int j = 0; j < kVpt; ++j) key[j] = L[j].key;
-    key_runs(key, head, len);
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) dst[j] = head[j] ? atomicAdd(cursor + key[j], len[j]) : 0u;
-#pragma unroll
-    for (int j = 1; j < kVpt; ++j)
-        if (key[j] != WPG_NO_KEY && !head[j]) dst[j] = dst[j - 1] + 1u;
-#pragma unroll
-    for (int j = 0; j < kVpt; ++j) {
-        if (key[j] == WPG_NO_KEY) continue;
-        const float2 *src = vis + (size_t)idx[j] * NPOL;
-        RecP<NPOL> out;
-#pragma unroll
-        for (int p = 0; p < NPOL; ++p) { const float2 v = __ldg(src + p); out.v[p] = make_float2(wt[j] * v.x, wt[j] * v.y); }
-        out.pos = L[j].pos; out.koff = L[j].koff;
-        rec[dst[j]] = out;
+            for (int p = 0; p < NP; ++p) {
+                const float2 q = __ldg(src + p);
+                if (rhead[j]) out.v[p] = make_float2(wt[j] * q.x, wt[j] * q.y);
+                else { out.v[p].x += wt[j] * q.x; out.v[p].y += wt[j] * q.y; }
+            }
+            out.pos = pos[j]; out.koff = koff[j];
+            const bool last = j + 1 == kVpt || key[j + 1 < kVpt ? j + 1 : j] == WPG_NO_KEY || rhead[j + 1 < kVpt ? j + 1 : j];
+            if (last) reinterpret_cast<RecP<NP> *>(rec_out)[dst[j]] = out;
+        }
     }
 }
 
@@ -438,9 +486,11 @@ int wpg_launch_exclusive_scan(wpg_ctx *ctx, unsigned *hist, unsigned n, unsigned
     return WPG_OK;
 }
 
-int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
-                   const double *d_freq, const PlaneTab &tab, const BinParams &bp,
-                   const WorkspaceLayout &ws, wpg_prec prec, char *w) {
+// The binning passes (npol = 1: Rec<float | double> records; npol = 2 | 4: RecP<npol>, fp32 — positions do not depend
+// on the correlation, so only the scatter differs).
+static int launch_bin_passes(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                             const double *d_freq, const PlaneTab &tab, const BinParams &bp,
+                             const WorkspaceLayout &ws, wpg_prec prec, int npol, char *w) {
     long long nvis = bp.nrow * bp.nchan;
     Counters *ctr = (Counters *)(w + ws.off_counters);
     // bucket_start[0 .. nkeys] lives at off_hist; the counts of key k are accumulated one element
@@ -452,64 +502,54 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
     unsigned *blocksum = (unsigned *)(w + ws.off_blocksum);
     cudaStream_t s = ctx->stream;
     double *fscale = (double *)(w + ws.off_fscale);
-    unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
-    if (bp.vis_block) {                // ceil(time steps / kVpt) * vis_block threads
+    dim3 nb((unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt)), 1, 1);
+    if (bp.vis_block) {                // ceil(vis_block / 256) blocks per group of kVpt time steps
         const long long nd = (nvis + bp.vis_block - 1) / bp.vis_block;
-        nb = (unsigned)((((nd + kVpt - 1) / kVpt) * bp.vis_block + 255) / 256);
+        const long long nblk = (long long)((bp.vis_block + 255) / 256) * ((nd + kVpt - 1) / kVpt);
+        if (nblk >= (1ll << 31)) return wpg_fail(ctx, WPG_EINVAL, "row_block = %u gives too many binning blocks", bp.vis_block / bp.nchan);
+        nb = dim3((unsigned)nblk, 1, 1);
     }
+    const bool any = nvis > 0;
+    const bool qp2 = bp.qshift >= 0;
     chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale, bp, ctr);
     if (bp.dyn_keys) {
-        census_kernel<<<ctx->sm_count * 8, 256, 0, s>>>(d_uvw, fscale, tab, bp, ctr);
+        census_kernel<<<ctx->sm_count * 4, 256, 0, s>>>(d_uvw, fscale, tab, bp, ctr);
         plan_keys_kernel<<<1, 32, 0, s>>>(ctr, bp.ncls, bp.N, ws.nkeys);
         ctx->n_launches += 2;
     }
-    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
+    if (any) {
+        if (qp2) bin_count_kernel<true><<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
+        else bin_count_kernel<false><<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
+    }
     scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
     scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
     scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
-    if (nb) {
-        if (prec == WPG_F32)
-            scatter_kernel<float><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
-                                                      (Rec<float> *)(w + ws.off_records));
-        else
-            scatter_kernel<double><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
-                                                       (Rec<double> *)(w + ws.off_records));
+    if (any) {
+        const float2 *v = (const float2 *)d_vis;
+        void *rec = w + ws.off_records;
+#define WPG_SCATTER(TT, NP)                                                                                              \
+        do {                                                                                                             \
+            if (qp2) scatter_kernel<TT, NP, true><<<nb, 256, 0, s>>>(v, d_uvw, d_weight, fscale, tab, bp, ctr, hist, rec);  \
+            else scatter_kernel<TT, NP, false><<<nb, 256, 0, s>>>(v, d_uvw, d_weight, fscale, tab, bp, ctr, hist, rec);     \
+        } while (0)
+        if (npol == 4) WPG_SCATTER(float, 4);
+        else if (npol == 2) WPG_SCATTER(float, 2);
+        else if (prec == WPG_F32) WPG_SCATTER(float, 1);
+        else WPG_SCATTER(double, 1);
+#undef WPG_SCATTER
     }
-    ctx->n_launches += nb ? 6 : 4;
+    ctx->n_launches += any ? 6 : 4;
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }
 
-// Binning for the polarised gridder: the count pass and the scan are those of wpg_launch_bin (positions do not
-// depend on the correlation), the scatter writes RecP<npol> records.
+int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                   const double *d_freq, const PlaneTab &tab, const BinParams &bp,
+                   const WorkspaceLayout &ws, wpg_prec prec, char *w) {
+    return launch_bin_passes(ctx, d_vis, d_uvw, d_weight, d_freq, tab, bp, ws, prec, 1, w);
+}
+
 int wpg_launch_bin_pol(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight, const double *d_freq,
                        const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, int npol, char *w) {
-    long long nvis = bp.nrow * bp.nchan;
-    Counters *ctr = (Counters *)(w + ws.off_counters);
-    unsigned *bucket_start = (unsigned *)(w + ws.off_hist);
-    unsigned *hist = bucket_start + 1;
-    unsigned *blocksum = (unsigned *)(w + ws.off_blocksum);
-    cudaStream_t s = ctx->stream;
-    double *fscale = (double *)(w + ws.off_fscale);
-    unsigned nb = (unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt));
-    if (bp.vis_block) {
-        const long long nd = (nvis + bp.vis_block - 1) / bp.vis_block;
-        nb = (unsigned)((((nd + kVpt - 1) / kVpt) * bp.vis_block + 255) / 256);
-    }
-    chan_scale_kernel<<<(bp.nchan + 255) / 256, 256, 0, s>>>(d_freq, bp.nchan, fscale, bp, ctr);
-    if (nb) bin_count_kernel<<<nb, 256, 0, s>>>(d_uvw, d_weight, fscale, tab, bp, ctr, hist);
-    scan_reduce_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
-    scan_blocksums_kernel<<<1, 1024, 0, s>>>(blocksum, ws.nblocks_scan, ctr);
-    scan_apply_kernel<<<ws.nblocks_scan, 1024, 0, s>>>(hist, ws.nkeys, blocksum);
-    if (nb) {
-        if (npol == 4)
-            scatter_pol_kernel<4><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
-                                                     (RecP<4> *)(w + ws.off_records));
-        else
-            scatter_pol_kernel<2><<<nb, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp, ctr, hist,
-                                                     (RecP<2> *)(w + ws.off_records));
-    }
-    ctx->n_launches += nb ? 6 : 4;
-    WPG_CUDA(ctx, cudaGetLastError());
-    return WPG_OK;
+    return launch_bin_passes(ctx, d_vis, d_uvw, d_weight, d_freq, tab, bp, ws, WPG_F32, npol, w);
 }

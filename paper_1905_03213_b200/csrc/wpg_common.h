@@ -40,6 +40,8 @@ struct BinParams {
     uint32_t keys_per_class;       // N * nkg; key = (cls * N + j0u) * nkg + (j0v >> kshift)
     uint32_t nkeys;                // size of the key space (ncls * keys_per_class, or the key budget if dynamic)
     int dyn_keys;                  // 1: per-class key layout chosen on the device (ragged stacks)
+    int S0;                        // support of class 0 (uniform stacks: THE support, no table lookup)
+    int compress;                  // 1: record compression (visibilities with equal window start and coefficient slice share a record)
 };
 
 // Sorted record.  pos = j0u | j0v << 16 (window start, cells); koff = element offset
@@ -85,6 +87,7 @@ struct wpg_ctx {
     int opt_timing = 0;       // 1: wpg_grid brackets its phases with CUDA events
     int64_t opt_row_block = 0; // rows per time step (0 = unknown), see wpg_set_option
     int opt_no_pairs = 0;     // 1: fp32 even supports also go through the run gridder (A/B comparison)
+    int opt_compress = 1;     // record compression in the binning pass (0: one record per gridded visibility)
     // instrumentation
     int64_t n_launches = 0;   // kernels of this library launched so far
     std::vector<cudaEvent_t> ev;   // triplets: start, after binning, after gridder (pool, reused)

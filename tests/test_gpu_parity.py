@@ -139,6 +139,7 @@ def test_binning_records_match_oracle_index_map(ctx):
         exp.append((j0u | (j0v << 16), (p * Q * Q + ov * Q + ou) * S * S,
                     np.float32(wl.vis[k, 0].real).view(np.uint32), np.float32(wl.vis[k, 0].imag).view(np.uint32)))
     exp = sorted(exp)
+    ctx.set_option("compress", 0)              # one record per gridded visibility (compression: test_record_compression)
     for kb in (0, 12):
         ctx.set_option("key_bits", kb)
         ws, info, stats = ctx.bin(*d, ks)
@@ -157,7 +158,70 @@ def test_binning_records_match_oracle_index_map(ctx):
         bs = raw[info["off_bucket_start"]:info["off_bucket_start"] + 4 * (info["n_keys"] + 1)].view(np.uint32)
         assert bs[0] == 0 and bs[-1] == 20000
         assert np.array_equal(bs.astype(np.int64), np.searchsorted(key, np.arange(info["n_keys"] + 1)))
-    ctx.set_option("key_bits", 0)
+    ctx.set_option("key_bits", 0); ctx.set_option("compress", 1)
+
+
+def test_record_compression(ctx):
+    """Record compression: with the rows-per-time-step hint a binning thread
+    holds consecutive samples of one baseline and channel; those with the same window start and coefficient slice
+    share one record carrying the sum of their weight * vis.  Checked on slowly drifting tracks: fewer records than
+    gridded visibilities; every record is an oracle (window, slice) pair; per pair the record values sum to the
+    oracle-side sum of weight * vis; counters count visibilities, not records; the grid is unchanged."""
+    rng = np.random.default_rng(17)
+    N, cell, Q, S, Nw, w_max = 256, 0.1 / 256, 8, 8, 8, 100.0
+    nbl, ndump, nchan = 97, 200, 2
+    nrow = nbl * ndump
+    b = np.arange(nrow) % nbl; t = np.arange(nrow) // nbl
+    uvw = np.stack([(b - 48) * 11.0 + 0.05 * t, (b % 9 - 4) * 95.0 + 0.03 * t, rng.uniform(-90, 90, nbl)[b]], 1)
+    freq = np.array([1.0, 1.01]) * synth.C0 / 0.5
+    vis = (rng.standard_normal((nrow, nchan)) + 1j * rng.standard_normal((nrow, nchan))).astype(np.complex64)
+    wt = rng.uniform(0.5, 2.0, (nrow, nchan)).astype(np.float32)
+    wt[rng.uniform(size=wt.shape) < 0.05] = 0.0
+    st = owk.build_stack(Nw, w_max, S, Q, N, cell)
+    ref, rstats = ogrid.grid(uvw, vis, wt, freq, st)
+    wl = synth.Workload("drift", uvw, freq, vis, wt, N, cell, Nw, w_max, S, Q)
+    d = dev(wl)
+    expect = {}
+    fs = freq / synth.C0
+    for k in range(nrow):
+        for c in range(nchan):
+            if wt[k, c] == 0.0:
+                continue
+            j0u, ou = ogrid.index_map(uvw[k, 0] * fs[c], N, cell, S, Q)
+            j0v, ov = ogrid.index_map(uvw[k, 1] * fs[c], N, cell, S, Q)
+            if j0u < 0 or j0v < 0 or j0u + S > N or j0v + S > N:
+                continue
+            p, _ = ogrid.plane_of(uvw[k, 2] * fs[c], w_max, Nw)
+            kk = (j0u | (j0v << 16), (p * Q * Q + ov * Q + ou) * S * S)
+            expect[kk] = expect.get(kk, 0j) + complex(np.float32(wt[k, c])) * complex(vis[k, c])
+    for prec, rb_bytes in ((wpgrid.F32, 16), (wpgrid.F64, 24)):
+        ks = upload(ctx, st, prec)
+        n_rec = {}
+        for rb, comp in ((nbl, 1), (nbl, 0), (0, 1)):
+            ctx.set_option("row_block", rb); ctx.set_option("compress", comp)
+            ws, info, stats = ctx.bin(*d, ks)
+            assert stats == rstats and info["record_bytes"] == rb_bytes
+            n = info["n_records"]
+            n_rec[(rb, comp)] = n
+            raw = ws.cpu().numpy()[info["off_records"]:info["off_records"] + rb_bytes * n]
+            got = {}
+            if prec == wpgrid.F32:
+                r = raw.view(np.uint32).reshape(-1, 4)
+                vals = r[:, :2].copy().view(np.float32).astype(np.float64); keys = r[:, 2:]
+            else:
+                vals = raw.view(np.float64).reshape(-1, 3)[:, :2]; keys = raw.view(np.uint32).reshape(-1, 6)[:, 4:]
+            for (re, im), (ps, ko) in zip(vals, keys):
+                kk = (int(ps), int(ko))
+                got[kk] = got.get(kk, 0j) + complex(re, im)
+            assert set(got) == set(expect)
+            tol = 2e-6 if prec == wpgrid.F32 else 1e-13
+            assert max(abs(got[k] - expect[k]) for k in expect) <= tol * max(abs(x) for x in expect.values())
+            g, s = ctx.grid(*d, ks, stats=True)
+            assert s == rstats and relerr(g.cpu().numpy(), ref) <= TOL[prec]
+        assert n_rec[(nbl, 0)] == rstats["n_gridded"]
+        assert n_rec[(nbl, 1)] < 0.6 * rstats["n_gridded"]        # consecutive samples drift by ~0.005 cells: runs of 4 merge
+        assert n_rec[(nbl, 1)] >= len(expect)
+    ctx.set_option("row_block", 0); ctx.set_option("compress", 1)
 
 
 # ------------------------------------------------------------------ edge cases
@@ -464,6 +528,7 @@ def test_binning_exactness_on_ties_and_near_ties(ctx):
                 continue
             exp.append((j0u | (j0v << 16), (p * Q * Q + ov * Q + ou) * S * S, i))
         d = (torch.from_numpy(vis).cuda(), torch.from_numpy(uvw).cuda(), torch.from_numpy(wt).cuda(), torch.from_numpy(freq).cuda())
+        ctx.set_option("compress", 0)
         for rb in (0, 7):
             ctx.set_option("row_block", rb)
             ws, info, stats = ctx.bin(*d, ks)
@@ -472,7 +537,7 @@ def test_binning_exactness_on_ties_and_near_ties(ctx):
             rec = raw[info["off_records"]:info["off_records"] + 16 * len(exp)].view(np.uint32).reshape(-1, 4)
             got = sorted((int(r[2]), int(r[3]), int(round(float(np.array([r[0]], np.uint32).view(np.float32)[0])))) for r in rec)
             assert got == sorted(exp)
-        ctx.set_option("row_block", 0)
+        ctx.set_option("row_block", 0); ctx.set_option("compress", 1)
 
 
 def test_odd_grid_size_and_small_grids(ctx):
