@@ -485,7 +485,7 @@ def run_pol(args, ctx, wl, stack, d_uvw, d_wt, d_freq, dev, world, rank, dist):
     nrow, nchan, N = d_uvw.shape[0], d_freq.shape[0], wl.grid_N
     gen = torch.Generator(device=dev).manual_seed(3)
     vis = torch.view_as_complex(torch.randn((nrow, nchan, npol, 2), dtype=torch.float32, device=dev, generator=gen))
-    need = int(ctx.lib.wpg_grid_pol_workspace_bytes(ctx.h, nrow, nchan, npol, ctypes.byref(stack.desc)))
+    need = int(ctx.lib.wpg_grid_pol_workspace_bytes(ctx.h, nrow, nchan, npol, ctypes.byref(stack.desc), stack.prec))
     ws = torch.empty(need, dtype=torch.uint8, device=dev)
     grid = torch.zeros((npol, N, N), dtype=torch.complex64, device=dev)
     iws = torch.empty(int(ctx.lib.wpg_dirty_image_workspace_bytes(N, stack.prec)), dtype=torch.uint8, device=dev)

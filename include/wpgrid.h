@@ -176,14 +176,17 @@ int  wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const double *d_uv
 /* ---- polarisation axis (data are row x channel x polarisation) ----------
  * The npol correlations of a (row, channel) share position, weight and coefficient slice:
  *   grid[pol][j0v+iv][j0u+iu] += (weight[r][c] * vis[r][c][pol]) * K[p][ov][ou][iv][iu]   for every pol,
- * i.e. npol independent griddings of wpg_grid with one coefficient fetch for all of them.  fp32 only,
- * npol = 2 or 4, uniform stacks of support 8 or 16 (WPG_EINVAL otherwise), 16-byte aligned stack.
- *   d_vis c64 [nrow][nchan][npol]    d_weight f32 [nrow][nchan]    d_grid c64 [npol][N][N], ACCUMULATED INTO.
+ * i.e. npol independent griddings of wpg_grid with one coefficient fetch for all of them.  npol = 2 or 4
+ * (WPG_EINVAL otherwise); fp32 and fp64; any stack wpg_grid takes (uniform or ragged, even or odd supports).
+ * Uniform fp32 stacks of support 8 or 16 (16-byte aligned) take the pair gridder (one 16-byte load feeds 2 npol
+ * updates), everything else the general cell gridder, one launch per support class.
+ *   d_vis c64 [nrow][nchan][npol]    d_weight f32 [nrow][nchan]    d_grid c64 | c128 [npol][N][N], ACCUMULATED INTO.
  * wpg_stats counts (row, channel) samples; n_updates = sum of S^2 over them (x npol grid-point updates). */
-size_t wpg_grid_pol_workspace_bytes(const wpg_ctx *ctx, int64_t nrow, int nchan, int npol, const wpg_kdesc *desc);
+size_t wpg_grid_pol_workspace_bytes(const wpg_ctx *ctx, int64_t nrow, int nchan, int npol, const wpg_kdesc *desc,
+                                    wpg_prec prec);
 int  wpg_grid_pol(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight, const double *d_freq,
-                  int64_t nrow, int nchan, int npol, const void *d_kernels, const wpg_kdesc *desc, void *d_grid,
-                  void *d_workspace, size_t workspace_bytes, wpg_stats *h_stats_or_null);
+                  int64_t nrow, int nchan, int npol, const void *d_kernels, const wpg_kdesc *desc, wpg_prec prec,
+                  void *d_grid, void *d_workspace, size_t workspace_bytes, wpg_stats *h_stats_or_null);
 
 /* ---- degridding: the adjoint of wpg_grid with unit weights ---------------
  *   vis_out[r][c] = sum over the S x S window of grid[j0v+iv][j0u+iu] * conj(K[p][ov][ou][iv][iu]),

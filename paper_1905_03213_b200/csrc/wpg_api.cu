@@ -314,35 +314,34 @@ extern "C" int wpg_grid(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, co
 }
 
 // ---- polarised gridder
-static int pol_plan(wpg_ctx *ctx, const wpg_kdesc *desc, int64_t nrow, int nchan, int npol, PlaneTab *tab, BinParams *bp,
-                    WorkspaceLayout *ws) {
+static int pol_plan(wpg_ctx *ctx, const wpg_kdesc *desc, int64_t nrow, int nchan, int npol, wpg_prec prec, PlaneTab *tab,
+                    BinParams *bp, WorkspaceLayout *ws) {
     if (npol != 2 && npol != 4) return wpg_fail(ctx, WPG_EINVAL, "npol = %d: 2 or 4 correlations", npol);
-    int rc = wpg_make_plan(ctx, desc, nrow, nchan, WPG_F32, tab, bp, ws);
+    int rc = wpg_make_plan(ctx, desc, nrow, nchan, prec, tab, bp, ws);
     if (rc) return rc;
-    if (bp->ncls != 1 || (tab->clsS[0] != 8 && tab->clsS[0] != 16))
-        return wpg_fail(ctx, WPG_EINVAL, "the polarised gridder takes uniform supports 8 or 16");
-    ws->total = ws->off_records + align_up((size_t)nrow * nchan * (8 * (size_t)npol + 8));
+    const size_t recb = (prec == WPG_F32 ? 8 : 16) * (size_t)npol + 8;
+    ws->total = ws->off_records + align_up((size_t)nrow * nchan * recb);
     return WPG_OK;
 }
 
-extern "C" size_t wpg_grid_pol_workspace_bytes(const wpg_ctx *ctx, int64_t nrow, int nchan, int npol, const wpg_kdesc *desc) {
+extern "C" size_t wpg_grid_pol_workspace_bytes(const wpg_ctx *ctx, int64_t nrow, int nchan, int npol, const wpg_kdesc *desc,
+                                               wpg_prec prec) {
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     wpg_ctx tmp;
     if (ctx) { tmp.opt_key_bits = ctx->opt_key_bits; }
-    if (pol_plan(&tmp, desc, nrow, nchan, npol, &tab, &bp, &ws)) return 0;
+    if (pol_plan(&tmp, desc, nrow, nchan, npol, prec, &tab, &bp, &ws)) return 0;
     return ws.total;
 }
 
 extern "C" int wpg_grid_pol(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
                             const double *d_freq, int64_t nrow, int nchan, int npol, const void *d_kernels,
-                            const wpg_kdesc *desc, void *d_grid, void *d_workspace, size_t workspace_bytes,
+                            const wpg_kdesc *desc, wpg_prec prec, void *d_grid, void *d_workspace, size_t workspace_bytes,
                             wpg_stats *h_stats) {
     int rc = check_ptrs(ctx, d_vis, d_uvw, d_weight, d_freq, nrow);
     if (rc) return rc;
     if (!d_kernels || !d_grid) return wpg_fail(ctx, WPG_EINVAL, "kernels or grid pointer is NULL");
-    if (((uintptr_t)d_kernels & 15) != 0) return wpg_fail(ctx, WPG_EINVAL, "the kernel stack must be 16-byte aligned");
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
-    rc = pol_plan(ctx, desc, nrow, nchan, npol, &tab, &bp, &ws);
+    rc = pol_plan(ctx, desc, nrow, nchan, npol, prec, &tab, &bp, &ws);
     if (rc) return rc;
     if (!d_workspace || workspace_bytes < ws.total)
         return wpg_fail(ctx, WPG_ENOMEM, "workspace of %zu bytes given, %zu needed", workspace_bytes, ws.total);
@@ -350,10 +349,10 @@ extern "C" int wpg_grid_pol(wpg_ctx *ctx, const void *d_vis, const double *d_uvw
     char *w = (char *)d_workspace;
     if ((rc = wpg_mark(ctx, 0))) return rc;
     WPG_CUDA(ctx, cudaMemsetAsync(w, 0, ws.off_blocksum, ctx->stream));
-    rc = wpg_launch_bin_pol(ctx, d_vis, d_uvw, d_weight, d_freq, tab, bp, ws, npol, w);
+    rc = wpg_launch_bin_pol(ctx, d_vis, d_uvw, d_weight, d_freq, tab, bp, ws, prec, npol, w);
     if (rc) return rc;
     if ((rc = wpg_mark(ctx, 1))) return rc;
-    rc = wpg_launch_grid_pol(ctx, tab, bp, ws, npol, d_kernels, d_grid, w);
+    rc = wpg_launch_grid_pol(ctx, tab, bp, ws, prec, npol, d_kernels, d_grid, w);
     if (rc) return rc;
     if ((rc = wpg_mark(ctx, 2))) return rc;
     if (h_stats) return read_stats(ctx, (const Counters *)(w + ws.off_counters), h_stats, nullptr);

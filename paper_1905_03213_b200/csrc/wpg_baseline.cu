@@ -76,49 +76,109 @@ __global__ void bl_chan_scale_kernel(const double *__restrict__ freq, int nchan,
     if (c < nchan) fscale[c] = __ddiv_rn(freq[c], WPG_C0);
 }
 
-// Pass 5: the records, in baseline-then-time order (record s * nchan + ch = row perm[s], channel ch).  A flagged
-// or out-of-grid visibility keeps its place in the time series as a zero-valued record at the window start
-// clamped into the grid (it adds zeros; the counters do not count it as gridded).
+// Support class of visibility idx of the baseline-then-time order (w -> plane -> class; G1-G2 only).
+__device__ __forceinline__ int bl_class_of(long long idx, const BinParams &P, const unsigned *__restrict__ perm,
+                                           const double *__restrict__ uvw, const double *__restrict__ fscale, const uint2 *s_tab) {
+    const unsigned s = (unsigned)(idx / P.nchan);
+    const int ch = (int)(idx - (long long)s * P.nchan);
+    const double w = __dmul_rn(__ldg(uvw + 3 * (long long)perm[s] + 2), __ldg(fscale + ch));
+    int p = 0;
+    if (P.dw > 0.0) {
+        const double ws = __dadd_rn(w, P.w_max);
+        double qd = wpg_div_const(ws, P.dw, P.rdw);
+        if (wpg_near_integer(qd)) qd = __ddiv_rn(ws, P.dw);
+        const double fp = floor(qd);
+        p = fp < 0.0 ? 0 : (fp > (double)(P.Nw - 1) ? P.Nw - 1 : (int)fp);
+    }
+    return (int)(s_tab[p].y >> 8);
+}
+
+// Ragged stacks, pass 4b: records per (support class, block of 256 consecutive positions of the baseline-then-time
+// order): ctab[cls * nblocks + block].  Its exclusive scan (class-major) gives every block the start of its records
+// inside each class, so that the classes are contiguous AND each keeps the baseline-then-time order (a stable
+// partition): the gridder of a class then walks its baselines' time series as in the uniform case.
+__global__ void __launch_bounds__(256)
+bl_class_count_kernel(const double *__restrict__ uvw, const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
+                      const __grid_constant__ BinParams P, const unsigned *__restrict__ perm, unsigned *__restrict__ ctab) {
+    __shared__ uint2 s_tab[WPG_MAX_NW];
+    __shared__ unsigned s_cnt[WPG_MAX_CLS];
+    wpg_stage_planetab(s_tab, T, P.Nw);
+    if (threadIdx.x < WPG_MAX_CLS) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    const long long nvis = P.nrow * P.nchan;
+    const long long idx = (long long)blockIdx.x * 256 + threadIdx.x;
+    if (idx < nvis) atomicAdd(&s_cnt[bl_class_of(idx, P, perm, uvw, fscale, s_tab)], 1u);
+    __syncthreads();
+    if ((int)threadIdx.x < P.ncls) ctab[(size_t)threadIdx.x * gridDim.x + blockIdx.x] = s_cnt[threadIdx.x];
+}
+
+// Pass 5: the records, in baseline-then-time order (record s * nchan + ch = row perm[s], channel ch; ragged stacks:
+// that order inside each support class, classes one after the other).  A flagged or out-of-grid visibility keeps its
+// place in the time series as a zero-valued record at the window start clamped into the grid (it adds zeros; the
+// counters do not count it as gridded).  bucket[c] = first record of class c, bucket[ncls] = number of records.
 template <typename TT>
 __global__ void __launch_bounds__(256)
 bl_build_records_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, const float *__restrict__ weight,
                         const double *__restrict__ fscale, const __grid_constant__ PlaneTab T,
                         const __grid_constant__ BinParams P, const unsigned *__restrict__ perm, Counters *__restrict__ ctr,
-                        Rec<TT> *__restrict__ rec, unsigned *__restrict__ bucket2) {
+                        Rec<TT> *__restrict__ rec, unsigned *__restrict__ bucket, const unsigned *__restrict__ ctab) {
     __shared__ uint2 s_tab[WPG_MAX_NW];
+    __shared__ unsigned s_wcnt[8][WPG_MAX_CLS];
     wpg_stage_planetab(s_tab, T, P.Nw);
+    if (P.ncls > 1) for (int i = threadIdx.x; i < 8 * WPG_MAX_CLS; i += 256) (&s_wcnt[0][0])[i] = 0;
     __syncthreads();
     const SmemPlaneTab ST{s_tab, nullptr};
     const long long nvis = P.nrow * P.nchan;
     const long long idx = (long long)blockIdx.x * 256 + threadIdx.x;
-    if (idx == 0) { bucket2[0] = 0u; bucket2[1] = (unsigned)nvis; }
+    if (P.ncls == 1) { if (idx == 0) { bucket[0] = 0u; bucket[1] = (unsigned)nvis; } }
+    else if (blockIdx.x == 0 && (int)threadIdx.x <= P.ncls)
+        bucket[threadIdx.x] = (int)threadIdx.x < P.ncls ? ctab[(size_t)threadIdx.x * gridDim.x] : (unsigned)nvis;
     unsigned c_grid = 0, c_oob = 0, c_zero = 0, c_clamp = 0, c_upd = 0;
-    if (idx < nvis) {
+    bool have = idx < nvis;
+    Rec<TT> out; out.re = out.im = (TT)0; out.pos = out.koff = 0;
+    int cls = 0;
+    if (have) {
         const unsigned s = (unsigned)(idx / P.nchan);
         const int ch = (int)(idx - (long long)s * P.nchan);
         const long long row = perm[s], i = row * P.nchan + ch;
         const float wt = __ldg(weight + i);
         VisPos r = wpg_locate(__ldg(uvw + 3 * row), __ldg(uvw + 3 * row + 1), __ldg(uvw + 3 * row + 2),
                               __ldg(fscale + ch), P, ST);
+        cls = ST.cls(r.p);
         const bool ok = wt != 0.0f && r.inside;
         if (wt == 0.0f) c_zero = 1; else if (!r.inside) c_oob = 1;
         else { c_grid = 1; c_clamp = r.clamped; c_upd = r.S * r.S; }
         const int j0u = min(max(r.j0u, 0), P.N - r.S), j0v = min(max(r.j0v, 0), P.N - r.S);
         const float2 v = __ldg(vis + i);
         // literal zeros for a flagged / off-grid sample: its value may be NaN or Inf (RFI), and 0 * NaN = NaN
-        Rec<TT> out;
         out.re = ok ? (TT)wt * (TT)v.x : (TT)0; out.im = ok ? (TT)wt * (TT)v.y : (TT)0;
         out.pos = (unsigned)j0u | ((unsigned)j0v << 16);
         out.koff = ok ? wpg_koff(r, P, ST) : (unsigned)ST.off(r.p);
-        rec[idx] = out;
     }
+    unsigned dst = (unsigned)idx;
+    if (P.ncls > 1) {
+        // stable rank inside the block among the records of the same class: lower lanes of the warp, then lower warps
+        const unsigned live = __ballot_sync(0xffffffffu, have);
+        unsigned rank = 0, m = 0;
+        if (have) {
+            m = __match_any_sync(live, cls);
+            rank = __popc(m & ((1u << (threadIdx.x & 31)) - 1u));
+            if (rank == 0) s_wcnt[threadIdx.x >> 5][cls] = __popc(m);
+        }
+        __syncthreads();
+        if (have) {
+            for (unsigned w = 0; w < (threadIdx.x >> 5); ++w) rank += s_wcnt[w][cls];
+            dst = ctab[(size_t)cls * gridDim.x + blockIdx.x] + rank;
+        }
+    }
+    if (have) rec[dst] = out;
     // statistics: warp sums, spread over the counter slots
     unsigned v5[5] = {c_grid, c_oob, c_zero, c_clamp, c_upd};
-    unsigned long long *dst[5] = {ctr->n_gridded, ctr->n_skipped_oob, ctr->n_skipped_zero_weight, ctr->n_clamped_w, ctr->n_updates};
+    unsigned long long *dstc[5] = {ctr->n_gridded, ctr->n_skipped_oob, ctr->n_skipped_zero_weight, ctr->n_clamped_w, ctr->n_updates};
 #pragma unroll
     for (int k = 0; k < 5; ++k) {
         const unsigned t = __reduce_add_sync(0xffffffffu, v5[k]);
-        if ((threadIdx.x & 31) == 0 && t) atomicAdd(dst[k] + (blockIdx.x * 8 + (threadIdx.x >> 5)) % kStatSlots, (unsigned long long)t);
+        if ((threadIdx.x & 31) == 0 && t) atomicAdd(dstc[k] + (blockIdx.x * 8 + (threadIdx.x >> 5)) % kStatSlots, (unsigned long long)t);
     }
 }
 
@@ -129,14 +189,14 @@ namespace {
 
 static size_t al(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct BlLayout { size_t off_counters, off_bucket2, off_bstart, off_cursor, off_blocksum, off_status, off_ib, off_perm, off_fscale, off_records, total; unsigned nb; };
+struct BlLayout { size_t off_counters, off_bucket2, off_bstart, off_cursor, off_blocksum, off_status, off_ib, off_perm, off_fscale, off_ctab, off_cblocksum, off_records, total; unsigned nb, nvblocks; };
 
 BlLayout bl_layout(int64_t nrow, int nchan, int n_ant, size_t rec_bytes) {
     BlLayout L{};
     L.nb = (unsigned)((int64_t)n_ant * (n_ant + 1) / 2);
     size_t o = 0;
     L.off_counters = o; o += al(sizeof(Counters));
-    L.off_bucket2 = o;  o += 256;
+    L.off_bucket2 = o;  o += 256;                       // class starts of the records: up to WPG_MAX_CLS + 1 words
     L.off_status = o;   o += 256;
     L.off_bstart = o;   o += al(((size_t)L.nb + 8) * 4);
     L.off_cursor = o;   o += al(((size_t)L.nb + 8) * 4);
@@ -144,6 +204,11 @@ BlLayout bl_layout(int64_t nrow, int nchan, int n_ant, size_t rec_bytes) {
     L.off_ib = o;       o += al((size_t)nrow * 4);
     L.off_perm = o;     o += al((size_t)nrow * 4);
     L.off_fscale = o;   o += al((size_t)nchan * 8);
+    // ragged stacks: records per (support class, block of 256 records), scanned class-major
+    L.nvblocks = (unsigned)(((size_t)nrow * nchan + 255) / 256);
+    const size_t nct = (size_t)WPG_MAX_CLS * L.nvblocks;
+    L.off_ctab = o;     o += al((nct + 8) * 4);
+    L.off_cblocksum = o; o += al(((nct + 1 + 4095) / 4096) * 4 + 8);
     L.off_records = o;  o += al((size_t)nrow * nchan * rec_bytes);
     L.total = o;
     return L;
@@ -217,7 +282,8 @@ extern "C" int wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const do
     PlaneTab tab; BinParams bp; WorkspaceLayout ws0;
     rc = wpg_make_plan(ctx, desc, nrow, nchan, prec, &tab, &bp, &ws0);
     if (rc) return rc;
-    if (bp.ncls != 1) return wpg_fail(ctx, WPG_EINVAL, "the baseline-ordered gridder takes uniform stacks only");
+    if ((int64_t)bp.ncls * ((nrow * nchan + 255) / 256) >= ((int64_t)1 << 31))
+        return wpg_fail(ctx, WPG_EINVAL, "too many visibilities for the per-class block table; chunk the input");
     const size_t recb = prec == WPG_F32 ? sizeof(Rec<float>) : sizeof(Rec<double>);
     const BlLayout L = bl_layout(nrow, nchan, n_ant, recb);
     if (!d_workspace || workspace_bytes < L.total)
@@ -233,19 +299,26 @@ extern "C" int wpg_grid_baseline_order(wpg_ctx *ctx, const void *d_vis, const do
     bl_chan_scale_kernel<<<(nchan + 255) / 256, 256, 0, s>>>(d_freq, nchan, fscale);
     Counters *ctr = (Counters *)(w + L.off_counters);
     const unsigned nbk = (unsigned)((nvis + 255) / 256);
+    unsigned *ctab = (unsigned *)(w + L.off_ctab);
+    if (nbk && bp.ncls > 1) {          // ragged stack: stable partition of the order by support class
+        bl_class_count_kernel<<<nbk, 256, 0, s>>>(d_uvw, fscale, tab, bp, (const unsigned *)(w + L.off_perm), ctab);
+        ctx->n_launches += 1;
+        rc = wpg_launch_exclusive_scan(ctx, ctab, (unsigned)bp.ncls * nbk, (unsigned *)(w + L.off_cblocksum), ctr);
+        if (rc) return rc;
+    }
     if (nbk) {
         if (prec == WPG_F32)
             bl_build_records_kernel<float><<<nbk, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp,
-                (const unsigned *)(w + L.off_perm), ctr, (Rec<float> *)(w + L.off_records), (unsigned *)(w + L.off_bucket2));
+                (const unsigned *)(w + L.off_perm), ctr, (Rec<float> *)(w + L.off_records), (unsigned *)(w + L.off_bucket2), ctab);
         else
             bl_build_records_kernel<double><<<nbk, 256, 0, s>>>((const float2 *)d_vis, d_uvw, d_weight, fscale, tab, bp,
-                (const unsigned *)(w + L.off_perm), ctr, (Rec<double> *)(w + L.off_records), (unsigned *)(w + L.off_bucket2));
+                (const unsigned *)(w + L.off_perm), ctr, (Rec<double> *)(w + L.off_records), (unsigned *)(w + L.off_bucket2), ctab);
     }
     ctx->n_launches += nbk ? 2 : 1;
     WPG_CUDA(ctx, cudaGetLastError());
     if ((rc = wpg_mark(ctx, 1))) return rc;
     if (nvis) {
-        // the gridder of wpg_grid.cu walks the records in this order: one class, key range [0, 1) = all records
+        // the gridder of wpg_grid.cu walks the records in this order: per class, key range [cls, cls + 1) = its records
         WorkspaceLayout ws{};
         ws.off_counters = L.off_counters; ws.off_hist = L.off_bucket2; ws.off_records = L.off_records;
         bp.dyn_keys = 0; bp.keys_per_class = 1; bp.nkeys = 1;

@@ -403,7 +403,8 @@ __device__ __forceinline__ void store_rec(Rec<double> *dst, double re, double im
 // advanced atomically once per run of equal keys: after this pass bucket_start[key] is the END of bucket key, i.e.
 // the array read one element earlier is the start array again — see wpg_launch_bin).  The record carries
 // weight * vis (R9, natural weighting), summed over the visibilities merged into it (compression).
-// NPOL = 1: Rec<TT>;  NPOL = 2 | 4: vis[row][chan][pol], one RecP<NPOL> record carries all correlations (fp32).
+// NPOL = 1: Rec<TT>;  NPOL = 2 | 4: vis[row][chan][pol], one RecP<NPOL> (fp32) / RecPD<NPOL> (fp64) record carries
+// all correlations.
 template <typename TT, int NPOL, bool QP2>
 __global__ void __launch_bounds__(256, NPOL == 1 ? 4 : 3)
 scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, const float *__restrict__ weight,
@@ -453,20 +454,22 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
     } else {
         // walk the thread's visibilities in order; a record is written when the next one starts a new record
         constexpr int NP = NPOL > 1 ? NPOL : 2;
-        RecP<NP> out;
+        using RP = typename RecPOf<TT, NP>::type;
+        RP out;
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) {
             if (key[j] == WPG_NO_KEY) continue;
             const float2 *src = vis + (size_t)V.i[j] * NP;
+            const TT w = (TT)wt[j];
 #pragma unroll
             for (int p = 0; p < NP; ++p) {
                 const float2 q = __ldg(src + p);
-                if (rhead[j]) out.v[p] = make_float2(wt[j] * q.x, wt[j] * q.y);
-                else { out.v[p].x += wt[j] * q.x; out.v[p].y += wt[j] * q.y; }
+                if (rhead[j]) { out.v[p].x = w * (TT)q.x; out.v[p].y = w * (TT)q.y; }
+                else { out.v[p].x += w * (TT)q.x; out.v[p].y += w * (TT)q.y; }
             }
             out.pos = pos[j]; out.koff = koff[j];
             const bool last = j + 1 == kVpt || key[j + 1 < kVpt ? j + 1 : j] == WPG_NO_KEY || rhead[j + 1 < kVpt ? j + 1 : j];
-            if (last) reinterpret_cast<RecP<NP> *>(rec_out)[dst[j]] = out;
+            if (last) reinterpret_cast<RP *>(rec_out)[dst[j]] = out;
         }
     }
 }
@@ -486,8 +489,8 @@ int wpg_launch_exclusive_scan(wpg_ctx *ctx, unsigned *hist, unsigned n, unsigned
     return WPG_OK;
 }
 
-// The binning passes (npol = 1: Rec<float | double> records; npol = 2 | 4: RecP<npol>, fp32 — positions do not depend
-// on the correlation, so only the scatter differs).
+// The binning passes (npol = 1: Rec<float | double> records; npol = 2 | 4: RecP<npol> / RecPD<npol> — positions do not
+// depend on the correlation, so only the scatter differs).
 static int launch_bin_passes(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
                              const double *d_freq, const PlaneTab &tab, const BinParams &bp,
                              const WorkspaceLayout &ws, wpg_prec prec, int npol, char *w) {
@@ -532,8 +535,10 @@ static int launch_bin_passes(wpg_ctx *ctx, const void *d_vis, const double *d_uv
             if (qp2) scatter_kernel<TT, NP, true><<<nb, 256, 0, s>>>(v, d_uvw, d_weight, fscale, tab, bp, ctr, hist, rec);  \
             else scatter_kernel<TT, NP, false><<<nb, 256, 0, s>>>(v, d_uvw, d_weight, fscale, tab, bp, ctr, hist, rec);     \
         } while (0)
-        if (npol == 4) WPG_SCATTER(float, 4);
-        else if (npol == 2) WPG_SCATTER(float, 2);
+        if (npol == 4 && prec == WPG_F32) WPG_SCATTER(float, 4);
+        else if (npol == 4) WPG_SCATTER(double, 4);
+        else if (npol == 2 && prec == WPG_F32) WPG_SCATTER(float, 2);
+        else if (npol == 2) WPG_SCATTER(double, 2);
         else if (prec == WPG_F32) WPG_SCATTER(float, 1);
         else WPG_SCATTER(double, 1);
 #undef WPG_SCATTER
@@ -550,6 +555,6 @@ int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const f
 }
 
 int wpg_launch_bin_pol(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight, const double *d_freq,
-                       const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, int npol, char *w) {
-    return launch_bin_passes(ctx, d_vis, d_uvw, d_weight, d_freq, tab, bp, ws, WPG_F32, npol, w);
+                       const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, wpg_prec prec, int npol, char *w) {
+    return launch_bin_passes(ctx, d_vis, d_uvw, d_weight, d_freq, tab, bp, ws, prec, npol, w);
 }

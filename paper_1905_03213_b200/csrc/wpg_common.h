@@ -54,6 +54,12 @@ static_assert(sizeof(Rec<double>) == 24, "fp64 record is 24 B");
 // window and the coefficient slice.
 template <int NPOL> struct RecP { float2 v[NPOL]; uint32_t pos, koff; };
 static_assert(sizeof(RecP<4>) == 40 && sizeof(RecP<2>) == 24, "polarised records are 8 NPOL + 8 bytes");
+struct Dpair { double x, y; };                                                    // (8-byte aligned, unlike double2)
+template <int NPOL> struct RecPD { Dpair v[NPOL]; uint32_t pos, koff; };        // fp64: 16 NPOL + 8 bytes
+static_assert(sizeof(RecPD<4>) == 72 && sizeof(RecPD<2>) == 40, "fp64 polarised records are 16 NPOL + 8 bytes");
+template <typename T, int NPOL> struct RecPOf;
+template <int NPOL> struct RecPOf<float, NPOL> { using type = RecP<NPOL>; };
+template <int NPOL> struct RecPOf<double, NPOL> { using type = RecPD<NPOL>; };
 
 // Device counters block at the head of the workspace.
 struct Counters {
@@ -142,8 +148,8 @@ void wpg_pswf_eval(const double *nu, int64_t n, double *out);     // wpg_pswf.cu
 int wpg_mark(wpg_ctx *ctx, int i);      // timing event i (0 start, 1 after binning / re-order, 2 after gridder) if option "timing"
 // launchers
 int wpg_launch_bin_pol(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight, const double *d_freq,
-                       const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, int npol, char *d_ws);
-int wpg_launch_grid_pol(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, int npol,
+                       const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, wpg_prec prec, int npol, char *d_ws);
+int wpg_launch_grid_pol(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, wpg_prec prec, int npol,
                         const void *d_kernels, void *d_grid, char *d_ws);
 int wpg_launch_exclusive_scan(wpg_ctx *ctx, unsigned *hist, unsigned n, unsigned *blocksum, Counters *ctr);
 int wpg_launch_bin(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,

@@ -374,6 +374,9 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         return (unsigned)(x & ~1) | ((unsigned)y << 16);
     };
 
+    U64 zero64;
+    asm volatile("mov.b64 %0, 0;" : "=l"(zero64));      // volatile: stays a register, not re-materialised at each use
+
     for (;;) {
         unsigned item = 0;
         if (lane == 0) item = atomicAdd(cursor, 1u);
@@ -403,10 +406,11 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
 #pragma unroll
         for (unsigned c = 0; c < 2; ++c) { fill(c); cp_async_commit(); }
 
+        constexpr unsigned kNoCell = 0xFFFFFFFFu;
         U64 acc0[NSLOT], acc1[NSLOT];                       // (re, im) sums of the pair's two cells
         unsigned qcur[NSLOT] = {};                          // (column | row << 16) of the pair's first cell
 #pragma unroll
-        for (int k = 0; k < NSLOT; ++k) { acc0[k] = acc1[k] = 0ull; qcur[k] = 0xFFFFFFFFu; }
+        for (int k = 0; k < NSLOT; ++k) { acc0[k] = acc1[k] = 0ull; qcur[k] = kNoCell; }
 
         // look-ahead ring (registers): coefficients, visibility and the lane-slot's cell of the DEPTH
         // records in flight
@@ -425,12 +429,13 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
             float2 *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
             // (two 8-byte reductions rather than one 16-byte red.v4: the latter wants both sums in one aligned
             // register quad, which costs register moves on every record)
+            // (the zero comes from a register: an immediate 64-bit zero costs four instructions per sum)
             asm volatile("{ .reg .f32 a, b, c, d;\n\t"
                          "mov.b64 {a, b}, %0; mov.b64 {c, d}, %1;\n\t"
                          "red.global.add.v2.f32 [%2], {a, b};\n\t"
                          "red.global.add.v2.f32 [%2 + 8], {c, d};\n\t"
-                         "mov.b64 %0, 0; mov.b64 %1, 0; }"
-                         : "+l"(acc0[k]), "+l"(acc1[k]) : "l"(g) : "memory");
+                         "mov.b64 %0, %3; mov.b64 %1, %3; }"
+                         : "+l"(acc0[k]), "+l"(acc1[k]) : "l"(g), "l"(zero64) : "memory");
         };
         // stage s <- record rp[0]: coefficient loads; the lane's offset inside the slice changes only
         // with the window (warp-uniform branch, taken once per run of equal window starts)
@@ -453,14 +458,14 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
                 }
 #pragma unroll
                 for (int k = 0; k < NSLOT; ++k) {
-                    qn[s][k] = act[k] && valid ? pos + dP[k] : 0xFFFFFFFFu;
+                    qn[s][k] = act[k] && valid ? pos + dP[k] : kNoCell;
                     ldg128(K + (koff + cP[k]), c0[s][k], c1[s][k]);
                 }
             } else {
 #pragma unroll
                 for (int k = 0; k < NSLOT; ++k) {
                     const unsigned d = offset_in_window(pos, k);
-                    qn[s][k] = act[k] && valid ? pos + d : 0xFFFFFFFFu;
+                    qn[s][k] = act[k] && valid ? pos + d : kNoCell;
                     const unsigned coff = (d >> 16) * (unsigned)S + (d & 0xFFFFu);
                     ldg128(K + (koff + (act[k] ? coff : 0u)), c0[s][k], c1[s][k]);
                 }
@@ -474,7 +479,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
 #pragma unroll
                 for (int k = 0; k < NSLOT; ++k) {
                     if (qn[s][k] != qcur[k]) {
-                        if (qcur[k] != 0xFFFFFFFFu) flush(k);      // (the sums are zero before the first window)
+                        if (qcur[k] != kNoCell) flush(k);      // (the sums are zero before the first window)
                         asm volatile("mov.b32 %0, %1;" : "+r"(qcur[k]) : "r"(qn[s][k]));    // tied: no second copy of qcur
                     }
                 }
@@ -524,7 +529,7 @@ grid_pairs_kernel(const Rec<float> *__restrict__ rec, const unsigned *__restrict
         }
 #pragma unroll
         for (int k = 0; k < NSLOT; ++k)
-            if (act[k] && qcur[k] != 0xFFFFFFFFu) flush(k);
+            if (act[k] && qcur[k] != kNoCell) flush(k);
         cp_async_wait<0>();
     }
 }
@@ -871,6 +876,163 @@ grid_cells_kernel(const Rec<T> *__restrict__ rec, const unsigned *__restrict__ b
     }
 }
 
+// ------------------------------------------------------------------------------------ cells, NPOL correlations
+// The general polarised gridder (data are row x channel x polarisation): any
+// support (even or odd, ragged stacks through the class loop), fp32 and fp64 (the paper runs both precisions
+// everywhere).  Structure of grid_cells_kernel with a runtime support: one cell per lane-slot, the
+// window's lane offsets tracked in the producer, the window split over `ws` work items of NSLOT lane-slot sets; the
+// NPOL correlations of a record share the coefficient load and the window bookkeeping.  grid[pol][N][N].
+template <typename T, int NPOL, int NSLOT, int DEPTH, int MINB>
+__global__ void __launch_bounds__(kRunThreads, MINB)
+grid_cells_pol_kernel(const typename RecPOf<T, NPOL>::type *__restrict__ rec, const unsigned *__restrict__ bucket_start,
+                      const unsigned *__restrict__ key_base, int cls, unsigned key_lo, unsigned key_hi, int S, unsigned magicS,
+                      unsigned ws, unsigned *__restrict__ cursor, const typename Cplx<T>::type *__restrict__ K,
+                      typename Cplx<T>::type *__restrict__ grid, int N, unsigned seg) {
+    using C = typename Cplx<T>::type;
+    using RP = typename RecPOf<T, NPOL>::type;
+    static_assert(kChunk % DEPTH == 0, "the look-ahead depth divides the chunk");
+    constexpr unsigned PIECES = sizeof(RP) / 8;
+    const int NC = S * S;
+    const int lane = threadIdx.x & 31;
+    if (key_base) { key_lo = __ldg(key_base + cls); key_hi = __ldg(key_base + cls + 1); }
+    const unsigned r_begin = __ldg(bucket_start + key_lo), r_end = __ldg(bucket_start + key_hi);
+    const unsigned nitems = ws * ((r_end - r_begin + seg - 1) / seg);
+    const size_t plane = (size_t)N * N;
+
+    __shared__ __align__(16) RP ring_all[kRunThreads / 32][kChunk * kRing];
+    RP *ring = ring_all[threadIdx.x >> 5];
+
+    int ra[NSLOT], rb[NSLOT];
+    bool act[NSLOT];
+    auto set_slots = [&](int part) {
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) {
+            int r = (part * NSLOT + k) * 32 + lane;
+            act[k] = r < NC;
+            r = act[k] ? r : 0;
+            rb[k] = r / S;
+            ra[k] = r - rb[k] * S;
+        }
+    };
+    auto fill = [&](unsigned i0, unsigned i1, unsigned c) {        // chunk c of the item into its ring slot, 8-byte pieces
+        const unsigned long long *g = reinterpret_cast<const unsigned long long *>(rec + i0 + c * kChunk);
+        unsigned long long *sm = reinterpret_cast<unsigned long long *>(ring + ((c * kChunk) & kRingMask));
+        const unsigned first = i0 + c * kChunk;
+        const unsigned npiece = first < i1 ? PIECES * min((unsigned)kChunk, i1 - first) : 0u;
+        for (unsigned q = lane; q < npiece; q += 32)
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(sm + q)), "l"(g + q) : "memory");
+    };
+
+    for (;;) {
+        unsigned item = 0;
+        if (lane == 0) item = atomicAdd(cursor, 1u);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= nitems) break;
+        set_slots((int)(item % ws)); item /= ws;
+        const unsigned i0 = r_begin + item * seg, i1 = min(i0 + seg, r_end);
+        const unsigned cnt = i1 - i0;
+
+        __syncwarp();
+#pragma unroll
+        for (unsigned c = 0; c < 2; ++c) { fill(i0, i1, c); cp_async_commit(); }
+
+        T accx[NSLOT][NPOL], accy[NSLOT][NPOL];
+        unsigned qcur[NSLOT];
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) {
+            qcur[k] = 0xFFFFFFFFu;
+#pragma unroll
+            for (int p = 0; p < NPOL; ++p) accx[k][p] = accy[k][p] = (T)0;
+        }
+        C cf[DEPTH][NSLOT];
+        T vre[DEPTH][NPOL], vim[DEPTH][NPOL];
+        unsigned qn[DEPTH][NSLOT];
+        unsigned posP = 0xFFFFFFFFu, dP[NSLOT], cP[NSLOT];
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k) dP[k] = cP[k] = 0;
+
+        auto flush = [&](int k) {
+            const unsigned q = qcur[k];
+            C *g = grid + ((q >> 16) * (unsigned)N + (q & 0xFFFFu));
+#pragma unroll
+            for (int p = 0; p < NPOL; ++p) flush_cell(g + p * plane, accx[k][p], accy[k][p]);
+        };
+        auto produce = [&](int s, const RP *rp) {
+#pragma unroll
+            for (int p = 0; p < NPOL; ++p) { vre[s][p] = rp->v[p].x; vim[s][p] = rp->v[p].y; }
+            const uint2 pk = *reinterpret_cast<const uint2 *>(&rp->pos);
+            const unsigned pos = pk.x, koff = pk.y;
+            if (__any_sync(0xffffffffu, pos != posP)) {      // offsets re-derived only when the window start changes
+                const unsigned j0u = pos & 0xFFFFu, j0v = pos >> 16;
+                const int ju = (int)(j0u - ((j0u * magicS) >> 20) * (unsigned)S);
+                const int jv = (int)(j0v - ((j0v * magicS) >> 20) * (unsigned)S);
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    int x = ra[k] - ju; x += x < 0 ? S : 0;
+                    int y = rb[k] - jv; y += y < 0 ? S : 0;
+                    dP[k] = (unsigned)x | ((unsigned)y << 16);
+                    cP[k] = act[k] ? (unsigned)(y * S + x) : 0u;
+                }
+                posP = pos;
+            }
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) {
+                qn[s][k] = act[k] ? pos + dP[k] : 0xFFFFFFFFu;
+                cf[s][k] = __ldg(K + (koff + cP[k]));
+            }
+        };
+        auto consume = [&](int s) {
+            bool any = false;
+#pragma unroll
+            for (int k = 0; k < NSLOT; ++k) any |= qn[s][k] != qcur[k];
+            if (__any_sync(0xffffffffu, any)) {
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    if (qn[s][k] != qcur[k]) {
+                        if (qcur[k] != 0xFFFFFFFFu) flush(k);
+                        asm volatile("mov.b32 %0, %1;" : "+r"(qcur[k]) : "r"(qn[s][k]));
+                    }
+                }
+            }
+#pragma unroll
+            for (int p = 0; p < NPOL; ++p) {
+                const T re = vre[s][p], im = vim[s][p];
+#pragma unroll
+                for (int k = 0; k < NSLOT; ++k) {
+                    accx[k][p] = fma(re, cf[s][k].x, accx[k][p]); accx[k][p] = fma(-im, cf[s][k].y, accx[k][p]);
+                    accy[k][p] = fma(re, cf[s][k].y, accy[k][p]); accy[k][p] = fma(im, cf[s][k].x, accy[k][p]);
+                }
+            }
+        };
+        auto enter_chunk = [&](unsigned c) {
+            __syncwarp();
+            fill(i0, i1, c + 2);
+            cp_async_commit();
+            cp_async_wait<2>();
+            __syncwarp();
+        };
+
+        enter_chunk(0);
+#pragma unroll
+        for (int s = 0; s < DEPTH; ++s)
+            if ((unsigned)s < cnt) produce(s, ring + s);
+        for (unsigned j = 0; j < cnt; j += DEPTH) {
+            const unsigned jp = j + DEPTH;
+            if ((jp & (kChunk - 1)) == 0 && jp < cnt) enter_chunk(jp / kChunk);
+            const RP *rp = ring + (jp & kRingMask);
+#pragma unroll
+            for (int s = 0; s < DEPTH; ++s) {
+                if (j + s < cnt) consume(s);
+                if (jp + s < cnt) produce(s, rp + s);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NSLOT; ++k)
+            if (act[k] && qcur[k] != 0xFFFFFFFFu) flush(k);
+        cp_async_wait<0>();
+    }
+}
+
 template <typename T, int SCT, int NSLOT, int DEPTH, int MINB, int WS = 1>
 int launch_cells(wpg_ctx *ctx, cudaStream_t strm, const BinParams &bp, const WorkspaceLayout &ws, const void *K, void *grid, char *w,
                    int cls, int S) {
@@ -1024,25 +1186,48 @@ int wpg_launch_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const
     return WPG_OK;
 }
 
-int wpg_launch_grid_pol(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, int npol,
-                        const void *K, void *grid, char *w) {
+int wpg_launch_grid_pol(wpg_ctx *ctx, const PlaneTab &tab, const BinParams &bp, const WorkspaceLayout &ws, wpg_prec prec,
+                        int npol, const void *K, void *grid, char *w) {
     if (bp.nrow == 0) return WPG_OK;
-    const int S = tab.clsS[0];
     Counters *ctr = (Counters *)(w + ws.off_counters);
     const unsigned seg = ctx->opt_segment ? (unsigned)ctx->opt_segment : 256u;
     const unsigned *bs = (const unsigned *)(w + ws.off_hist);
     cudaStream_t s = ctx->stream;
+    const bool aligned = ((uintptr_t)K & 15) == 0;
+    // the fp32 pair gridders for uniform supports 8 and 16 (one LDG.128 feeds 2 * npol updates)
+    if (prec == WPG_F32 && bp.ncls == 1 && aligned && !ctx->opt_no_pairs && (tab.clsS[0] == 8 || tab.clsS[0] == 16)) {
+        const int S = tab.clsS[0];
 #define WPG_POL(SS, NS, DD, MB, NP, WW)                                                                                 \
-    grid_pairs_pol_kernel<SS, NS, DD, MB, NP, WW><<<ctx->sm_count * (ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MB),     \
-        kRunThreads, 0, s>>>((const RecP<NP> *)(w + ws.off_records), bs, 0u, bp.keys_per_class, &ctr->cursor[0],        \
-                             (const float2 *)K, (float2 *)grid, bp.N, seg)
-    if (S == 8 && npol == 4) WPG_POL(8, 1, 4, 3, 4, 1);
-    else if (S == 8 && npol == 2) WPG_POL(8, 1, 4, 3, 2, 1);
-    else if (S == 16 && npol == 4) WPG_POL(16, 1, 4, 3, 4, 4);      // window split over four work items
-    else if (S == 16 && npol == 2) WPG_POL(16, 2, 2, 2, 2, 2);
-    else return wpg_fail(ctx, WPG_EINVAL, "the polarised gridder takes uniform supports 8 or 16 and 2 or 4 correlations");
+        grid_pairs_pol_kernel<SS, NS, DD, MB, NP, WW><<<ctx->sm_count * (ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MB), \
+            kRunThreads, 0, s>>>((const RecP<NP> *)(w + ws.off_records), bs, 0u, bp.keys_per_class, &ctr->cursor[0],        \
+                                 (const float2 *)K, (float2 *)grid, bp.N, seg)
+        if (S == 8 && npol == 4) WPG_POL(8, 1, 4, 3, 4, 1);
+        else if (S == 8 && npol == 2) WPG_POL(8, 1, 4, 3, 2, 1);
+        else if (S == 16 && npol == 4) WPG_POL(16, 1, 4, 3, 4, 4);      // window split over four work items
+        else WPG_POL(16, 2, 2, 2, 2, 2);
 #undef WPG_POL
-    ctx->n_launches += 1;
+        ctx->n_launches += 1;
+        WPG_CUDA(ctx, cudaGetLastError());
+        return WPG_OK;
+    }
+    // everything else — other supports, ragged stacks (one launch per support class), fp64 — through the cell gridder
+    for (int cls = bp.ncls - 1; cls >= 0; --cls) {
+        const int S = tab.clsS[cls];
+        const unsigned magicS = (1u << 20) / (unsigned)S + 1u;
+        const unsigned nslot = (unsigned)(S * S + 31) / 32;
+#define WPG_POLC(TT, NP, NS, DD, MB)                                                                                    \
+        grid_cells_pol_kernel<TT, NP, NS, DD, MB><<<ctx->sm_count * (ctx->opt_ctas_per_sm ? ctx->opt_ctas_per_sm : MB),     \
+            kRunThreads, 0, s>>>((const typename RecPOf<TT, NP>::type *)(w + ws.off_records), bs,                          \
+                                 bp.dyn_keys ? ctr->key_base : nullptr, cls, (unsigned)cls * bp.keys_per_class,            \
+                                 (unsigned)(cls + 1) * bp.keys_per_class, S, magicS, (nslot + NS - 1) / NS, &ctr->cursor[cls], \
+                                 (const typename Cplx<TT>::type *)K, (typename Cplx<TT>::type *)grid, bp.N, seg)
+        if (prec == WPG_F32 && npol == 4) WPG_POLC(float, 4, 2, 2, 2);
+        else if (prec == WPG_F32) WPG_POLC(float, 2, 2, 2, 3);
+        else if (npol == 4) WPG_POLC(double, 4, 1, 2, 2);
+        else WPG_POLC(double, 2, 2, 2, 2);
+#undef WPG_POLC
+        ctx->n_launches += 1;
+    }
     WPG_CUDA(ctx, cudaGetLastError());
     return WPG_OK;
 }

@@ -99,8 +99,8 @@ def load():
     lib.wpg_degrid_workspace_bytes.argtypes = [cint]; lib.wpg_degrid_workspace_bytes.restype = sz
     lib.wpg_degrid.argtypes = [vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, vp, sz, ctypes.POINTER(i64)]
     lib.wpg_degrid.restype = cint
-    lib.wpg_grid_pol_workspace_bytes.argtypes = [vp, i64, cint, cint, kd]; lib.wpg_grid_pol_workspace_bytes.restype = sz
-    lib.wpg_grid_pol.argtypes = [vp, vp, vp, vp, vp, i64, cint, cint, vp, kd, vp, vp, sz, stp]; lib.wpg_grid_pol.restype = cint
+    lib.wpg_grid_pol_workspace_bytes.argtypes = [vp, i64, cint, cint, kd, cint]; lib.wpg_grid_pol_workspace_bytes.restype = sz
+    lib.wpg_grid_pol.argtypes = [vp, vp, vp, vp, vp, i64, cint, cint, vp, kd, cint, vp, vp, sz, stp]; lib.wpg_grid_pol.restype = cint
     lib.wpg_microbench.argtypes = [vp, cint, cint, vp, sz, ctypes.POINTER(dbl)]; lib.wpg_microbench.restype = cint
     _lib = lib
     return lib
@@ -360,23 +360,23 @@ class Context:
 
     # ---- polarisation axis
     def grid_pol(self, vis, uvw, weight, freq, stack, grid=None, workspace=None, stats=False):
-        """vis [nrow][nchan][npol] complex64 -> grid [npol][N][N] (accumulated into), fp32 stacks of support 8 / 16."""
+        """vis [nrow][nchan][npol] complex64 -> grid [npol][N][N] (accumulated into), in the stack's precision."""
         t = self.torch
         assert vis.dtype == t.complex64 and vis.dim() == 3 and vis.is_cuda and vis.is_contiguous()
         nrow, nchan, npol = vis.shape
-        assert uvw.shape == (nrow, 3) and weight.numel() == nrow * nchan and freq.shape[0] == nchan and stack.prec == F32
+        assert uvw.shape == (nrow, 3) and weight.numel() == nrow * nchan and freq.shape[0] == nchan
         N = stack.desc.grid_N
         if grid is None:
-            grid = t.zeros((npol, N, N), dtype=t.complex64, device=self.device)
-        if workspace is None:
-            need = int(self.lib.wpg_grid_pol_workspace_bytes(self.h, nrow, nchan, npol, ctypes.byref(stack.desc)))
-            if need == 0:
-                raise WpgError(EINVAL, "wpg_grid_pol_workspace_bytes: bad arguments (npol 2|4, uniform support 8|16)")
-            workspace = self._temp(need)
+            grid = t.zeros((npol, N, N), dtype=t.complex64 if stack.prec == F32 else t.complex128, device=self.device)
         self._check_grid(grid, stack, lead=(npol,))
+        if workspace is None:
+            need = int(self.lib.wpg_grid_pol_workspace_bytes(self.h, nrow, nchan, npol, ctypes.byref(stack.desc), stack.prec))
+            if need == 0:
+                raise WpgError(EINVAL, "wpg_grid_pol_workspace_bytes: bad arguments (npol must be 2 or 4)")
+            workspace = self._temp(need)
         st = Stats()
         self._check(self.lib.wpg_grid_pol(self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(),
-                                          nrow, nchan, npol, stack.data.data_ptr(), ctypes.byref(stack.desc),
+                                          nrow, nchan, npol, stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec,
                                           grid.data_ptr(), workspace.data_ptr(), workspace.numel(),
                                           ctypes.byref(st) if stats else None))
         return grid, (st.as_dict() if stats else None)

@@ -120,8 +120,30 @@ def test_grid_in_baseline_order_matches_oracle(ctx):
             gh = gg.cpu().numpy()
             assert np.isfinite(gh).all()
             assert float(np.max(np.abs(gh - ref)) / np.max(np.abs(ref))) <= TOL[prec]
-    # ragged stacks are refused
-    sup = np.array([8, 8, 10, 10, 12, 12, 8, 8], np.int32)
-    ks = ctx.wkernel_build(Nw, w_max, sup, Q, N, cell, wpgrid.F32)
-    with pytest.raises(wpgrid.WpgError):
-        ctx.grid_baseline_order(*d, n_ant, ks)
+    # ragged stack on the same tracks: the order is partitioned by support class (stably), one gridder launch per class
+    sup = np.array([8, 8, 10, 10, 12, 12, 8, 9], np.int32)
+    st_r = owk.build_stack(Nw, w_max, sup, Q, N, cell)
+    ref_r, rstats_r = ogrid.grid(uvw, vis, wt, freq, st_r)
+    for prec in (wpgrid.F32, wpgrid.F64):
+        ks = ctx.stack_from_host(st_r.data, Nw, w_max, sup, Q, N, cell, prec)
+        g, s = ctx.grid_baseline_order(*d, n_ant, ks, stats=True)
+        assert s == rstats_r
+        err = float(np.max(np.abs(g.cpu().numpy() - ref_r)) / np.max(np.abs(ref_r)))
+        assert err <= TOL[prec], (prec, err)
+
+
+def test_baseline_order_ragged_config4_layout(ctx):
+    """The paper's order on config 4's layout (512 SKA-low-like stations, 8 channels, N = 8192, w-dependent support —
+    PAPER.md:192 (6) names SKA-size images as the case to keep in mind): 2 dumps, every support class of the input."""
+    wl = synth.config4(n_dump=2, values="random")
+    sup = owk.ragged_support(wl.Nw, wl.w_max, wl.grid_N, wl.cell, 8, 32)
+    st = owk.build_stack(wl.Nw, wl.w_max, sup, wl.oversample, wl.grid_N, wl.cell)
+    assert len(set(sup.tolist())) >= 4
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    a1, a2 = synth.track_antennas(wl.notes["n_ant"], wl.uvw.shape[0])
+    d = [torch.from_numpy(x).cuda() for x in (wl.vis, wl.uvw, wl.weight, wl.freq, a1, a2)]
+    ks = ctx.stack_from_host(st.data, st.Nw, st.w_max, sup, st.oversample, st.grid_N, st.cell, wpgrid.F32)
+    g, s = ctx.grid_baseline_order(*d, wl.notes["n_ant"], ks, stats=True)
+    assert s == rstats
+    err = float(np.max(np.abs(g.cpu().numpy() - ref)) / np.max(np.abs(ref)))
+    assert err <= TOL[wpgrid.F32], err
