@@ -200,6 +200,17 @@ int  wpg_degrid(wpg_ctx *ctx, const void *d_grid, const double *d_uvw, const dou
                 const void *d_kernels, const wpg_kdesc *desc, wpg_prec prec, void *d_vis_out,
                 void *d_workspace, size_t workspace_bytes, int64_t *h_counts2_or_null);
 
+/* ---- multi-GPU: shard the rows, one reduce of the grid -------------------------
+ * The paper's decomposition: the visibility rows are split among the ranks, every rank
+ * grids its rows into a private full-size grid, and the grids are summed on the master.  The library side of it is
+ * this host function; the sum is ONE collective of the N x N complex grid, issued by the binding through
+ * torch.distributed (NCCL reduce over NVLink on GPUs; paper_1905_03213_b200/sharded.py).
+ * Rows [*row0, *row1) of rank `rank` of `world`: contiguous, disjoint, covering [0, nrow) exactly, sizes equal to
+ * within one unit; the unit is one row, or `row_block` rows (a time step of time-major data) if row_block > 0, so that
+ * a shard keeps whole time steps and the binning's rows-per-time-step hint stays valid inside it.
+ * Host only; returns WPG_EINVAL for world < 1, rank outside [0, world), nrow < 0 or row_block < 0. */
+int  wpg_shard_rows(int64_t nrow, int64_t row_block, int world, int rank, int64_t *row0, int64_t *row1);
+
 /* Machine-limit microbenchmarks (instrumentation; SURVEY.md §8(d) wants fractions of MEASURED peaks).
  * which: 0 = red.global.add.v2.f32, a warp per 256-byte row segment at a pseudo-random place of the buffer (the
  *            naive gridder's pattern; "write access ... in an atomic manner");

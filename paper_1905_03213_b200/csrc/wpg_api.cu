@@ -456,3 +456,17 @@ extern "C" int wpg_grid_host(wpg_ctx *ctx, const void *h_vis, const double *h_uv
     WPG_CUDA(ctx, cudaStreamSynchronize(s));
     return WPG_OK;
 }
+
+// Row range of one rank (see wpgrid.h): units of row_block rows (or single rows) dealt out as evenly as possible,
+// the first (units % world) ranks take one unit more.
+extern "C" int wpg_shard_rows(int64_t nrow, int64_t row_block, int world, int rank, int64_t *row0, int64_t *row1) {
+    if (!row0 || !row1 || world < 1 || rank < 0 || rank >= world || nrow < 0 || row_block < 0) return WPG_EINVAL;
+    const int64_t unit = row_block > 0 ? row_block : 1;
+    const int64_t units = (nrow + unit - 1) / unit;
+    const int64_t base = units / world, extra = units % world;
+    const int64_t u0 = rank * base + std::min<int64_t>(rank, extra);
+    const int64_t u1 = u0 + base + (rank < extra ? 1 : 0);
+    *row0 = std::min(nrow, u0 * unit);
+    *row1 = std::min(nrow, u1 * unit);
+    return WPG_OK;
+}

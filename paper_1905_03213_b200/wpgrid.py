@@ -22,7 +22,7 @@ EXPORTS = (
     "wpg_grid", "wpg_grid_naive", "wpg_grid_host", "wpg_bin", "wpg_dirty_image_workspace_bytes",
     "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms", "wpg_microbench",
     "wpg_baseline_workspace_bytes", "wpg_baseline_reorder", "wpg_grid_baseline_order",
-    "wpg_degrid_workspace_bytes", "wpg_degrid", "wpg_grid_pol_workspace_bytes", "wpg_grid_pol",
+    "wpg_degrid_workspace_bytes", "wpg_degrid", "wpg_grid_pol_workspace_bytes", "wpg_grid_pol", "wpg_shard_rows",
 )
 
 
@@ -102,6 +102,7 @@ def load():
     lib.wpg_grid_pol_workspace_bytes.argtypes = [vp, i64, cint, cint, kd, cint]; lib.wpg_grid_pol_workspace_bytes.restype = sz
     lib.wpg_grid_pol.argtypes = [vp, vp, vp, vp, vp, i64, cint, cint, vp, kd, cint, vp, vp, sz, stp]; lib.wpg_grid_pol.restype = cint
     lib.wpg_microbench.argtypes = [vp, cint, cint, vp, sz, ctypes.POINTER(dbl)]; lib.wpg_microbench.restype = cint
+    lib.wpg_shard_rows.argtypes = [i64, i64, cint, cint, ctypes.POINTER(i64), ctypes.POINTER(i64)]; lib.wpg_shard_rows.restype = cint
     _lib = lib
     return lib
 

@@ -1,6 +1,8 @@
 """GPU <-> oracle parity (-m gpu).  Everything goes through the C ABI (libwpgrid.so) via the
 thin binding.  Tolerances (north_star / DESIGN.md R17): max|g - g_oracle| <= 1e-4 max|g_oracle|
 for fp32 and <= 1e-10 max|g_oracle| for fp64; integer outputs (counters, records) bit-exact."""
+import os
+
 import numpy as np
 import pytest
 
@@ -556,3 +558,22 @@ def test_odd_grid_size_and_small_grids(ctx):
         assert rstats["n_gridded"] > 100 and rstats["n_skipped_oob"] > 100
         wl = synth.Workload("odd%d" % N, uvw, freq, vis, wt, N, cell, 3, 25.0, S, Q)
         check_all_paths(ctx, wl, st, ref, rstats)
+
+
+def test_sharded_gridding_one_rank_nccl(ctx):
+    """paper_1905_03213_b200/sharded.py on the GPU with a one-rank NCCL group (the box has one GPU): the rank's shard
+    is everything, the reduce is the identity; the multi-rank logic is covered on CPU (tests/test_sharded_gloo.py)."""
+    import torch.distributed as dist
+    from paper_1905_03213_b200 import sharded
+    wl = synth.config2(nvis=2016 * 70 + 3)
+    st = oracle_stack(wl)
+    ref, rstats = ogrid.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=4)
+    ks = upload(ctx, st, wpgrid.F32)
+    dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % (33000 + os.getpid() % 2000), rank=0, world_size=1,
+                            device_id=torch.device("cuda", 0))
+    try:
+        g, s = sharded.grid_sharded(ctx, *dev(wl), ks, dist, rows="all", row_block=wl.notes["row_block"], stats=True)
+        assert s == rstats and relerr(g.cpu().numpy(), ref) <= TOL[wpgrid.F32]
+    finally:
+        dist.destroy_process_group()
+        ctx.set_option("row_block", 0)
