@@ -267,6 +267,20 @@ def aggregate_value(n_updates_per_rank, world, ms_step_max):
 
 
 # --------------------------------------------------------------------------- the CUDA arm
+def measured_peaks(ctx, f32):
+    """(ALU TFLOP/s, L1 GB/s, HBM GB/s, HBM source): the first two measured in this run through wpg_microbench
+    (fma.rn.f32x2 | fma.rn.f64 issue rate; L1-resident 16-byte loads), HBM from the driver's MEASURED_PEAKS.json."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            hbm_gbs = float(json.load(f)["hbm_gbs"]); hbm_src = "measured (MEASURED_PEAKS.json)"
+    except (OSError, ValueError, KeyError):
+        hbm_gbs, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
+    fma_per_s, _ = ctx.microbench(3 if f32 else 4, 20000 if f32 else 10000)          # packed f32x2 FMAs (2 FMA) | f64 FMAs
+    alu_tflops = fma_per_s * (4.0 if f32 else 2.0) / 1e12
+    l1_loads_per_s, _ = ctx.microbench(2, 4000)                                       # L1-resident 16-byte loads
+    return alu_tflops, l1_loads_per_s * 16 / 1e9, hbm_gbs, hbm_src
+
+
 def traffic_from_profiles(workload, prec):
     """dram bytes per gridder launch from the committed ncu --set full capture, if there is one."""
     path = os.path.join(ROOT, "profiles", "gridder_traffic.json")
@@ -403,15 +417,7 @@ def run_b200(args):
     # (MEASURED_PEAKS.json hbm_gbs), never derived.
     f32 = prec == wpgrid.F32
     coef_bytes, rec_bytes = (8, 16) if f32 else (16, 24)
-    try:
-        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-            hbm_gbs = float(json.load(f)["hbm_gbs"]); hbm_src = "measured (MEASURED_PEAKS.json)"
-    except (OSError, ValueError, KeyError):
-        hbm_gbs, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
-    fma_per_s, _ = ctx.microbench(3 if f32 else 4, 20000 if f32 else 10000)          # packed f32x2 FMAs (2 FMA) | f64 FMAs
-    alu_tflops = fma_per_s * (4.0 if f32 else 2.0) / 1e12
-    l1_loads_per_s, _ = ctx.microbench(2, 4000)                                       # L1-resident 16-byte loads
-    l1_gbs = l1_loads_per_s * 16 / 1e9
+    alu_tflops, l1_gbs, hbm_gbs, hbm_src = measured_peaks(ctx, f32)
     upd_per_s = n_updates / (grid_ms * 1e-3)
     bounds = {"alu": alu_tflops * 1e12 / FLOP_PER_UPDATE,
               "l1": l1_gbs * 1e9 / coef_bytes,
@@ -477,17 +483,40 @@ def run_b200(args):
         dist.destroy_process_group()
 
 
+def timed_loop(step, args, dist, dev, local):
+    """Warm-up, then K timed steps bracketed by barrier + synchronize, CUDA events, max over ranks, clocks sampled."""
+    import torch
+    for _ in range(max(args.warmup, 3)):
+        step()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier(); sampler.start(); e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record(); barrier()
+    clocks = sampler.stop()
+    return max_over_ranks(e0.elapsed_time(e1), dist, dev) / args.steps, clocks
+
+
 def run_pol(args, ctx, wl, stack, d_uvw, d_wt, d_freq, dev, world, rank, dist):
     """Polarised gridding, not the headline metric: a step = zero-fill of the npol grids +
     binning + polarised gridder + one dirty image per correlation."""
     import torch
+    from paper_1905_03213_b200 import wpgrid
     npol = args.npol
+    f32 = stack.prec == wpgrid.F32
     nrow, nchan, N = d_uvw.shape[0], d_freq.shape[0], wl.grid_N
     gen = torch.Generator(device=dev).manual_seed(3)
     vis = torch.view_as_complex(torch.randn((nrow, nchan, npol, 2), dtype=torch.float32, device=dev, generator=gen))
     need = int(ctx.lib.wpg_grid_pol_workspace_bytes(ctx.h, nrow, nchan, npol, ctypes.byref(stack.desc), stack.prec))
     ws = torch.empty(need, dtype=torch.uint8, device=dev)
-    grid = torch.zeros((npol, N, N), dtype=torch.complex64, device=dev)
+    grid = torch.zeros((npol, N, N), dtype=torch.complex64 if f32 else torch.complex128, device=dev)
     iws = torch.empty(int(ctx.lib.wpg_dirty_image_workspace_bytes(N, stack.prec)), dtype=torch.uint8, device=dev)
     wsum = float(wl.weight.sum())
     _, stats = ctx.grid_pol(vis, d_uvw, d_wt, d_freq, stack, grid=torch.zeros_like(grid), workspace=ws, stats=True)
@@ -499,54 +528,83 @@ def run_pol(args, ctx, wl, stack, d_uvw, d_wt, d_freq, dev, world, rank, dist):
         for p in range(npol):
             ctx.dirty_image(grid[p], stack, wsum, workspace=iws)
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    torch.cuda.synchronize(); ctx.phase_ms()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record(); torch.cuda.synchronize()
-    ms = max_over_ranks(e0.elapsed_time(e1), dist, dev) / args.steps
+    step(); torch.cuda.synchronize(); ctx.phase_ms()
+    launches0 = ctx.launch_count()
+    ms, clocks = timed_loop(step, args, dist, dev, dev.index or 0)
+    launches = (ctx.launch_count() - launches0) * args.steps // (args.steps + max(args.warmup, 3))
     bin_ms, grid_ms = ctx.phase_ms()
     if rank == 0:
+        # one coefficient (8 | 16 B) feeds npol updates: L1 bytes per update shrink by npol, the ALU work does not
+        alu_tflops, l1_gbs, hbm_gbs, hbm_src = measured_peaks(ctx, f32)
         ups = n_updates / (grid_ms * 1e-3)
-        print(json.dumps({"metric": METRIC + ", %d correlations" % npol, "unit": UNIT, "value": aggregate_value(n_updates, world, ms),
-                          "ms_per_step": ms, "n_gpus": world, "steps": args.steps, "dtype": "f32", "data": "synthetic",
-                          "config": dict(workload_config(wl, "f32"), npol=npol), "stats": stats,
-                          "roofline": {"bound": "alu", "binning_ms": bin_ms, "gridder_ms": grid_ms, "gridder_updates_per_s": ups,
-                                       "achieved": ups * FLOP_PER_UPDATE / 1e12,
-                                       "peak": SM_COUNT * FP32_LANES * 2 * SM_MAX_GHZ / 1e3,
-                                       "frac": ups * FLOP_PER_UPDATE / 1e12 / (SM_COUNT * FP32_LANES * 2 * SM_MAX_GHZ / 1e3)}}))
+        coef = (8 if f32 else 16) / npol
+        bounds = {"alu": alu_tflops * 1e12 / FLOP_PER_UPDATE, "l1": l1_gbs * 1e9 / coef}
+        binding = min(bounds, key=bounds.get)
+        ach, peak, unit = ((ups * FLOP_PER_UPDATE / 1e12, alu_tflops, "TFLOP/s") if binding == "alu"
+                           else (ups * coef / 1e9, l1_gbs, "GB/s"))
+        out = {"metric": METRIC + ", %d correlations" % npol, "unit": UNIT, "value": aggregate_value(n_updates, world, ms),
+               "ms_per_step": ms, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+               "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": args.prec, "data": "synthetic (positions of the workload, N(0,1) visibilities per correlation)",
+               "config": dict(workload_config(wl, args.prec), npol=npol), "stats": stats, "clocks": clocks,
+               "gpu_launches": int(launches),
+               "roofline": {"bound": binding, "kernel": "polarised gridder", "achieved": ach, "peak": peak, "unit": unit,
+                            "frac": ach / peak, "traffic": None, "peak_source": "measured in this run (wpg_microbench)",
+                            "binning_ms": bin_ms, "gridder_ms": grid_ms, "gridder_updates_per_s": ups,
+                            "bounds_updates_per_s": bounds}}
+        print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
 
 
 def run_degrid(args, ctx, wl, stack, d_uvw, d_freq, prec, dev, world, rank, dist):
-    """Degridding throughput (not the headline metric): K timed wpg_degrid calls of one random grid."""
+    """Degridding throughput (not the headline metric): a step = one wpg_degrid of a random grid
+    for all visibilities of the workload.  A gather: per update one grid value and one coefficient (16 | 32 B) come
+    through L1 — that feed is the bound, half the gridder's."""
     import torch
     from paper_1905_03213_b200 import wpgrid
+    f32 = prec == wpgrid.F32
     N = wl.grid_N
     gen = torch.Generator(device=dev).manual_seed(1)
-    g = torch.randn((N, N), dtype=torch.complex64 if prec == wpgrid.F32 else torch.complex128, device=dev, generator=gen)
+    g = torch.randn((N, N), dtype=torch.complex64 if f32 else torch.complex128, device=dev, generator=gen)
     out, cnt = ctx.degrid(g, d_uvw, d_freq, stack, counts=True)
     sup = stack.support.astype(np.int64)
     # updates = sum S_p^2 over predicted visibilities: exact for uniform stacks
     n_updates = cnt["n_predicted"] * int(sup[0]) ** 2 if stack.uniform else None
-    for _ in range(max(args.warmup, 3)):
+
+    def step():
         ctx.degrid(g, d_uvw, d_freq, stack, out=out)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        ctx.degrid(g, d_uvw, d_freq, stack, out=out)
-    e1.record(); torch.cuda.synchronize()
-    ms = max_over_ranks(e0.elapsed_time(e1), dist, dev) / args.steps
+
+    launches0 = ctx.launch_count()
+    ms, clocks = timed_loop(step, args, dist, dev, dev.index or 0)
+    launches = (ctx.launch_count() - launches0) * args.steps // (args.steps + max(args.warmup, 3))
     if rank == 0:
-        print(json.dumps({"metric": "grid-point updates/sec (degridding, vis x support^2)", "unit": UNIT,
-                          "value": None if n_updates is None else aggregate_value(n_updates, world, ms),
-                          "ms_per_step": ms, "n_gpus": world, "steps": args.steps, "dtype": args.prec, "data": "synthetic",
-                          "config": workload_config(wl, args.prec), "counts": cnt, "op": "degrid"}))
+        line = {"metric": "grid-point updates/sec (degridding, vis x support^2)", "unit": UNIT,
+                "value": None if n_updates is None else aggregate_value(n_updates, world, ms),
+                "ms_per_step": ms, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.prec,
+                "data": "synthetic (positions of the workload, N(0,1) grid)", "config": workload_config(wl, args.prec),
+                "counts": cnt, "op": "degrid", "clocks": clocks, "gpu_launches": int(launches)}
+        if n_updates is not None:
+            alu_tflops, l1_gbs, hbm_gbs, hbm_src = measured_peaks(ctx, f32)
+            ups = n_updates / (ms * 1e-3)
+            per_upd = 16 if f32 else 32
+            line["roofline"] = {"bound": "l1", "kernel": "degrid_kernel", "achieved": ups * per_upd / 1e9, "peak": l1_gbs,
+                                "unit": "GB/s", "frac": ups * per_upd / 1e9 / l1_gbs, "traffic": None,
+                                "algorithmic": "%d B per update through L1 (grid value + coefficient)" % per_upd,
+                                "peak_source": "measured in this run (wpg_microbench: L1-resident LDG.128)",
+                                "alu_frac": ups * FLOP_PER_UPDATE / 1e12 / alu_tflops}
+            if not args.no_cpu_baseline and world == 1:
+                from oracle import gridder as ogrid
+                st = oracle_stack(wl)
+                rows = min(wl.uvw.shape[0], 400_000)
+                gh = g.cpu().numpy().astype(np.complex128)
+                t0 = time.perf_counter()
+                _, c = ogrid.degrid(wl.uvw[:rows], wl.freq, st, gh)
+                dt = time.perf_counter() - t0
+                line["cpu_baseline"] = {"value": c["n_predicted"] * int(sup[0]) ** 2 / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                        "sample": "oracle_degrid (plain C, fp64, 1 thread) on the first %d rows, %.1f s" % (rows, dt)}
+        print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
 

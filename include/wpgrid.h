@@ -99,8 +99,12 @@ int  wpg_ragged_support(int Nw, double w_max, int grid_N, double cell, int overs
 int64_t wpg_wkernel_elems(int Nw, int support, int oversample);          /* Nw*Q*Q*S*S */
 /* Build the stack described by *desc (uniform if desc->support == NULL) into d_kernels_out
  * (caller-allocated, c64 for WPG_F32 — rounded from fp64 — or c128 for WPG_F64).
- * All arithmetic is fp64 on the device. */
-int  wpg_wkernel_build(wpg_ctx *ctx, const wpg_kdesc *desc, wpg_prec prec, void *d_kernels_out);
+ * All arithmetic is fp64 on the device, including the taper and the normalisation scalar (K5): the call allocates
+ * nothing, copies nothing from the host and does not synchronise; temporaries live in the caller's workspace
+ * (wpg_wkernel_workspace_bytes: the image-plane samples, twiddles and tables of the largest support group). */
+size_t wpg_wkernel_workspace_bytes(const wpg_kdesc *desc);
+int  wpg_wkernel_build(wpg_ctx *ctx, const wpg_kdesc *desc, wpg_prec prec, void *d_kernels_out,
+                       void *d_workspace, size_t workspace_bytes);
 
 /* ---- a1 + a2: binning and gridding — PAPER.md:30, 62-84 ------------------------------------ */
 /* Bytes of device scratch wpg_grid needs for this problem size. */

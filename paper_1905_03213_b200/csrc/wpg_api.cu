@@ -56,7 +56,6 @@ extern "C" void wpg_destroy(wpg_ctx *ctx) {
     if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
     for (int i = 0; i < 4; ++i) if (ctx->ev_chunk[i]) cudaEventDestroy(ctx->ev_chunk[i]);
     if (ctx->plan) cufftDestroy(ctx->plan);
-    if (ctx->d_taper) cudaFree(ctx->d_taper);
     if (ctx->d_host_scratch) cudaFree(ctx->d_host_scratch);
     delete ctx;
 }

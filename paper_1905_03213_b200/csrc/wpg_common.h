@@ -107,8 +107,6 @@ struct wpg_ctx {
     cudaEvent_t ev_start = nullptr, ev_chunk[4] = {nullptr, nullptr, nullptr, nullptr};
     // cuFFT plan cache
     cufftHandle plan = 0; int plan_N = 0; int plan_prec = -1;
-    // taper table cache for dirty_image
-    double *d_taper = nullptr; int taper_N = 0;
     // device scratch of the host-buffer variant (grow-only)
     void *d_host_scratch = nullptr; size_t host_scratch_bytes = 0;
 };
@@ -143,7 +141,8 @@ struct DeviceGuard {
 int wpg_check_desc(wpg_ctx *ctx, const wpg_kdesc *d);
 int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg_prec prec,
                   PlaneTab *tab, BinParams *bp, WorkspaceLayout *ws);
-void wpg_pswf_eval(const double *nu, int64_t n, double *out);     // wpg_pswf.cu (host)
+void wpg_pswf_eval(const double *nu, int64_t n, double *out);     // wpg_wkernel.cu (host)
+int wpg_launch_taper(wpg_ctx *ctx, double *d_out, int n, double step);   // psi(2 (j - n/2) step), j < n, on the device
 
 int wpg_mark(wpg_ctx *ctx, int i);      // timing event i (0 start, 1 after binning / re-order, 2 after gridder) if option "timing"
 // launchers

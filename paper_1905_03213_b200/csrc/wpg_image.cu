@@ -40,9 +40,11 @@ const char *cufft_str(cufftResult r) {
 
 }  // namespace
 
+// workspace: the transform's output [N][N] complex, then the taper table psi[N] (fp64)
+static size_t fft_bytes(int N, wpg_prec prec) { return (((size_t)N * N * (prec == WPG_F32 ? 8 : 16)) + 255) & ~(size_t)255; }
 extern "C" size_t wpg_dirty_image_workspace_bytes(int grid_N, wpg_prec prec) {
     if (grid_N < 2) return 0;
-    return (size_t)grid_N * grid_N * (prec == WPG_F32 ? 8 : 16);
+    return fft_bytes(grid_N, prec) + (size_t)grid_N * 8;
 }
 
 extern "C" int wpg_dirty_image(wpg_ctx *ctx, const void *d_grid, const wpg_kdesc *desc, double weight_sum,
@@ -67,26 +69,19 @@ extern "C" int wpg_dirty_image(wpg_ctx *ctx, const void *d_grid, const wpg_kdesc
     }
     cufftResult r = cufftSetStream(ctx->plan, ctx->stream);
     if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftSetStream: %s", cufft_str(r));
-    if (ctx->taper_N != N) {
-        if (ctx->d_taper) { cudaFree(ctx->d_taper); ctx->d_taper = nullptr; ctx->taper_N = 0; }
-        std::vector<double> nu(N), t(N);
-        double fov = (double)N * desc->cell;
-        for (int j = 0; j < N; ++j) nu[j] = 2.0 * ((j - N / 2) * desc->cell) / fov;
-        wpg_pswf_eval(nu.data(), N, t.data());
-        WPG_CUDA(ctx, cudaMalloc((void **)&ctx->d_taper, (size_t)N * 8));
-        WPG_CUDA(ctx, cudaMemcpy(ctx->d_taper, t.data(), (size_t)N * 8, cudaMemcpyHostToDevice));
-        ctx->taper_N = N;
-    }
+    // taper psi(2 l_j / FoV), l_j = (j - N/2) cell: evaluated on the device into the caller's workspace (N values)
+    double *d_taper = (double *)((char *)d_workspace + fft_bytes(N, prec));
+    if ((rc = wpg_launch_taper(ctx, d_taper, N, 1.0 / N))) return rc;
     dim3 gr((N + 255) / 256, N);
     cudaStream_t s = ctx->stream;
     if (prec == WPG_F32) {
         r = cufftExecC2C(ctx->plan, (cufftComplex *)const_cast<void *>(d_grid), (cufftComplex *)d_workspace, CUFFT_INVERSE);
         if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftExecC2C: %s", cufft_str(r));
-        correct_kernel<float2, float><<<gr, 256, 0, s>>>((const float2 *)d_workspace, (float *)d_image, ctx->d_taper, N, 1.0 / weight_sum);
+        correct_kernel<float2, float><<<gr, 256, 0, s>>>((const float2 *)d_workspace, (float *)d_image, d_taper, N, 1.0 / weight_sum);
     } else {
         r = cufftExecZ2Z(ctx->plan, (cufftDoubleComplex *)const_cast<void *>(d_grid), (cufftDoubleComplex *)d_workspace, CUFFT_INVERSE);
         if (r != CUFFT_SUCCESS) return wpg_fail(ctx, WPG_ECUDA, "cufftExecZ2Z: %s", cufft_str(r));
-        correct_kernel<double2, double><<<gr, 256, 0, s>>>((const double2 *)d_workspace, (double *)d_image, ctx->d_taper, N, 1.0 / weight_sum);
+        correct_kernel<double2, double><<<gr, 256, 0, s>>>((const double2 *)d_workspace, (double *)d_image, d_taper, N, 1.0 / weight_sum);
     }
     ctx->n_launches += 1;
     WPG_CUDA(ctx, cudaGetLastError());

@@ -18,7 +18,7 @@ OK, EINVAL, ENOMEM, ECUDA = 0, -1, -2, -3
 
 EXPORTS = (
     "wpg_create", "wpg_destroy", "wpg_last_error", "wpg_version", "wpg_set_option", "wpg_taper",
-    "wpg_ragged_support", "wpg_wkernel_elems", "wpg_wkernel_build", "wpg_grid_workspace_bytes",
+    "wpg_ragged_support", "wpg_wkernel_elems", "wpg_wkernel_workspace_bytes", "wpg_wkernel_build", "wpg_grid_workspace_bytes",
     "wpg_grid", "wpg_grid_naive", "wpg_grid_host", "wpg_bin", "wpg_dirty_image_workspace_bytes",
     "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms", "wpg_microbench",
     "wpg_baseline_workspace_bytes", "wpg_baseline_reorder", "wpg_grid_baseline_order",
@@ -78,7 +78,8 @@ def load():
     lib.wpg_ragged_support.argtypes = [cint, dbl, cint, dbl, cint, cint, cint, vp, vp]
     lib.wpg_ragged_support.restype = cint
     lib.wpg_wkernel_elems.argtypes = [cint, cint, cint]; lib.wpg_wkernel_elems.restype = i64
-    lib.wpg_wkernel_build.argtypes = [vp, kd, cint, vp]; lib.wpg_wkernel_build.restype = cint
+    lib.wpg_wkernel_workspace_bytes.argtypes = [kd]; lib.wpg_wkernel_workspace_bytes.restype = sz
+    lib.wpg_wkernel_build.argtypes = [vp, kd, cint, vp, vp, sz]; lib.wpg_wkernel_build.restype = cint
     lib.wpg_grid_workspace_bytes.argtypes = [vp, i64, cint, kd, cint]; lib.wpg_grid_workspace_bytes.restype = sz
     lib.wpg_grid.argtypes = [vp, vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, vp, sz, stp]
     lib.wpg_grid.restype = cint
@@ -214,7 +215,11 @@ class Context:
         t = self.torch
         d, sup, off, uniform = make_desc(Nw, w_max, support, oversample, grid_N, cell)
         K = t.empty(int(off[-1]), dtype=t.complex64 if prec == F32 else t.complex128, device=self.device)
-        self._check(self.lib.wpg_wkernel_build(self.h, ctypes.byref(d), prec, K.data_ptr()))
+        need = int(self.lib.wpg_wkernel_workspace_bytes(ctypes.byref(d)))
+        if need == 0:
+            raise WpgError(EINVAL, "wpg_wkernel_workspace_bytes: bad kernel descriptor")
+        ws = self._temp(need)
+        self._check(self.lib.wpg_wkernel_build(self.h, ctypes.byref(d), prec, K.data_ptr(), ws.data_ptr(), ws.numel()))
         return Stack(K, d, prec, sup, off, uniform)
 
     def stack_from_host(self, data, Nw, w_max, support, oversample, grid_N, cell, prec=F32):
