@@ -137,6 +137,10 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     bp->vis_block = 0;
     if (ctx->opt_row_block > 0 && ctx->opt_row_block * nchan < ((int64_t)1 << 31) && nvis >= 64 * ctx->opt_row_block * nchan)
         bp->vis_block = (uint32_t)(ctx->opt_row_block * nchan);
+    bp->row_block = bp->vis_block ? (uint32_t)ctx->opt_row_block : 0u;
+    bp->vis_nbx = (bp->vis_block + 255u) / 256u;
+    bp->chan_shift = -1;
+    for (int sft = 0; sft < 16; ++sft) if ((1 << sft) == nchan) bp->chan_shift = sft;
     bp->N = d->grid_N; bp->Q = d->oversample; bp->Nw = d->Nw;
     bp->w_max = d->w_max;
     bp->dw = 2.0 * d->w_max / (double)d->Nw;

@@ -131,11 +131,12 @@ __device__ __forceinline__ VisIdx vis_indices(const BinParams &P) {
     VisIdx V;
     const unsigned nvis = (unsigned)(P.nrow * P.nchan);             // < 2^32 - 2 (wpg_make_plan)
     if (P.vis_block) {
-        const unsigned nbx = (P.vis_block + 255u) / 256u, dg = blockIdx.x / nbx;      // (uniform: one division per block)
+        const unsigned nbx = P.vis_nbx, dg = blockIdx.x / nbx;             // (uniform: one division per block)
         const unsigned x = (blockIdx.x - dg * nbx) * 256u + threadIdx.x;
-        const unsigned xr = P.nchan > 1 ? x / (unsigned)P.nchan : x;      // one division per thread, not per visibility
+        // one division per thread, not per visibility — a shift for a power-of-two channel count
+        const unsigned xr = P.chan_shift >= 0 ? x >> P.chan_shift : x / (unsigned)P.nchan;
         const int ch = (int)(x - xr * (unsigned)P.nchan);
-        const unsigned rows_per_step = P.vis_block / (unsigned)P.nchan;
+        const unsigned rows_per_step = P.row_block;
 #pragma unroll
         for (int j = 0; j < kVpt; ++j) {
             const unsigned long long step = (unsigned long long)dg * kVpt + j;
@@ -151,7 +152,7 @@ __device__ __forceinline__ VisIdx vis_indices(const BinParams &P) {
             const unsigned long long i = (unsigned long long)blockIdx.x * (256 * kVpt) + j * 256 + threadIdx.x;
             const bool ok = i < nvis;
             V.i[j] = ok ? (unsigned)i : 0xFFFFFFFFu;
-            const unsigned r = P.nchan > 1 ? (unsigned)i / (unsigned)P.nchan : (unsigned)i;
+            const unsigned r = P.chan_shift >= 0 ? (unsigned)i >> P.chan_shift : (unsigned)i / (unsigned)P.nchan;
             V.row[j] = r; V.ch[j] = (int)((unsigned)i - r * (unsigned)P.nchan);
         }
     }

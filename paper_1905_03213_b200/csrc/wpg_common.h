@@ -28,6 +28,8 @@ struct PlaneTab {
 struct BinParams {
     int64_t nrow;
     int nchan;
+    uint32_t row_block, vis_nbx;   // with vis_block: rows per time step; ceil(vis_block / 256) (host-computed: no divisions in the kernels)
+    int chan_shift;                // log2 nchan if nchan is a power of two, else -1
     uint32_t vis_block;            // 0, or visibilities per time step (row_block * nchan): a binning thread then takes
                                    // the SAME baseline/channel at consecutive time steps (see wpg_vis_index)
     int N, Q, Nw;
