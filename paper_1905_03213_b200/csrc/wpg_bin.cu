@@ -214,6 +214,7 @@ template <bool QP2>
 __device__ __forceinline__ Located locate_vis(const RawVis &v, const uint2 *s_tab, const uint4 *s_ck, const BinParams &P) {
     Located L; L.key = WPG_NO_KEY; L.pos = L.koff = 0; L.S = 0; L.clamped = false;
     int p, j0u, j0v, ou, ov, S;
+    uint2 tab_e = make_uint2(0u, 0u);
     bool inside, clamped, risk = !QP2;
     if (QP2) {
         const double u = __dmul_rn(v.um, v.f), vv = __dmul_rn(v.vm, v.f), w = __dmul_rn(v.wm, v.f);     // G1
@@ -224,7 +225,8 @@ __device__ __forceinline__ Located locate_vis(const RawVis &v, const uint2 *s_ta
             const double qd = wpg_div_const(__dadd_rn(w, P.w_max), P.dw, P.rdw);
             p = min(max(floor_magic(qd, 1048576.0, risk), 0), P.Nw - 1);
         }
-        S = P.ncls == 1 ? P.S0 : (int)(s_tab[p].y & 0xFFu);
+        if (P.ncls > 1) tab_e = s_tab[p];                   // {plane offset, S | class << 8}: one read, used twice
+        S = P.ncls == 1 ? P.S0 : (int)(tab_e.y & 0xFFu);
         const int c = (S - 2) * P.Q / 2;
         const double Qd = (double)P.Q, lim = 1073741824.0;
         // G3.  x * Q is exact for Q = 2^k, so the fused form rounds once, like the written two-step form.  Far outside
@@ -242,6 +244,7 @@ __device__ __forceinline__ Located locate_vis(const RawVis &v, const uint2 *s_ta
         const int4 o = locate_exact(v.um, v.vm, v.wm, v.f, P, s_tab);
         p = o.x & 0xFFFF; S = (o.x >> 16) & 0xFF; inside = (o.x >> 24) & 1; clamped = (o.x >> 25) & 1;
         j0u = o.y; j0v = o.z; ou = o.w & 0xFF; ov = o.w >> 8;
+        if (P.ncls > 1) tab_e = s_tab[p];
     }
     if (!inside) return L;
     L.S = S; L.clamped = clamped;
@@ -249,10 +252,9 @@ __device__ __forceinline__ Located locate_vis(const RawVis &v, const uint2 *s_ta
         L.key = (unsigned)j0u * (unsigned)P.nkg + ((unsigned)j0v >> P.kshift);
         L.koff = (unsigned)(((p * P.Q + ov) * P.Q + ou) * S * S);
     } else {
-        const uint2 e = s_tab[p];
-        const uint4 ck = s_ck[e.y >> 8];
+        const uint4 ck = s_ck[tab_e.y >> 8];
         L.key = ck.x + (unsigned)j0u * ck.y + ((unsigned)j0v >> ck.z);
-        L.koff = e.x + (unsigned)((ov * P.Q + ou) * S * S);
+        L.koff = tab_e.x + (unsigned)((ov * P.Q + ou) * S * S);
     }
     L.pos = (unsigned)j0u | ((unsigned)j0v << 16);
     return L;
