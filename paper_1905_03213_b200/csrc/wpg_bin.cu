@@ -191,61 +191,14 @@ __device__ __forceinline__ void key_runs(const unsigned (&key)[kVpt], const unsi
 struct RawVis { double um, vm, wm, f; float wt; };
 struct Located { unsigned key, pos, koff; int S; bool clamped; };
 
-__device__ __forceinline__ int floor_magic(double t, double lim, bool &risk) {
-    // |t| < lim <= 2^30: t + M holds rint(t) in its low word; t - rint(t) is exact.  One ulp of t is below 2.4e-7 there.
-    // Outside the range (also NaN) the flag is raised and the value returned is not used.
-    const double M = 6755399441055744.0;
-    const double tm = __dadd_rn(t, M);
-    const double d = __dadd_rn(t, -__dadd_rn(tm, -M));           // in [-0.5, 0.5]
-    risk |= !(fabs(d) >= 1e-6) | !(fabs(t) < lim);
-    return __double2loint(tm) - (d < 0.0 ? 1 : 0);
-}
-
-// the rare exact path (IEEE divisions, the written order), out of line so that the fast path stays compact;
-// returns {p | S << 16 | inside << 24 | clamped << 25, j0u, j0v, ou | ov << 8}
-__device__ __noinline__ int4 locate_exact(double um, double vm, double wm, double f, const BinParams &P, const uint2 *s_tab) {
-    const SmemPlaneTab T{s_tab, nullptr};
-    const VisPos r = wpg_locate(um, vm, wm, f, P, T);
-    return make_int4(r.p | (r.S << 16) | (r.inside ? 1 << 24 : 0) | (r.clamped ? 1 << 25 : 0), r.j0u, r.j0v, r.ou | (r.ov << 8));
-}
-
 // QP2: the oversampling factor is a power of two (else the general form is used throughout)
 template <bool QP2>
 __device__ __forceinline__ Located locate_vis(const RawVis &v, const uint2 *s_tab, const uint4 *s_ck, const BinParams &P) {
     Located L; L.key = WPG_NO_KEY; L.pos = L.koff = 0; L.S = 0; L.clamped = false;
-    int p, j0u, j0v, ou, ov, S;
-    uint2 tab_e = make_uint2(0u, 0u);
-    bool inside, clamped, risk = !QP2;
-    if (QP2) {
-        const double u = __dmul_rn(v.um, v.f), vv = __dmul_rn(v.vm, v.f), w = __dmul_rn(v.wm, v.f);     // G1
-        clamped = fabs(w) > P.w_max;                                                                      // G2
-        p = 0;
-        if (P.dw > 0.0) {               // (uniform branch)
-            // (far outside [-w_max, w_max], and for NaN, the flag is raised: the exact path clamps)
-            const double qd = wpg_div_const(__dadd_rn(w, P.w_max), P.dw, P.rdw);
-            p = min(max(floor_magic(qd, 1048576.0, risk), 0), P.Nw - 1);
-        }
-        if (P.ncls > 1) tab_e = s_tab[p];                   // {plane offset, S | class << 8}: one read, used twice
-        S = P.ncls == 1 ? P.S0 : (int)(tab_e.y & 0xFFu);
-        const int c = (S - 2) * P.Q / 2;
-        const double Qd = (double)P.Q, lim = 1073741824.0;
-        // G3.  x * Q is exact for Q = 2^k, so the fused form rounds once, like the written two-step form.  Far outside
-        // any grid (also NaN) the flag is raised and the exact path reports "outside".
-        const double tu = __fma_rn(__dadd_rn(wpg_div_const(u, P.du, P.rdu), P.halfN), Qd, 0.5);
-        const double tv = __fma_rn(__dadd_rn(wpg_div_const(vv, P.du, P.rdu), P.halfN), Qd, 0.5);
-        const int Yu = floor_magic(tu, lim, risk) - c;
-        const int Yv = floor_magic(tv, lim, risk) - c;
-        j0u = Yu >> P.qshift; ou = Yu & (P.Q - 1);
-        j0v = Yv >> P.qshift; ov = Yv & (P.Q - 1);
-        const unsigned lim_j = (unsigned)(P.N - S);
-        inside = (unsigned)j0u <= lim_j && (unsigned)j0v <= lim_j;                                       // G4
-    }
-    if (risk) {
-        const int4 o = locate_exact(v.um, v.vm, v.wm, v.f, P, s_tab);
-        p = o.x & 0xFFFF; S = (o.x >> 16) & 0xFF; inside = (o.x >> 24) & 1; clamped = (o.x >> 25) & 1;
-        j0u = o.y; j0v = o.z; ou = o.w & 0xFF; ov = o.w >> 8;
-        if (P.ncls > 1) tab_e = s_tab[p];
-    }
+    const LeanPos r = wpg_locate_lean<QP2>(v.um, v.vm, v.wm, v.f, P, s_tab);
+    const int p = r.p, j0u = r.j0u, j0v = r.j0v, ou = r.ou, ov = r.ov, S = r.S;
+    const bool inside = r.inside, clamped = r.clamped;
+    const uint2 tab_e = r.tab_e;
     if (!inside) return L;
     L.S = S; L.clamped = clamped;
     if (P.ncls == 1) {

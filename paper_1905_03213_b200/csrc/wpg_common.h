@@ -256,6 +256,76 @@ __device__ __forceinline__ VisPos wpg_locate(double um, double vm, double wm, do
     return r;
 }
 
+// ---------------------------------------------------------------------------------------------
+// The lean form of wpg_locate used by the hot passes (binning, degridding).  Straight-line code: quotients by
+// Markstein's sequence (wpg_div_const), floor() through the 2^52 + 2^51 rounding constant instead of the conversion
+// pipe, and ONE flag that says whether any of the three values whose floor is taken lies within 1e-6 of an integer (or
+// outside the range where the trick is valid).  Only then — a few visibilities in a million — the written form with
+// IEEE divisions is evaluated out of line (wpg_locate), so that G6 holds whatever the constant-divisor sequence does
+// in its last bit.
+__device__ __forceinline__ int wpg_floor_magic(double t, double lim, bool &risk) {
+    // |t| < lim <= 2^30: t + M holds rint(t) in its low word; t - rint(t) is exact.  One ulp of t is below 2.4e-7 there.
+    // Outside the range (also NaN) the flag is raised and the value returned is not used.
+    const double M = 6755399441055744.0;
+    const double tm = __dadd_rn(t, M);
+    const double d = __dadd_rn(t, -__dadd_rn(tm, -M));           // in [-0.5, 0.5]
+    risk |= !(fabs(d) >= 1e-6) | !(fabs(t) < lim);
+    return __double2loint(tm) - (d < 0.0 ? 1 : 0);
+}
+
+// the rare exact path, out of line so that the fast path stays compact;
+// returns {p | S << 16 | inside << 24 | clamped << 25, j0u, j0v, ou | ov << 8}
+static __device__ __noinline__ int4 wpg_locate_exact(double um, double vm, double wm, double f, const BinParams &P, const uint2 *s_tab) {
+    const SmemPlaneTab T{s_tab, nullptr};
+    VisPos r;
+    if (P.ncls == 1) {                    // uniform stack: no table in shared memory
+        struct OneS { int s; __device__ int S(int) const { return s; } };
+        r = wpg_locate(um, vm, wm, f, P, OneS{P.S0});
+    } else {
+        r = wpg_locate(um, vm, wm, f, P, T);
+    }
+    return make_int4(r.p | (r.S << 16) | (r.inside ? 1 << 24 : 0) | (r.clamped ? 1 << 25 : 0), r.j0u, r.j0v, r.ou | (r.ov << 8));
+}
+
+// s_tab: the packed per-plane table in shared memory (ragged stacks; not read for uniform stacks).  tab_e: its entry
+// for the plane (ragged stacks).  QP2: the oversampling factor is a power of two (else the general form throughout).
+struct LeanPos { int p, S, j0u, j0v, ou, ov; bool inside, clamped; uint2 tab_e; };
+template <bool QP2>
+__device__ __forceinline__ LeanPos wpg_locate_lean(double um, double vm, double wm, double f, const BinParams &P, const uint2 *s_tab) {
+    LeanPos r; r.p = 0; r.S = 0; r.j0u = r.j0v = r.ou = r.ov = 0; r.inside = false; r.clamped = false; r.tab_e = make_uint2(0u, 0u);
+    bool risk = !QP2;
+    if (QP2) {
+        const double u = __dmul_rn(um, f), vv = __dmul_rn(vm, f), w = __dmul_rn(wm, f);                  // G1
+        r.clamped = fabs(w) > P.w_max;                                                                    // G2
+        if (P.dw > 0.0) {               // (uniform branch)
+            // (far outside [-w_max, w_max], and for NaN, the flag is raised: the exact path clamps)
+            const double qd = wpg_div_const(__dadd_rn(w, P.w_max), P.dw, P.rdw);
+            r.p = min(max(wpg_floor_magic(qd, 1048576.0, risk), 0), P.Nw - 1);
+        }
+        if (P.ncls > 1) r.tab_e = s_tab[r.p];               // {plane offset, S | class << 8}
+        r.S = P.ncls == 1 ? P.S0 : (int)(r.tab_e.y & 0xFFu);
+        const int c = (r.S - 2) * P.Q / 2;
+        const double Qd = (double)P.Q, lim = 1073741824.0;
+        // G3.  x * Q is exact for Q = 2^k, so the fused form rounds once, like the written two-step form.  Far outside
+        // any grid (also NaN) the flag is raised and the exact path reports "outside".
+        const double tu = __fma_rn(__dadd_rn(wpg_div_const(u, P.du, P.rdu), P.halfN), Qd, 0.5);
+        const double tv = __fma_rn(__dadd_rn(wpg_div_const(vv, P.du, P.rdu), P.halfN), Qd, 0.5);
+        const int Yu = wpg_floor_magic(tu, lim, risk) - c;
+        const int Yv = wpg_floor_magic(tv, lim, risk) - c;
+        r.j0u = Yu >> P.qshift; r.ou = Yu & (P.Q - 1);
+        r.j0v = Yv >> P.qshift; r.ov = Yv & (P.Q - 1);
+        const unsigned lim_j = (unsigned)(P.N - r.S);
+        r.inside = (unsigned)r.j0u <= lim_j && (unsigned)r.j0v <= lim_j;                                 // G4
+    }
+    if (risk) {
+        const int4 o = wpg_locate_exact(um, vm, wm, f, P, s_tab);
+        r.p = o.x & 0xFFFF; r.S = (o.x >> 16) & 0xFF; r.inside = (o.x >> 24) & 1; r.clamped = (o.x >> 25) & 1;
+        r.j0u = o.y; r.j0v = o.z; r.ou = o.w & 0xFF; r.ov = o.w >> 8;
+        if (P.ncls > 1) r.tab_e = s_tab[r.p];
+    }
+    return r;
+}
+
 template <typename Tab>
 __device__ __forceinline__ uint32_t wpg_koff(const VisPos &r, const BinParams &P, const Tab &T) {
     return (uint32_t)(T.off(r.p) + (r.ov * P.Q + r.ou) * r.S * r.S);
