@@ -75,6 +75,10 @@ int  wpg_version(void);
  * baseline at consecutive time steps, whose samples mostly hit the same grid point, and
  * updates the bucket counter once per run instead of once per visibility.  A hint only: any value gives
  * the same result.
+ * "compress" 0/1 (default 1): record compression — a binning thread's consecutive
+ * visibilities with the same plane, window start and sub-cell offsets share one sorted record carrying the sum of their
+ * weight * vis; the grid is unchanged (gridding is linear), the counters still count visibilities.  Effective with
+ * "row_block" (consecutive samples of one baseline and channel).
  * Unknown name -> WPG_EINVAL. */
 int  wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value);
 
@@ -227,7 +231,8 @@ int  wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_
 /* ---- a3: dirty image — PAPER.md:52, 88 (IFFT of the grid), R11 (grid correction) ---------- */
 size_t wpg_dirty_image_workspace_bytes(int grid_N, wpg_prec prec);
 /* image[jm][jl] = Re(centred inverse FFT of grid) * N^2-normalised / weight_sum / taper;
- * d_image real fp32|fp64 [N][N]; d_grid is not modified. */
+ * d_image real fp32|fp64 [N][N]; d_grid is not modified.  Workspace (caller's): the transform's output and the taper
+ * table, evaluated on the device at every call; the context keeps only the cuFFT plan.  Does not synchronise. */
 int  wpg_dirty_image(wpg_ctx *ctx, const void *d_grid, const wpg_kdesc *desc, double weight_sum,
                      wpg_prec prec, void *d_image, void *d_workspace, size_t workspace_bytes);
 
