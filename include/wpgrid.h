@@ -75,6 +75,9 @@ int  wpg_version(void);
  * baseline at consecutive time steps, whose samples mostly hit the same grid point, and
  * updates the bucket counter once per run instead of once per visibility.  A hint only: any value gives
  * the same result.
+ * "bin_tile" (with "row_block"; default 16, rounded down to a power of two): consecutive blocks of the binning passes
+ * take this many successive groups of time steps of the same 256 baselines / channels, so that the blocks resident
+ * together hit the same bucket counters and record stretches while those are still in L2.
  * "compress" 0/1 (default 1): record compression — a binning thread's consecutive
  * visibilities with the same plane, window start and sub-cell offsets share one sorted record carrying the sum of their
  * weight * vis; the grid is unchanged (gridding is linear), the counters still count visibilities.  Effective with

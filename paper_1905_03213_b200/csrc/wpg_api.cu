@@ -72,6 +72,7 @@ extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
     else if (!strcmp(name, "timing")) { ctx->opt_timing = value != 0; }
     else if (!strcmp(name, "no_pairs")) { ctx->opt_no_pairs = value != 0; }
     else if (!strcmp(name, "compress")) { ctx->opt_compress = value != 0; }
+    else if (!strcmp(name, "bin_tile")) { if (value < 0 || value > 65536) return wpg_fail(ctx, WPG_EINVAL, "bin_tile must be 0..65536"); ctx->opt_bin_tile = (int)value; }
     else if (!strcmp(name, "row_block")) { if (value < 0) return wpg_fail(ctx, WPG_EINVAL, "row_block must be >= 0"); ctx->opt_row_block = value; }
     else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
     return WPG_OK;
@@ -139,6 +140,12 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
         bp->vis_block = (uint32_t)(ctx->opt_row_block * nchan);
     bp->row_block = bp->vis_block ? (uint32_t)ctx->opt_row_block : 0u;
     bp->vis_nbx = (bp->vis_block + 255u) / 256u;
+    bp->vis_ngroups = bp->vis_block ? (uint32_t)(((nvis + bp->vis_block - 1) / bp->vis_block + 3) / 4) : 0u;     // kVpt = 4 (wpg_bin.cu)
+    // block tile of the binning passes: a power of two, default 16, raised until the number of tiles fits grid.y
+    bp->vis_tile_shift = 4;
+    if (ctx->opt_bin_tile > 0) { bp->vis_tile_shift = 0; while ((2u << bp->vis_tile_shift) <= (uint32_t)ctx->opt_bin_tile) bp->vis_tile_shift++; }
+    while (bp->vis_tile_shift < 30 && ((bp->vis_ngroups + (1u << bp->vis_tile_shift) - 1) >> bp->vis_tile_shift) > 65535u) bp->vis_tile_shift++;
+    bp->vis_tile = 1u << bp->vis_tile_shift;
     bp->chan_shift = -1;
     for (int sft = 0; sft < 16; ++sft) if ((1 << sft) == nchan) bp->chan_shift = sft;
     bp->N = d->grid_N; bp->Q = d->oversample; bp->Nw = d->Nw;

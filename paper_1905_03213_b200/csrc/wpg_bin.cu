@@ -33,7 +33,7 @@ __device__ __forceinline__ void block_count(Counters *ctr, unsigned flags, unsig
         unsigned long long *dst = threadIdx.x == 0 ? ctr->n_gridded : threadIdx.x == 1 ? ctr->n_skipped_oob
                                 : threadIdx.x == 2 ? ctr->n_skipped_zero_weight : threadIdx.x == 3 ? ctr->n_clamped_w
                                 : ctr->n_updates;
-        atomicAdd(dst + blockIdx.x % kStatSlots, (unsigned long long)s_cnt[threadIdx.x]);
+        atomicAdd(dst + (blockIdx.x + blockIdx.y) % kStatSlots, (unsigned long long)s_cnt[threadIdx.x]);
     }
 }
 
@@ -131,8 +131,14 @@ __device__ __forceinline__ VisIdx vis_indices(const BinParams &P) {
     VisIdx V;
     const unsigned nvis = (unsigned)(P.nrow * P.nchan);             // < 2^32 - 2 (wpg_make_plan)
     if (P.vis_block) {
-        const unsigned nbx = P.vis_nbx, dg = blockIdx.x / nbx;             // (uniform: one division per block)
-        const unsigned x = (blockIdx.x - dg * nbx) * 256u + threadIdx.x;
+        // Block order: tiles of vis_tile groups of time steps; inside a tile consecutive blocks — the ones resident
+        // together — take the SAME 256 baselines / channels at successive time groups.  A baseline's track crosses a
+        // window in ~10 samples, so these blocks hit the same bucket counters and append to the same stretches of the
+        // sorted records while those are still in L2; across tiles the inputs are still read front to back.
+        // (grid.y = tile, grid.x = (block of 256 baselines / channels) * vis_tile + group inside the tile; vis_tile = 2^k)
+        const unsigned bx = blockIdx.x >> P.vis_tile_shift;
+        const unsigned dg = blockIdx.y * P.vis_tile + (blockIdx.x & (P.vis_tile - 1u));
+        const unsigned x = bx * 256u + threadIdx.x;
         // one division per thread, not per visibility — a shift for a power-of-two channel count
         const unsigned xr = P.chan_shift >= 0 ? x >> P.chan_shift : x / (unsigned)P.nchan;
         const int ch = (int)(x - xr * (unsigned)P.nchan);
@@ -198,16 +204,16 @@ __device__ __forceinline__ Located locate_vis(const RawVis &v, const uint2 *s_ta
     const LeanPos r = wpg_locate_lean<QP2>(v.um, v.vm, v.wm, v.f, P, s_tab);
     const int p = r.p, j0u = r.j0u, j0v = r.j0v, ou = r.ou, ov = r.ov, S = r.S;
     const bool inside = r.inside, clamped = r.clamped;
-    const uint2 tab_e = r.tab_e;
     if (!inside) return L;
     L.S = S; L.clamped = clamped;
     if (P.ncls == 1) {
         L.key = (unsigned)j0u * (unsigned)P.nkg + ((unsigned)j0v >> P.kshift);
         L.koff = (unsigned)(((p * P.Q + ov) * P.Q + ou) * S * S);
     } else {
-        const uint4 ck = s_ck[tab_e.y >> 8];
+        const uint2 e = s_tab[p];
+        const uint4 ck = s_ck[e.y >> 8];
         L.key = ck.x + (unsigned)j0u * ck.y + ((unsigned)j0v >> ck.z);
-        L.koff = tab_e.x + (unsigned)((ov * P.Q + ou) * S * S);
+        L.koff = e.x + (unsigned)((ov * P.Q + ou) * S * S);
     }
     L.pos = (unsigned)j0u | ((unsigned)j0v << 16);
     return L;
@@ -464,9 +470,10 @@ static int launch_bin_passes(wpg_ctx *ctx, const void *d_vis, const double *d_uv
     dim3 nb((unsigned)((nvis + 256 * kVpt - 1) / (256 * kVpt)), 1, 1);
     if (bp.vis_block) {                // ceil(vis_block / 256) blocks per group of kVpt time steps
         const long long nd = (nvis + bp.vis_block - 1) / bp.vis_block;
-        const long long nblk = (long long)((bp.vis_block + 255) / 256) * ((nd + kVpt - 1) / kVpt);
-        if (nblk >= (1ll << 31)) return wpg_fail(ctx, WPG_EINVAL, "row_block = %u gives too many binning blocks", bp.vis_block / bp.nchan);
-        nb = dim3((unsigned)nblk, 1, 1);
+        const long long ngr = (nd + kVpt - 1) / kVpt, ntile = (ngr + bp.vis_tile - 1) / bp.vis_tile;
+        if (ntile > 65535 || (long long)bp.vis_nbx * bp.vis_tile >= (1ll << 31))
+            return wpg_fail(ctx, WPG_EINVAL, "row_block = %u gives too many binning blocks", bp.vis_block / bp.nchan);
+        nb = dim3(bp.vis_nbx * bp.vis_tile, (unsigned)ntile, 1);                    // (groups past the end find no visibility)
     }
     const bool any = nvis > 0;
     const bool qp2 = bp.qshift >= 0;

@@ -29,6 +29,9 @@ struct BinParams {
     int64_t nrow;
     int nchan;
     uint32_t row_block, vis_nbx;   // with vis_block: rows per time step; ceil(vis_block / 256) (host-computed: no divisions in the kernels)
+    uint32_t vis_ngroups;          // with vis_block: groups of kVpt time steps
+    uint32_t vis_tile_shift;       // log2 vis_tile
+    uint32_t vis_tile;             // (a power of two) with vis_block: consecutive blocks take vis_tile successive time groups of the same 256 baselines / channels
     int chan_shift;                // log2 nchan if nchan is a power of two, else -1
     uint32_t vis_block;            // 0, or visibilities per time step (row_block * nchan): a binning thread then takes
                                    // the SAME baseline/channel at consecutive time steps (see wpg_vis_index)
@@ -96,6 +99,7 @@ struct wpg_ctx {
     int64_t opt_row_block = 0; // rows per time step (0 = unknown), see wpg_set_option
     int opt_no_pairs = 0;     // 1: fp32 even supports also go through the run gridder (A/B comparison)
     int opt_compress = 1;     // record compression in the binning pass (0: one record per gridded visibility)
+    int opt_bin_tile = 0;     // time groups per block tile of the binning passes, 0 = default
     // instrumentation
     int64_t n_launches = 0;   // kernels of this library launched so far
     std::vector<cudaEvent_t> ev;   // triplets: start, after binning, after gridder (pool, reused)
@@ -287,12 +291,11 @@ static __device__ __noinline__ int4 wpg_locate_exact(double um, double vm, doubl
     return make_int4(r.p | (r.S << 16) | (r.inside ? 1 << 24 : 0) | (r.clamped ? 1 << 25 : 0), r.j0u, r.j0v, r.ou | (r.ov << 8));
 }
 
-// s_tab: the packed per-plane table in shared memory (ragged stacks; not read for uniform stacks).  tab_e: its entry
-// for the plane (ragged stacks).  QP2: the oversampling factor is a power of two (else the general form throughout).
-struct LeanPos { int p, S, j0u, j0v, ou, ov; bool inside, clamped; uint2 tab_e; };
+// s_tab: the packed per-plane table in shared memory (ragged stacks; not read for uniform stacks).  QP2: the oversampling factor is a power of two (else the general form throughout).
+struct LeanPos { int p, S, j0u, j0v, ou, ov; bool inside, clamped; };
 template <bool QP2>
 __device__ __forceinline__ LeanPos wpg_locate_lean(double um, double vm, double wm, double f, const BinParams &P, const uint2 *s_tab) {
-    LeanPos r; r.p = 0; r.S = 0; r.j0u = r.j0v = r.ou = r.ov = 0; r.inside = false; r.clamped = false; r.tab_e = make_uint2(0u, 0u);
+    LeanPos r; r.p = 0; r.S = 0; r.j0u = r.j0v = r.ou = r.ov = 0; r.inside = false; r.clamped = false;
     bool risk = !QP2;
     if (QP2) {
         const double u = __dmul_rn(um, f), vv = __dmul_rn(vm, f), w = __dmul_rn(wm, f);                  // G1
@@ -302,8 +305,7 @@ __device__ __forceinline__ LeanPos wpg_locate_lean(double um, double vm, double 
             const double qd = wpg_div_const(__dadd_rn(w, P.w_max), P.dw, P.rdw);
             r.p = min(max(wpg_floor_magic(qd, 1048576.0, risk), 0), P.Nw - 1);
         }
-        if (P.ncls > 1) r.tab_e = s_tab[r.p];               // {plane offset, S | class << 8}
-        r.S = P.ncls == 1 ? P.S0 : (int)(r.tab_e.y & 0xFFu);
+        r.S = P.ncls == 1 ? P.S0 : (int)(s_tab[r.p].y & 0xFFu);      // {plane offset, S | class << 8}
         const int c = (r.S - 2) * P.Q / 2;
         const double Qd = (double)P.Q, lim = 1073741824.0;
         // G3.  x * Q is exact for Q = 2^k, so the fused form rounds once, like the written two-step form.  Far outside
@@ -321,7 +323,6 @@ __device__ __forceinline__ LeanPos wpg_locate_lean(double um, double vm, double 
         const int4 o = wpg_locate_exact(um, vm, wm, f, P, s_tab);
         r.p = o.x & 0xFFFF; r.S = (o.x >> 16) & 0xFF; r.inside = (o.x >> 24) & 1; r.clamped = (o.x >> 25) & 1;
         r.j0u = o.y; r.j0v = o.z; r.ou = o.w & 0xFF; r.ov = o.w >> 8;
-        if (P.ncls > 1) r.tab_e = s_tab[r.p];
     }
     return r;
 }
