@@ -75,14 +75,41 @@ micro_dfma_kernel(double *__restrict__ sink, int iters, double seed) {
     if (s == 123.456) sink[0] = s;
 }
 
+// which = 5 / 6: the same row-segment reductions as which = 0, issued as ONE bulk reduction per segment by the copy
+// engine (cp.reduce.async.bulk.global.shared::cta.add.f32): the lanes stage the sums in shared memory, one lane issues.
+// 5: 256-byte segments (32 cells, like which = 0); 6: 64-byte segments (8 cells: one window row at S = 8).
+__global__ void __launch_bounds__(256)
+micro_bulkred_kernel(float2 *__restrict__ buf, unsigned ncell_mask, int iters, int cells) {
+    __shared__ __align__(128) float2 stage[8][4][32];              // per warp: ring of four staging rows
+    const unsigned gtid = blockIdx.x * 256u + threadIdx.x;
+    const unsigned lane = threadIdx.x & 31u, gwarp = gtid >> 5, w = threadIdx.x >> 5;
+    unsigned x = gwarp * 2654435761u + 12345u;
+    for (int i = 0; i < iters; ++i) {
+        x = x * 1664525u + 1013904223u;
+        const unsigned cell = ((x >> 4) & ncell_mask) & ~31u;
+        float2 *row = stage[w][i & 3];
+        if ((i & 3) == 0 && i) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the ring's rows are free again
+        __syncwarp();
+        if ((int)lane < cells) row[lane] = make_float2(1.0f, 0.5f);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) {
+            asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;"
+                         ::"l"(buf + cell), "r"((unsigned)__cvta_generic_to_shared(row)), "r"(cells * 8) : "memory");
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+    }
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
 }  // namespace
 
 // h_out[0] = operations per second (reductions of one cell, 16-byte loads, packed FMAs = 2 FMA, FMAs),
 // h_out[1] = kernel milliseconds.  d_buf: device scratch of at least buf_bytes >= 1 MiB (power of two used).
 extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_bytes, double *h_out) {
     if (!ctx || !h_out || !d_buf) return WPG_EINVAL;
-    if (which < 0 || which > 4 || iters < 1 || buf_bytes < ((size_t)1 << 20))
-        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which 0..4, iters >= 1, buffer >= 1 MiB");
+    if (which < 0 || which > 6 || iters < 1 || buf_bytes < ((size_t)1 << 20))
+        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which 0..6, iters >= 1, buffer >= 1 MiB");
     WPG_DEVICE(ctx);
     size_t ncell = 1;
     while (ncell * 2 * sizeof(float2) <= buf_bytes) ncell *= 2;
@@ -97,6 +124,7 @@ extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, s
         if (which <= 1) micro_red_kernel<<<blocks, 256, 0, s>>>((float2 *)d_buf, (unsigned)(ncell - 1), iters, which);
         else if (which == 2) micro_l1_kernel<<<blocks, 256, 0, s>>>((const float4 *)d_buf, (float *)d_buf, iters);
         else if (which == 3) micro_ffma2_kernel<<<blocks, 256, 0, s>>>((float *)d_buf, iters, 1.0f);
+        else if (which >= 5) micro_bulkred_kernel<<<blocks, 256, 0, s>>>((float2 *)d_buf, (unsigned)(ncell - 1), iters, which == 5 ? 32 : 8);
         else micro_dfma_kernel<<<blocks, 256, 0, s>>>((double *)d_buf, iters, 1.0);
         WPG_CUDA(ctx, cudaEventRecord(e1, s));
         ctx->n_launches += 1;
@@ -107,7 +135,9 @@ extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, s
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     WPG_CUDA(ctx, cudaGetLastError());
     const double threads = (double)blocks * 256.0;
-    const double ops = threads * (double)iters * (which == 0 || which == 1 ? 1.0 : 8.0);
+    // reductions of one cell (0, 1: one per lane; 5, 6: 32 or 8 per warp), else 8 operations per thread and trip
+    const double ops = which >= 5 ? threads / 32.0 * (double)iters * (which == 5 ? 32.0 : 8.0)
+                                  : threads * (double)iters * (which == 0 || which == 1 ? 1.0 : 8.0);
     h_out[0] = ops / (ms * 1e-3);
     h_out[1] = ms;
     return WPG_OK;
