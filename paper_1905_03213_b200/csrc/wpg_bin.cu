@@ -88,34 +88,52 @@ census_kernel(const double *__restrict__ uvw, const double *__restrict__ fscale,
     }
 }
 
-// Ragged stacks, pass 0c (one thread): split the key budget among the classes.  Every class starts with one
-// key per grid column; the class with the most visibilities per key is refined (one more bit of j0v) as long
-// as the total stays within the budget.
+// Ragged stacks, pass 0c (one warp, lane = support class): split the key budget among the classes.  Every class
+// starts with one key per grid column; the class with the most visibilities per key is refined (one more bit of
+// j0v) as long as the total stays within the budget.
 __global__ void plan_keys_kernel(Counters *__restrict__ ctr, int ncls, int N, unsigned budget) {
-    if (blockIdx.x || threadIdx.x) return;
-    unsigned sh[WPG_MAX_CLS];
-    unsigned long long total = 0;
+    static_assert(WPG_MAX_CLS <= 32, "one lane per support class");
+    if (blockIdx.x) return;
+    const int c = threadIdx.x;                       // 32 threads
+    const bool have = c < ncls;
     auto keys = [&](unsigned s_) { return (unsigned long long)N * (unsigned)((N + (1 << s_) - 1) >> s_); };
-    for (int c = 0; c < ncls; ++c) { sh[c] = 13; total += keys(13); }
+    const float census = have ? (float)ctr->census[c] + 1.0f : 0.0f;
+    unsigned sh = 13;
+    while (have && sh && keys(sh - 1) == keys(sh)) sh -= 1;          // bits that do not add keys (N < 2^13)
+    unsigned long long total = 0;
+    {
+        unsigned long long mine = have ? keys(sh) : 0ull;
+        for (int d = 16; d > 0; d >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, d);
+        total = mine;
+    }
     for (;;) {
-        int best = -1; double best_d = -1.0;
-        for (int c = 0; c < ncls; ++c) {
-            if (sh[c] == 0 || keys(sh[c] - 1) == keys(sh[c])) { if (sh[c] && keys(sh[c] - 1) == keys(sh[c])) { sh[c] -= 1; c -= 1; } continue; }
-            if (total - keys(sh[c]) + keys(sh[c] - 1) > budget) continue;
-            const double d = ((double)ctr->census[c] + 1.0) / (double)keys(sh[c]);
-            if (d > best_d) { best_d = d; best = c; }
+        // this lane's candidate: one more bit, if it adds keys and fits
+        const unsigned long long grow = have && sh ? keys(sh - 1) - keys(sh) : 0ull;
+        const bool can = have && sh && grow > 0 && total + grow <= budget;
+        float d = can ? census / (float)keys(sh) : -1.0f;
+        // argmax over the lanes (lowest class wins ties)
+        float best = d; int who = c;
+        for (int o = 16; o > 0; o >>= 1) {
+            const float ob = __shfl_xor_sync(0xffffffffu, best, o);
+            const int ow = __shfl_xor_sync(0xffffffffu, who, o);
+            if (ob > best || (ob == best && ow < who)) { best = ob; who = ow; }
         }
-        if (best < 0) break;
-        total += keys(sh[best] - 1) - keys(sh[best]);
-        sh[best] -= 1;
+        if (best < 0.0f) break;
+        const unsigned long long g = __shfl_sync(0xffffffffu, grow, who);
+        if (c == who) { sh -= 1; while (sh && keys(sh - 1) == keys(sh)) sh -= 1; }
+        total += g;
     }
-    unsigned base = 0;
-    for (int c = 0; c < ncls; ++c) {
-        ctr->key_base[c] = base; ctr->key_shift[c] = sh[c];
-        ctr->key_nkg[c] = (unsigned)((N + (1 << sh[c]) - 1) >> sh[c]);
-        base += (unsigned)keys(sh[c]);
+    // bases: exclusive prefix sum of the classes' key counts
+    unsigned long long mine = have ? keys(sh) : 0ull, incl = mine;
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, o);
+        if (c >= o) incl += t;
     }
-    ctr->key_base[ncls] = base;
+    if (have) {
+        ctr->key_base[c] = (unsigned)(incl - mine); ctr->key_shift[c] = sh;
+        ctr->key_nkg[c] = (unsigned)((N + (1 << sh) - 1) >> sh);
+        if (c == ncls - 1) ctr->key_base[ncls] = (unsigned)incl;
+    }
 }
 
 constexpr int kVpt = 4;            // visibilities per thread: four independent atomics in flight per thread
