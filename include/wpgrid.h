@@ -226,7 +226,9 @@ int  wpg_shard_rows(int64_t nrow, int64_t row_block, int world, int rank, int64_
  * which: 0 = red.global.add.v2.f32, a warp per 256-byte row segment at a pseudo-random place of the buffer (the
  *            naive gridder's pattern; "write access ... in an atomic manner");
  *        1 = the same, every lane its own pseudo-random cell;   2 = L1-resident 16-byte loads;
- *        3 = fma.rn.f32x2;   4 = fma.rn.f64.
+ *        3 = fma.rn.f32x2;   4 = fma.rn.f64;
+ *        5 / 6 = the pattern of 0 issued as one cp.reduce.async.bulk (copy engine) per 256-byte / 64-byte segment staged
+ *            in shared memory.
  * d_buf: device scratch, buf_bytes >= 1 MiB (the reductions use the largest power-of-two number of 8-byte cells
  * that fits; its contents are overwritten).  h_out[0] = operations/s, h_out[1] = kernel ms.  Synchronises. */
 int  wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_bytes, double *h_out /*[2]*/);
