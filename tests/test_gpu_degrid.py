@@ -29,12 +29,15 @@ def check(ctx, uvw, freq, st, g, support):
     for prec in (wpgrid.F32, wpgrid.F64):
         ks = ctx.stack_from_host(st.data, st.Nw, st.w_max, support, st.oversample, st.grid_N, st.cell, prec)
         dg = torch.from_numpy(g.astype(np.complex64 if prec == wpgrid.F32 else np.complex128)).cuda()
-        out, cnt = ctx.degrid(dg, du, df, ks, counts=True)
-        assert cnt == rcnt
-        o = out.cpu().numpy().astype(np.complex128)
-        err = float(np.max(np.abs(o - ref)) / np.max(np.abs(ref)))
-        assert err <= TOL[prec], (prec, err)
-        assert np.array_equal(o == 0, ref == 0) or prec == wpgrid.F32
+        for general in (0, 1):            # 0: degrid_fast_kernel where it applies (S = 4, 8, 16); 1: degrid_kernel always
+            ctx.set_option("no_pairs", general)
+            out, cnt = ctx.degrid(dg, du, df, ks, counts=True)
+            ctx.set_option("no_pairs", 0)
+            assert cnt == rcnt
+            o = out.cpu().numpy().astype(np.complex128)
+            err = float(np.max(np.abs(o - ref)) / np.max(np.abs(ref)))
+            assert err <= TOL[prec], (prec, general, err)
+            assert np.array_equal(o == 0, ref == 0) or prec == wpgrid.F32
 
 
 @pytest.mark.parametrize("S", [4, 7, 8, 12, 16, 32])
