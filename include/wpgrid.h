@@ -69,7 +69,8 @@ int  wpg_version(void);
  * unless that exceeds the cap,
  * then low bits of j0v are dropped.  Ragged stacks: the cap is a budget (default: about one key per visibility,
  * 2^24 .. 2^27) split among the support classes on the device after a census of the classes.  "timing" 0/1 (see wpg_phase_ms); "no_pairs" 0/1 (1: fp32 even
- * supports go through the generic run gridder instead of the pair gridder — for A/B comparison);
+ * supports go through the generic run gridder instead of the pair gridder, and wpg_degrid / wpg_grid_pol take their
+ * general kernels — for A/B comparison);
  * "row_block" = rows per time step when the rows come time-major, baseline-minor (the row order of a
  * Measurement Set; 0 = unknown, the default): a binning thread then handles the same
  * baseline at consecutive time steps, whose samples mostly hit the same grid point, and
