@@ -79,6 +79,10 @@ int  wpg_version(void);
  * "bin_tile" (with "row_block"; default 16, rounded down to a power of two): consecutive blocks of the binning passes
  * take this many successive groups of time steps of the same 256 baselines / channels, so that the blocks resident
  * together hit the same bucket counters and record stretches while those are still in L2.
+ * "chunk_sort" 0/1 (default 1): where the sort key drops low bits of j0v (grids above 4096^2, the sparse support classes
+ * of a ragged stack) a fourth pass sorts chunks of 32 consecutive records by the full window start, so that the gridder's
+ * window sweeps each bucket monotonically; with it on, the default key cap of a uniform stack whose full-resolution key
+ * space exceeds 2^24 follows the data (about 16 records per key, 2^20 .. 2^24).
  * "compress" 0/1 (default 1): record compression — a binning thread's consecutive
  * visibilities with the same plane, window start and sub-cell offsets share one sorted record carrying the sum of their
  * weight * vis; the grid is unchanged (gridding is linear), the counters still count visibilities.  Effective with

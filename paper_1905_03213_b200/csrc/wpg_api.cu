@@ -72,6 +72,7 @@ extern "C" int wpg_set_option(wpg_ctx *ctx, const char *name, int64_t value) {
     else if (!strcmp(name, "timing")) { ctx->opt_timing = value != 0; }
     else if (!strcmp(name, "no_pairs")) { ctx->opt_no_pairs = value != 0; }
     else if (!strcmp(name, "compress")) { ctx->opt_compress = value != 0; }
+    else if (!strcmp(name, "chunk_sort")) { ctx->opt_chunk_sort = value != 0; }
     else if (!strcmp(name, "bin_tile")) { if (value < 0 || value > 65536) return wpg_fail(ctx, WPG_EINVAL, "bin_tile must be 0..65536"); ctx->opt_bin_tile = (int)value; }
     else if (!strcmp(name, "row_block")) { if (value < 0) return wpg_fail(ctx, WPG_EINVAL, "row_block must be >= 0"); ctx->opt_row_block = value; }
     else return wpg_fail(ctx, WPG_EINVAL, "unknown option '%s'", name);
@@ -166,9 +167,17 @@ int wpg_make_plan(wpg_ctx *ctx, const wpg_kdesc *d, int64_t nrow, int nchan, wpg
     // down the v axis, so a window that moves on leaves whole grid-row segments behind (contiguous write-outs)
     // and keeps its column ownership (the parity of j0u is fixed within a sweep); full resolution unless the
     // key space would exceed 2^key_bits
-    // default cap: 2^24 keys (a 64 MB offset table stays in L2; at 2^26 the binning of N = 8192 takes twice as
-    // long); ragged stacks multiply the key space by the number of support classes and get 2^26
-    const int64_t cap = (int64_t)1 << (ctx->opt_key_bits ? ctx->opt_key_bits : (bp->ncls > 1 ? 26 : 24));
+    // (ragged stacks multiply the key space by the number of support classes: their budget is set further down)
+    // Default cap of a uniform stack: 2^24 keys (a 64 MB offset table; at 2^26 the binning of N = 8192 takes twice as
+    // long).  Where full resolution does not fit (N > 4096) the cap follows the data instead — about 16 records per
+    // key, 2^20 .. 2^24 — and the chunk sort (wpg_bin.cu, pass 4) restores the fine order inside the buckets: measured
+    // on config 3 at N = 8192, 2^22 keys + chunk sort beat 2^24 keys without it by 10 % of the step.
+    int def_bits = 24;
+    if (bp->ncls == 1 && ctx->opt_chunk_sort && (int64_t)d->grid_N * d->grid_N > ((int64_t)1 << 24)) {
+        def_bits = 20;
+        while (def_bits < 24 && ((int64_t)16 << def_bits) < nvis) ++def_bits;
+    }
+    const int64_t cap = (int64_t)1 << (ctx->opt_key_bits ? ctx->opt_key_bits : (bp->ncls > 1 ? 26 : def_bits));
     int kshift = 0;
     while ((int64_t)bp->ncls * d->grid_N * (((int64_t)d->grid_N + (1 << kshift) - 1) >> kshift) > cap && kshift < 13) ++kshift;
     bp->kshift = kshift;
@@ -208,7 +217,7 @@ extern "C" size_t wpg_grid_workspace_bytes(const wpg_ctx *ctx, int64_t nrow, int
                                            wpg_prec prec) {
     PlaneTab tab; BinParams bp; WorkspaceLayout ws;
     wpg_ctx tmp;
-    if (ctx) { tmp.opt_segment = ctx->opt_segment; tmp.opt_key_bits = ctx->opt_key_bits; }
+    if (ctx) { tmp.opt_segment = ctx->opt_segment; tmp.opt_key_bits = ctx->opt_key_bits; tmp.opt_chunk_sort = ctx->opt_chunk_sort; }
     if (wpg_make_plan(&tmp, desc, nrow, nchan, prec, &tab, &bp, &ws)) return 0;
     return ws.total;
 }

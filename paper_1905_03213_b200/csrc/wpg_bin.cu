@@ -454,6 +454,61 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
     }
 }
 
+// Pass 4 (only where the sort key drops low bits of j0v: large grids, the sparse support classes of a ragged stack):
+// inside a bucket the records stand in the order the atomics gave them, so the gridder's window would jump back and
+// forth over the bucket's rows and write its sums out at every jump.  Every warp sorts chunks of 32 consecutive records
+// of the class by the full window start (j0u, then j0v) — a bitonic network over the lanes on (key, source lane), then
+// one gather of the records.
+// Buckets are contiguous and ordered, so sorting a chunk by the full key restores the column-major sweep inside it
+// (a bucket cut by a chunk boundary becomes two sorted runs).  W = 32-bit words per record (4: fp32, 6: fp64).
+template <int W>
+__global__ void __launch_bounds__(256)
+chunk_sort_kernel(unsigned *__restrict__ rec, const unsigned *__restrict__ bucket_start, const Counters *__restrict__ ctr,
+                  int cls, unsigned key_lo, unsigned key_hi, int uniform_shift) {
+    unsigned shift = (unsigned)uniform_shift;
+    if (uniform_shift < 0) { key_lo = ctr->key_base[cls]; key_hi = ctr->key_base[cls + 1]; shift = ctr->key_shift[cls]; }
+    if (shift == 0) return;                                    // full resolution already
+    const unsigned r0 = __ldg(bucket_start + key_lo), r1 = __ldg(bucket_start + key_hi);
+    // dense classes (more than two records per window position on average) are left alone: their windows repeat,
+    // a chunk of 32 records does not span a bucket, and the pass would cost more than the gridder gains
+    if ((unsigned long long)(r1 - r0) > 2ull * ((unsigned long long)(key_hi - key_lo) << shift)) return;
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned nwarp = (gridDim.x * 256u) >> 5;
+    for (unsigned c0 = r0 + 32u * ((blockIdx.x * 256u + threadIdx.x) >> 5); c0 < r1; c0 += 32u * nwarp) {
+        const unsigned i = c0 + lane;
+        const bool have = i < r1;
+        unsigned v[W];
+#pragma unroll
+        for (int k = 0; k < W; k += 2) {
+            const uint2 t = have ? *reinterpret_cast<const uint2 *>(rec + (size_t)i * W + k) : make_uint2(0u, 0u);
+            v[k] = t.x; v[k + 1] = t.y;
+        }
+        const unsigned pos = v[W - 2];
+        unsigned key = have ? ((pos << 16) | (pos >> 16)) : 0xFFFFFFFFu;       // j0u major, j0v minor; empty lanes last
+        // already sorted (runs of equal windows, monotone sweeps): nothing to do
+        const unsigned prev = __shfl_up_sync(0xffffffffu, key, 1);
+        if (!__any_sync(0xffffffffu, lane > 0 && prev > key)) continue;
+        // sort (key, source lane) pairs, then fetch the record of the source lane: two words per exchange instead of W
+        unsigned src = lane;
+#pragma unroll
+        for (unsigned k = 2; k <= 32; k <<= 1) {
+#pragma unroll
+            for (unsigned j = k >> 1; j > 0; j >>= 1) {
+                const unsigned pk = __shfl_xor_sync(0xffffffffu, key, j), ps = __shfl_xor_sync(0xffffffffu, src, j);
+                const bool lower = (lane & j) == 0, asc = (lane & k) == 0;
+                const bool take = (lower == asc) ? key > pk : key < pk;
+                if (take) { key = pk; src = ps; }
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < W; ++q) v[q] = __shfl_sync(0xffffffffu, v[q], src);
+        if (have) {
+#pragma unroll
+            for (int k = 0; k < W; k += 2) *reinterpret_cast<uint2 *>(rec + (size_t)i * W + k) = make_uint2(v[k], v[k + 1]);
+        }
+    }
+}
+
 }  // namespace
 
 // Exclusive prefix sum of hist[0 .. n-1] in place, hist[n] = total (also written to ctr->n_records);
@@ -523,6 +578,19 @@ static int launch_bin_passes(wpg_ctx *ctx, const void *d_vis, const double *d_uv
         else if (prec == WPG_F32) WPG_SCATTER(float, 1);
         else WPG_SCATTER(double, 1);
 #undef WPG_SCATTER
+        // fine order inside the buckets of keys that dropped bits of j0v (single-correlation records)
+        if (npol == 1 && ctx->opt_chunk_sort && (bp.dyn_keys || bp.kshift > 0)) {
+            unsigned *r32 = (unsigned *)rec;
+            const unsigned *bs = (const unsigned *)(w + ws.off_hist);
+            const int blocks = ctx->sm_count * 8;
+            for (int cls = 0; cls < bp.ncls; ++cls) {
+                const unsigned lo = (unsigned)cls * bp.keys_per_class, hi = (unsigned)(cls + 1) * bp.keys_per_class;
+                const int ush = bp.dyn_keys ? -1 : bp.kshift;
+                if (prec == WPG_F32) chunk_sort_kernel<4><<<blocks, 256, 0, s>>>(r32, bs, ctr, cls, lo, hi, ush);
+                else chunk_sort_kernel<6><<<blocks, 256, 0, s>>>(r32, bs, ctr, cls, lo, hi, ush);
+                ctx->n_launches += 1;
+            }
+        }
     }
     ctx->n_launches += any ? 6 : 4;
     WPG_CUDA(ctx, cudaGetLastError());

@@ -100,6 +100,7 @@ struct wpg_ctx {
     int opt_no_pairs = 0;     // 1: fp32 even supports also go through the run gridder (A/B comparison)
     int opt_compress = 1;     // record compression in the binning pass (0: one record per gridded visibility)
     int opt_bin_tile = 0;     // time groups per block tile of the binning passes, 0 = default
+    int opt_chunk_sort = 1;   // fine order inside coarse buckets (chunk_sort_kernel); 0: off
     // instrumentation
     int64_t n_launches = 0;   // kernels of this library launched so far
     std::vector<cudaEvent_t> ev;   // triplets: start, after binning, after gridder (pool, reused)
