@@ -233,7 +233,10 @@ int  wpg_shard_rows(int64_t nrow, int64_t row_block, int world, int rank, int64_
  *        1 = the same, every lane its own pseudo-random cell;   2 = L1-resident 16-byte loads;
  *        3 = fma.rn.f32x2;   4 = fma.rn.f64;
  *        5 / 6 = the pattern of 0 issued as one cp.reduce.async.bulk (copy engine) per 256-byte / 64-byte segment staged
- *            in shared memory.
+ *            in shared memory;
+ *        7 / 8 = the inner loop of a shared-memory subgrid accumulator (64 x 64-cell tile + halo per CTA, S = 8, one
+ *            L1-resident coefficient slice per record): 7 with red.shared.add.f32, 8 with plain load / add / store
+ *            (the ceiling of a warp-owned tile); h_out[0] = grid updates/s.  2, 7, 8 need buf_bytes >= 16 MiB.
  * d_buf: device scratch, buf_bytes >= 1 MiB (the reductions use the largest power-of-two number of 8-byte cells
  * that fits; its contents are overwritten).  h_out[0] = operations/s, h_out[1] = kernel ms.  Synchronises. */
 int  wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_bytes, double *h_out /*[2]*/);

@@ -102,19 +102,60 @@ micro_bulkred_kernel(float2 *__restrict__ buf, unsigned ncell_mask, int iters, i
     asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
+// which = 7 / 8: the inner loop of a shared-memory-staged subgrid accumulator (SURVEY.md §8 north_star's alternative
+// to register accumulation): a CTA owns a 64 x 64-cell tile plus the S - 1 = 7 halo in shared memory (72-cell rows);
+// per trip every warp takes one "record" - an L1-resident 512-byte coefficient slice as in which = 2, a window start
+// picked pseudo-randomly in the tile - and adds its 64 products into the tile, lane <-> (window row, cell pair).
+// 7: red.shared.add.f32 (correct whoever else touches the cells); 8: plain 8-byte load / FFMA2 / store, i.e. the
+// ceiling of a scheme that needs no atomics because one warp owns the tile (the write races here are deliberate).
+__global__ void __launch_bounds__(256)
+micro_subgrid_kernel(const float4 *src, float2 *sink, int iters, int atomic) {
+    constexpr int kRow = 72, kCells = 71 * kRow;
+    extern __shared__ float2 tile[];
+    for (int i = threadIdx.x; i < kCells; i += 256) tile[i] = make_float2(0.f, 0.f);
+    __syncthreads();
+    const unsigned gwarp = (blockIdx.x * 256u + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
+    const float4 *p = src + (size_t)(gwarp & 4095u) * 256u + lane;
+    const unsigned r = lane >> 2, c = (lane & 3u) * 2u;
+    unsigned x = gwarp * 2654435761u + 12345u;
+    const float vr = 1.0f + (float)lane, vi = 0.5f;
+    for (int i = 0; i < iters; ++i) {
+        x = x * 1664525u + 1013904223u;
+        float4 k;
+        asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(k.x), "=f"(k.y), "=f"(k.z), "=f"(k.w) : "l"(p + (i & 7) * 32));
+        float2 *cell = tile + (((x >> 8) & 63u) + r) * kRow + ((x >> 16) & 63u) + c;
+        const float a0 = vr * k.x - vi * k.y, b0 = vr * k.y + vi * k.x, a1 = vr * k.z - vi * k.w, b1 = vr * k.w + vi * k.z;
+        if (atomic) {
+            atomicAdd(&cell[0].x, a0); atomicAdd(&cell[0].y, b0);
+            atomicAdd(&cell[1].x, a1); atomicAdd(&cell[1].y, b1);
+        } else {
+            float2 t0 = cell[0], t1 = cell[1];
+            t0.x += a0; t0.y += b0; t1.x += a1; t1.y += b1;
+            cell[0] = t0; cell[1] = t1;
+        }
+    }
+    __syncthreads();
+    float2 acc = make_float2(0.f, 0.f);
+    for (int i = threadIdx.x; i < kCells; i += 256) { acc.x += tile[i].x; acc.y += tile[i].y; }
+    if (acc.x == 123.456f) sink[0] = acc;
+}
+
 }  // namespace
 
-// h_out[0] = operations per second (reductions of one cell, 16-byte loads, packed FMAs = 2 FMA, FMAs),
+// h_out[0] = operations per second (reductions of one cell, 16-byte loads, packed FMAs = 2 FMA, FMAs, grid updates),
 // h_out[1] = kernel milliseconds.  d_buf: device scratch of at least buf_bytes >= 1 MiB (power of two used).
 extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_bytes, double *h_out) {
     if (!ctx || !h_out || !d_buf) return WPG_EINVAL;
-    if (which < 0 || which > 6 || iters < 1 || buf_bytes < ((size_t)1 << 20))
-        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which 0..6, iters >= 1, buffer >= 1 MiB");
+    if (which < 0 || which > 8 || iters < 1 || buf_bytes < ((size_t)1 << 20))
+        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which 0..8, iters >= 1, buffer >= 1 MiB");
     WPG_DEVICE(ctx);
     size_t ncell = 1;
     while (ncell * 2 * sizeof(float2) <= buf_bytes) ncell *= 2;
-    if (which == 2 && buf_bytes < ((size_t)16 << 20)) return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which = 2 needs a 16 MiB buffer");
-    const int blocks = ctx->sm_count * (which == 2 ? 2 : 8);
+    if ((which == 2 || which >= 7) && buf_bytes < ((size_t)16 << 20))
+        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which = 2, 7, 8 need a 16 MiB buffer");
+    const int blocks = ctx->sm_count * (which == 2 ? 2 : which >= 7 ? 4 : 8);
+    constexpr int kSubgridBytes = 71 * 72 * (int)sizeof(float2);
+    if (which >= 7) WPG_CUDA(ctx, cudaFuncSetAttribute(micro_subgrid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSubgridBytes));
     cudaEvent_t e0, e1;
     WPG_CUDA(ctx, cudaEventCreate(&e0));
     WPG_CUDA(ctx, cudaEventCreate(&e1));
@@ -124,6 +165,7 @@ extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, s
         if (which <= 1) micro_red_kernel<<<blocks, 256, 0, s>>>((float2 *)d_buf, (unsigned)(ncell - 1), iters, which);
         else if (which == 2) micro_l1_kernel<<<blocks, 256, 0, s>>>((const float4 *)d_buf, (float *)d_buf, iters);
         else if (which == 3) micro_ffma2_kernel<<<blocks, 256, 0, s>>>((float *)d_buf, iters, 1.0f);
+        else if (which >= 7) micro_subgrid_kernel<<<blocks, 256, kSubgridBytes, s>>>((const float4 *)d_buf, (float2 *)d_buf, iters, which == 7);
         else if (which >= 5) micro_bulkred_kernel<<<blocks, 256, 0, s>>>((float2 *)d_buf, (unsigned)(ncell - 1), iters, which == 5 ? 32 : 8);
         else micro_dfma_kernel<<<blocks, 256, 0, s>>>((double *)d_buf, iters, 1.0);
         WPG_CUDA(ctx, cudaEventRecord(e1, s));
@@ -136,7 +178,8 @@ extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, s
     WPG_CUDA(ctx, cudaGetLastError());
     const double threads = (double)blocks * 256.0;
     // reductions of one cell (0, 1: one per lane; 5, 6: 32 or 8 per warp), else 8 operations per thread and trip
-    const double ops = which >= 5 ? threads / 32.0 * (double)iters * (which == 5 ? 32.0 : 8.0)
+    const double ops = which >= 7 ? threads / 32.0 * (double)iters * 64.0           // 7, 8: grid updates (64 per record)
+                     : which >= 5 ? threads / 32.0 * (double)iters * (which == 5 ? 32.0 : 8.0)
                                   : threads * (double)iters * (which == 0 || which == 1 ? 1.0 : 8.0);
     h_out[0] = ops / (ms * 1e-3);
     h_out[1] = ms;
