@@ -20,7 +20,9 @@ gridder    O4  G1-G7 convolutional gridding (data model
                row x channel PAPER.md:56), plain C loops in grid_oracle.c;
                degrid(): its adjoint with unit weights (PAPER.md:36);
                flux(): P11's right-hand side and the grid's first moments in
-               O(nvis) without a grid (checks full-size GPU runs)
+               O(nvis) without a grid (checks full-size GPU runs);
+               cells(): single grid cells one by one, G5 read as a gather
+               (full-size GPU runs on sampled outputs)
 image      O5  dirty image = centred inverse FFT / taper
            O6  brute-force direct 3-D DFT image (pin for the whole chain)
 baseline_  Eqs. (1)-(2): baseline index from antenna IDs, count array C, exclusive
@@ -33,7 +35,8 @@ P4 w=0 separability, P5 slice sums ~ 1, P6/P7 worked index/plane examples
 (tests/golden/), P8 stored kernel values (tests/golden/), P9 gridded dirty
 image vs direct 3-D DFT, P10 single-visibility footprint, P11 flux
 conservation (and oracle_flux against the Python P11 sum, hand-written moment
-sums and the gridded result), P12 linearity/chunking; Eqs. (1)-(2): worked example, bijection onto the antenna
+sums and the gridded result; oracle_cells against the gather written out in
+Python and against the scatter-form grid, every cell), P12 linearity/chunking; Eqs. (1)-(2): worked example, bijection onto the antenna
 triangle, closed-form row starts, numpy cumsum / stable argsort
 (tests/test_oracle_baseline_order.py); degridder: adjoint identity, single-cell
 grids, prediction of the measurement model (tests/test_oracle_degrid.py).  No function here is "parity unpinned".

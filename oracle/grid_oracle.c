@@ -258,6 +258,67 @@ int oracle_flux(const double *uvw, const float *vis, const float *weight, const 
     return 0;
 }
 
+/* The gridded value of single cells, one by one (G5 read as a gather; for checking full-size GPU runs on sampled
+ * outputs): cell (cv[k], cu[k]) = sum over every visibility whose window covers it,
+ *     j0v <= cv < j0v + S  and  j0u <= cu < j0u + S,
+ * of wt V K[p][ov][ou][cv - j0v][cu - j0u].  Plane, window, sub-cell offsets and validity exactly as in grid_rows
+ * (G1-G4): every visibility is tested against every requested cell, nothing cleverer.
+ * out: 2 doubles per cell (re, im); l1_out: sum of |wt V| |K| per cell (the scale of its rounding error).
+ * Threads split the rows; each sums into its own copy, the copies are added in thread order. */
+int oracle_cells(const double *uvw, const float *vis, const float *weight, const double *freq,
+                 int64_t nrow, int nchan, const double *K, const int *support, const int64_t *plane_offset,
+                 int Nw, int Q, int N, double cell, double w_max,
+                 const int *cu, const int *cv, int ncell, double *out, double *l1_out, int nthreads) {
+    if (nthreads < 1) nthreads = 1;
+    double *acc = (double *)calloc((size_t)nthreads * 3 * (size_t)(ncell > 0 ? ncell : 1), sizeof(double));
+    if (!acc) return -1;
+#pragma omp parallel num_threads(nthreads)
+    {
+#ifdef _OPENMP
+        int t = omp_get_thread_num(), nt = omp_get_num_threads();
+#else
+        int t = 0, nt = 1;
+#endif
+        double *a = acc + (size_t)t * 3 * ncell;
+        int64_t r0 = nrow * t / nt, r1 = nrow * (t + 1) / nt;
+        for (int64_t r = r0; r < r1; ++r) {
+            for (int c = 0; c < nchan; ++c) {
+                double wt = (double)weight[r * nchan + c];
+                if (wt == 0.0) continue;
+                double f = freq[c] / C0;
+                double u = uvw[3 * r + 0] * f, v = uvw[3 * r + 1] * f, w = uvw[3 * r + 2] * f;
+                int clamped;
+                int p = oracle_plane(w, w_max, Nw, &clamped);
+                int S = support[p];
+                int64_t j0u, j0v; int ou, ov;
+                oracle_index_map(u, N, cell, S, Q, &j0u, &ou);
+                oracle_index_map(v, N, cell, S, Q, &j0v, &ov);
+                if (j0u < 0 || j0v < 0 || j0u + S > N || j0v + S > N) continue;
+                double vr = wt * (double)vis[2 * (r * nchan + c) + 0];
+                double vi = wt * (double)vis[2 * (r * nchan + c) + 1];
+                const double *Ks = K + 2 * (plane_offset[p] + ((int64_t)ov * Q + ou) * S * S);
+                for (int k = 0; k < ncell; ++k) {
+                    int64_t iv = (int64_t)cv[k] - j0v, iu = (int64_t)cu[k] - j0u;
+                    if (iv < 0 || iv >= S || iu < 0 || iu >= S) continue;
+                    double kr = Ks[2 * (iv * S + iu)], ki = Ks[2 * (iv * S + iu) + 1];
+                    a[3 * k]     += vr * kr - vi * ki;
+                    a[3 * k + 1] += vr * ki + vi * kr;
+                    a[3 * k + 2] += sqrt(vr * vr + vi * vi) * sqrt(kr * kr + ki * ki);
+                }
+            }
+        }
+    }
+    for (int k = 0; k < ncell; ++k) {
+        double sr = 0, si = 0, sl = 0;
+        for (int t = 0; t < nthreads; ++t) {
+            sr += acc[((size_t)t * ncell + k) * 3]; si += acc[((size_t)t * ncell + k) * 3 + 1]; sl += acc[((size_t)t * ncell + k) * 3 + 2];
+        }
+        out[2 * k] = sr; out[2 * k + 1] = si; l1_out[k] = sl;
+    }
+    free(acc);
+    return 0;
+}
+
 int oracle_max_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -45,6 +45,8 @@ def _load():
         lib.oracle_degrid.restype = cint
         lib.oracle_flux.argtypes = [vp, vp, vp, vp, i64, cint, vp, vp, cint, cint, cint, dbl, dbl, vp, vp, cint]
         lib.oracle_flux.restype = cint
+        lib.oracle_cells.argtypes = [vp, vp, vp, vp, i64, cint, vp, vp, vp, cint, cint, cint, dbl, dbl, vp, vp, cint, vp, vp, cint]
+        lib.oracle_cells.restype = cint
         lib.oracle_max_threads.restype = cint
         _lib = lib
     return _lib
@@ -156,3 +158,29 @@ def flux(uvw, vis, weight, freq, stack, threads=1):
         raise RuntimeError("oracle_flux failed rc=%d" % rc)
     return ({"sum": complex(out[0], out[1]), "mom_u": complex(out[2], out[3]), "mom_v": complex(out[4], out[5]),
              "l1": float(out[6])}, dict(zip(STAT_NAMES, (int(x) for x in st))))
+
+
+def cells(uvw, vis, weight, freq, stack, cu, cv, threads=1):
+    """Gridded value of the single cells (cv[k], cu[k]), one by one (oracle_cells in grid_oracle.c: G5 read as a
+    gather, every visibility tested against every requested cell) — what a full-size GPU run is checked against on
+    sampled outputs.  Returns (values complex128 [ncell], l1 float64 [ncell] = sum |wt V| |K| per cell)."""
+    uvw = np.ascontiguousarray(uvw, dtype=np.float64)
+    vis = np.ascontiguousarray(vis, dtype=np.complex64)
+    weight = np.ascontiguousarray(weight, dtype=np.float32)
+    freq = np.ascontiguousarray(freq, dtype=np.float64)
+    cu = np.ascontiguousarray(cu, dtype=np.int32)
+    cv = np.ascontiguousarray(cv, dtype=np.int32)
+    nrow, nchan = uvw.shape[0], freq.shape[0]
+    assert vis.size == nrow * nchan and weight.size == nrow * nchan and cu.shape == cv.shape and cu.ndim == 1
+    K = np.ascontiguousarray(stack.data, dtype=np.complex128)
+    sup = np.ascontiguousarray(stack.support, dtype=np.int32)
+    off = np.ascontiguousarray(stack.plane_offset, dtype=np.int64)
+    out = np.zeros(cu.size, dtype=np.complex128)
+    l1 = np.zeros(cu.size, dtype=np.float64)
+    rc = _load().oracle_cells(uvw.ctypes.data, vis.ctypes.data, weight.ctypes.data, freq.ctypes.data, nrow, nchan,
+                              K.ctypes.data, sup.ctypes.data, off.ctypes.data, stack.Nw, stack.oversample,
+                              stack.grid_N, stack.cell, stack.w_max, cu.ctypes.data, cv.ctypes.data, int(cu.size),
+                              out.ctypes.data, l1.ctypes.data, int(threads))
+    if rc != 0:
+        raise RuntimeError("oracle_cells failed rc=%d" % rc)
+    return out, l1

@@ -5,8 +5,13 @@ full runs are checked with what SURVEY.md §8(c) prescribes for them: the counte
 conservation — whose right-hand side is O(nvis): oracle.gridder.flux (oracle_flux in grid_oracle.c, pinned in
 tests/test_oracle_gridder.py) gives sum(grid) and, beyond P11, the two first moments sum(grid * ju), sum(grid * jv),
 which also pin where the flux went.  fp64 makes the check sharp (a single dropped, duplicated or misplaced
-visibility is orders of magnitude outside the bound); fp32 is bounded by its accumulation error.  Element-wise
-parity on seeded prefixes through the full-size grid is in test_gpu_parity.py.
+visibility is orders of magnitude outside the bound); fp32 is bounded by its accumulation error.  On top of that,
+sampled outputs the oracle computes one by one: oracle.gridder.cells (oracle_cells in grid_oracle.c, G5 read as a
+gather over ALL visibilities, pinned in tests/test_oracle_gridder.py) gives the exact value of a seeded sample of
+grid cells — cells inside the windows of randomly drawn visibilities, so that they follow the density of the
+coverage, plus uniformly drawn ones — which the GPU grid must match to north_star's 1e-4 / 1e-10 of the largest
+sampled magnitude (at most the grid's largest, so the bound is the stricter one).  Element-wise parity on seeded
+prefixes through the full-size grid is in test_gpu_parity.py.
 """
 import os
 
@@ -25,6 +30,8 @@ from paper_1905_03213_b200 import synth, wpgrid
 # reductions in arbitrary order, far below one visibility (|V sigma| / L1 ~ 3e-9 on config 4, larger elsewhere).  fp32: the
 # accumulated rounding of the c64 grid, measured 1e-12 .. 3e-9 of L1; fp64 measured 1e-17 (profiles/r02_fullsize_parity.md).
 FLUX_TOL = {wpgrid.F32: 2e-8, wpgrid.F64: 1e-14}
+CELL_TOL = {wpgrid.F32: 1e-4, wpgrid.F64: 1e-10}        # north_star, relative to the largest |reference| (here: of the sample)
+N_CELL_VIS, N_CELL_UNIFORM = 160, 32
 THREADS = min(os.cpu_count() or 1, 32)
 
 
@@ -42,6 +49,27 @@ def oracle_stack(wl):
     if not np.isscalar(sup):
         sup = owk.ragged_support(wl.Nw, wl.w_max, wl.grid_N, wl.cell, sup[1], sup[2])
     return owk.build_stack(wl.Nw, wl.w_max, sup, wl.oversample, wl.grid_N, wl.cell)
+
+
+def sample_cells(wl, st, seed):
+    """Seeded sample of grid cells: one cell inside the window of each of N_CELL_VIS randomly drawn visibilities (so
+    the sample follows the coverage: most lie where the grid is dense), plus N_CELL_UNIFORM uniformly drawn cells."""
+    rng = np.random.default_rng(seed)
+    N, nchan = wl.grid_N, wl.freq.size
+    cu, cv = [], []
+    while len(cu) < N_CELL_VIS:
+        r, c = int(rng.integers(0, wl.uvw.shape[0])), int(rng.integers(0, nchan))
+        f = wl.freq[c] / synth.C0
+        p, _ = ogrid.plane_of(wl.uvw[r, 2] * f, wl.w_max, wl.Nw)
+        S = int(st.support[p])
+        j0u, _ = ogrid.index_map(wl.uvw[r, 0] * f, N, wl.cell, S, wl.oversample)
+        j0v, _ = ogrid.index_map(wl.uvw[r, 1] * f, N, wl.cell, S, wl.oversample)
+        u, v = j0u + int(rng.integers(0, S)), j0v + int(rng.integers(0, S))
+        if 0 <= u < N and 0 <= v < N:
+            cu.append(u); cv.append(v)
+    cu += [int(x) for x in rng.integers(0, N, N_CELL_UNIFORM)]
+    cv += [int(x) for x in rng.integers(0, N, N_CELL_UNIFORM)]
+    return np.array(cu, dtype=np.int32), np.array(cv, dtype=np.int32)
 
 
 def grid_sums(g):
@@ -62,6 +90,11 @@ def check_full(ctx, wl, precs, label):
     st = oracle_stack(wl)
     fl, rstats = ogrid.flux(wl.uvw, wl.vis, wl.weight, wl.freq, st, threads=THREADS)
     assert rstats["n_gridded"] + rstats["n_skipped_oob"] + rstats["n_skipped_zero_weight"] == wl.nvis
+    cu, cv = sample_cells(wl, st, 2024)
+    cref, cl1 = ogrid.cells(wl.uvw, wl.vis, wl.weight, wl.freq, st, cu, cv, threads=THREADS)
+    cmax = float(np.max(np.abs(cref)))
+    assert np.count_nonzero(cref) >= N_CELL_VIS                            # the sample is not a set of empty cells
+    t_cu, t_cv = torch.from_numpy(cu.astype(np.int64)).cuda(), torch.from_numpy(cv.astype(np.int64)).cuda()
     d = (torch.from_numpy(wl.vis).cuda(), torch.from_numpy(wl.uvw).cuda(),
          torch.from_numpy(wl.weight).cuda(), torch.from_numpy(wl.freq).cuda())
     nrow, nchan, N = wl.uvw.shape[0], wl.freq.size, wl.grid_N
@@ -85,6 +118,13 @@ def check_full(ctx, wl, precs, label):
                       % (label, "f32" if prec == wpgrid.F32 else "f64", rep, e0, eu, ev, fl["l1"], s["n_updates"]))
                 assert max(e0, eu, ev) <= FLUX_TOL[prec], (label, prec, e0, eu, ev)
                 assert bool(torch.isfinite(torch.view_as_real(g)).all())
+                got = g[t_cv, t_cu].cpu().numpy().astype(np.complex128)
+                ec = float(np.max(np.abs(got - cref))) / cmax
+                el = float(np.max(np.abs(got - cref)[cl1 > 0] / cl1[cl1 > 0]))
+                print("%s prec %s rep %d: %d sampled cells, max err %.2e of the largest sampled |value| %.3e (%.2e of a cell's own L1)"
+                      % (label, "f32" if prec == wpgrid.F32 else "f64", rep, cu.size, ec, cmax, el))
+                assert ec <= CELL_TOL[prec], (label, prec, ec)
+                assert np.all(got[cl1 == 0] == 0)                          # a cell no window covers stays exactly zero
             out[prec] = (e0, eu, ev)
             del g, grid, ws, ks
     finally:

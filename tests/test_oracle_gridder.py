@@ -216,3 +216,54 @@ def test_flux_ragged_multichannel_flags_and_threads():
         assert abs(g.sum() - fl["sum"]) <= 1e-13 * fl["l1"]
         assert abs((g * ju[None, :]).sum() - fl["mom_u"]) <= 1e-13 * fl["l1"] * N
         assert abs((g * ju[:, None]).sum() - fl["mom_v"]) <= 1e-13 * fl["l1"] * N
+
+
+# ---------------------------------------------------------------- single cells, one by one (oracle_cells)
+def test_cells_match_python_gather_and_scatter_grid_on_config1(cfg1_small):
+    """oracle_cells (G5 read as a gather: what full-size GPU runs are checked against on sampled outputs) against
+    the gather written out here in Python from index_map / plane_of and the stack array, and against the
+    corresponding entries of the scatter-form oracle_grid — every cell of the grid."""
+    wl, st = cfg1_small
+    N = wl.grid_N
+    K = st.as_array()                                       # [p][ov][ou][iv][iu]
+    exp = np.zeros((N, N), dtype=np.complex128)
+    for k in range(wl.uvw.shape[0]):
+        j0u, ou = gridder.index_map(wl.uvw[k, 0], N, wl.cell, 7, 8)
+        j0v, ov = gridder.index_map(wl.uvw[k, 1], N, wl.cell, 7, 8)
+        p, _ = gridder.plane_of(wl.uvw[k, 2], wl.w_max, wl.Nw)
+        for cv in range(j0v, j0v + 7):
+            for cu in range(j0u, j0u + 7):
+                exp[cv, cu] += complex(wl.vis[k, 0]) * float(wl.weight[k, 0]) * K[p, ov, ou, cv - j0v, cu - j0u]
+    cv, cu = np.divmod(np.arange(N * N), N)
+    val, l1 = gridder.cells(wl.uvw, wl.vis, wl.weight, wl.freq, st, cu, cv)
+    val = val.reshape(N, N)
+    assert np.max(np.abs(val - exp)) <= 1e-13 * np.max(np.abs(exp))
+    g, _ = gridder.grid(wl.uvw, wl.vis, wl.weight, wl.freq, st)
+    assert np.max(np.abs(val - g)) <= 1e-13 * np.max(np.abs(g))
+    assert np.all(l1.reshape(N, N) >= np.abs(val) * (1 - 1e-12)) and np.count_nonzero(l1) == np.count_nonzero(np.abs(g) > 0)
+    # transposed cell coordinates (a plausible mistake) do not pass
+    valT, _ = gridder.cells(wl.uvw, wl.vis, wl.weight, wl.freq, st, cv, cu)
+    assert np.max(np.abs(valT.reshape(N, N) - g)) > 1e-3 * np.max(np.abs(g))
+
+
+def test_cells_ragged_multichannel_flags_and_threads():
+    """oracle_cells on a ragged stack with several channels, zero weights, clamped w and off-grid windows, on a
+    seeded sample of cells (border cells included): equals the gridded result there; threads change nothing."""
+    N, cell, Q, Nw, w_max = 128, 0.2 / 128, 4, 4, 400.0
+    sup = wkernel.ragged_support(Nw, w_max, N, cell, 8, 32)
+    st = wkernel.build_stack(Nw, w_max, sup, Q, N, cell)
+    rng = np.random.default_rng(12)
+    n, nchan = 500, 3
+    uvw = np.stack([rng.uniform(-330, 330, n), rng.uniform(-330, 330, n), rng.uniform(-450, 450, n)], 1)
+    freq = np.array([0.9, 1.0, 1.1]) * synth.C0
+    vis = (rng.standard_normal((n, nchan)) + 1j * rng.standard_normal((n, nchan))).astype(np.complex64)
+    wt = rng.uniform(0.0, 2.0, (n, nchan)).astype(np.float32)
+    wt[rng.uniform(size=wt.shape) < 0.1] = 0.0
+    g, stats = gridder.grid(uvw, vis, wt, freq, st)
+    assert stats["n_skipped_oob"] > 0 and stats["n_skipped_zero_weight"] > 0 and stats["n_clamped_w"] > 0
+    cu = np.concatenate([rng.integers(0, N, 300), [0, N - 1, 0, N - 1]])
+    cv = np.concatenate([rng.integers(0, N, 300), [0, 0, N - 1, N - 1]])
+    for threads in (1, 3):
+        val, l1 = gridder.cells(uvw, vis, wt, freq, st, cu, cv, threads=threads)
+        assert np.max(np.abs(val - g[cv, cu])) <= 1e-13 * np.max(np.abs(g))
+        assert np.count_nonzero(val) > 100
