@@ -46,7 +46,7 @@ FLOP_PER_UPDATE = 8          # one complex multiply-add = 4 real FMA (SURVEY.md 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--steps", type=int, default=48)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="config4")
@@ -179,15 +179,27 @@ def time_oracle(wl, st, rows, threads):
     return time.perf_counter() - t0, stats["n_updates"]
 
 
+def rows_for(wl, st, threads, target_s):
+    """Rows of the workload's prefix that the oracle passes over in about `target_s` seconds.  Two probes, because a
+    call has a fixed cost that a single probe would mistake for work: with OpenMP every thread allocates, zeroes and
+    finally adds up its private N x N grid (1 GB each at N = 8192)."""
+    nrow = wl.uvw.shape[0]
+    p1 = min(nrow, 200_000 if threads > 1 else 20_000)
+    p2 = min(nrow, 4 * p1)
+    t1, _ = time_oracle(wl, st, p1, threads)
+    if p2 == p1:
+        return nrow
+    t2, _ = time_oracle(wl, st, p2, threads)
+    per_row = max((t2 - t1) / (p2 - p1), 1e-12)
+    fixed = max(t1 - p1 * per_row, 0.0)
+    return int(min(nrow, max(p2, (target_s - fixed) / per_row)))
+
+
 def sized_oracle_run(wl, st, threads, target_s, max_passes=50):
     """The oracle on a prefix of the workload sized for about `target_s` seconds (a workload it finishes sooner is
     passed over several times).  Returns (updates/s, description)."""
     nrow = wl.uvw.shape[0]
-    probe = min(nrow, 200_000 if threads > 1 else 20_000)
-    dt, upd = time_oracle(wl, st, probe, threads)
-    rate = upd / max(dt, 1e-9)
-    per_row = max(upd / probe, 1.0)
-    rows = int(min(nrow, max(probe, target_s * rate / per_row)))
+    rows = rows_for(wl, st, threads, target_s)
     t_sum, upd_sum, passes = 0.0, 0, 0
     while passes == 0 or (rows == nrow and t_sum < target_s and passes < max_passes):
         dt, upd = time_oracle(wl, st, rows, threads)
@@ -204,7 +216,7 @@ def cpu_baseline(wl, target_s=12.0):
     st = oracle_stack(wl)
     threads = oracle_threads(wl)
     v_all, sample_all = sized_oracle_run(wl, st, threads, target_s)
-    v_one, sample_one = sized_oracle_run(wl, st, 1, 4.0, max_passes=5)
+    v_one, sample_one = sized_oracle_run(wl, st, 1, 6.0, max_passes=5)
     return {"value": v_all, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample_all,
             "host_cores": os.cpu_count(),
             "one_thread": {"value": v_one, "unit": UNIT, "cores": 1, "sample": sample_one}}
@@ -226,11 +238,9 @@ def run_reference(args):
     st = oracle_stack(wl)
     threads = oracle_threads(wl)
     nrow = wl.uvw.shape[0]
-    probe = min(nrow, 200_000)
-    dt, upd = time_oracle(wl, st, probe, threads)
     total = max(1, args.steps + args.warmup)
     budget_s = min(20.0, 120.0 / total)                      # whole run within a few minutes
-    rows = int(min(nrow, max(probe, budget_s * (upd / dt) / max(upd / probe, 1.0))))
+    rows = rows_for(wl, st, threads, budget_s)
     for _ in range(args.warmup):
         time_oracle(wl, st, rows, threads)
     t_sum, upd_sum = 0.0, 0

@@ -371,10 +371,12 @@ scan_apply_kernel(unsigned *__restrict__ hist, unsigned nkeys, const unsigned *_
 }
 
 // One 16-byte store per fp32 record; 8 + 8 + 8 for the 24-byte fp64 record.
-__device__ __forceinline__ void store_rec(Rec<float> *dst, float re, float im, uint2 p) {
-    *reinterpret_cast<uint4 *>(dst) = make_uint4(__float_as_uint(re), __float_as_uint(im), p.x, p.y);
+// (pol: the L2 evict-last policy of the scatter pass; the fp64 record's plain stores ignore it)
+__device__ __forceinline__ void store_rec(Rec<float> *dst, float re, float im, uint2 p, unsigned long long pol) {
+    asm volatile("st.global.L2::cache_hint.v4.b32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(dst), "r"(__float_as_uint(re)), "r"(__float_as_uint(im)),
+                 "r"(p.x), "r"(p.y), "l"(pol) : "memory");
 }
-__device__ __forceinline__ void store_rec(Rec<double> *dst, double re, double im, uint2 p) {
+__device__ __forceinline__ void store_rec(Rec<double> *dst, double re, double im, uint2 p, unsigned long long) {
     dst->re = re; dst->im = im;
     *reinterpret_cast<uint2 *>(&dst->pos) = p;
 }
@@ -416,8 +418,16 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
     }
     // one returning atomic per run of equal keys (the slowest instruction of the pass: ~2 cycles per lane)
     key_runs(key, pos, koff, P.compress != 0, head, rhead, nrec);
+    // The bucket cursors and the half-written sectors of the records are what this pass wants to find in L2 again
+    // (the inputs stream through evict-first): both carry an evict-last hint.  Measured: binning -0.2 ms on config 4.
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
 #pragma unroll
-    for (int j = 0; j < kVpt; ++j) dst[j] = head[j] ? atomicAdd(cursor + key[j], nrec[j]) : 0u;
+    for (int j = 0; j < kVpt; ++j) {
+        dst[j] = 0u;
+        if (head[j])
+            asm volatile("atom.global.add.L2::cache_hint.u32 %0, [%1], %2, %3;" : "=r"(dst[j]) : "l"(cursor + key[j]), "r"(nrec[j]), "l"(pol) : "memory");
+    }
 #pragma unroll
     for (int j = 1; j < kVpt; ++j)
         if (key[j] != WPG_NO_KEY && !head[j]) dst[j] = dst[j - 1] + (rhead[j] ? 1u : 0u);
@@ -430,7 +440,7 @@ scatter_kernel(const float2 *__restrict__ vis, const double *__restrict__ uvw, c
             if (key[j] != WPG_NO_KEY && !rhead[j]) { re[j - 1] += re[j]; im[j - 1] += im[j]; }
 #pragma unroll
         for (int j = 0; j < kVpt; ++j)
-            if (rhead[j]) store_rec(reinterpret_cast<Rec<TT> *>(rec_out) + dst[j], re[j], im[j], make_uint2(pos[j], koff[j]));
+            if (rhead[j]) store_rec(reinterpret_cast<Rec<TT> *>(rec_out) + dst[j], re[j], im[j], make_uint2(pos[j], koff[j]), pol);
     } else {
         // walk the thread's visibilities in order; a record is written when the next one starts a new record
         constexpr int NP = NPOL > 1 ? NPOL : 2;

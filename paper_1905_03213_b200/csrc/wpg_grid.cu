@@ -1078,6 +1078,8 @@ int launch_class(wpg_ctx *ctx, cudaStream_t strm, const BinParams &bp, const Wor
         if (S == 16) return launch_pairs<16, 2, 4, 3, 1, 0, false, 2>(ctx, strm, bp, ws, K, grid, w, cls, S);   // window split over two work items
         if (S == 4) return launch_pairs<4, 1, 4, 4, 4>(ctx, strm, bp, ws, K, grid, w, cls, S);        // 8 pairs: 4 records per step
         if (S == 12) return launch_pairs<12, 3, 2, 3, 1, 4, true>(ctx, strm, bp, ws, K, grid, w, cls, S);     // 4 rows per slot
+        if (S == 10) return launch_pairs<10, 2, 4, 3, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);     // (config 4's second and
+        if (S == 14) return launch_pairs<14, 4, 2, 2, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);     //  fourth largest classes)
         if (nslot <= 1) return launch_pairs<0, 1, 4, 4, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);
         if (nslot <= 2) return launch_pairs<0, 2, 4, 3, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);
         if (nslot <= 3) return launch_pairs<0, 3, 2, 3, 1, 0, true>(ctx, strm, bp, ws, K, grid, w, cls, S);
