@@ -134,6 +134,26 @@ int  wpg_grid(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float 
               const double *d_freq, int64_t nrow, int nchan, const void *d_kernels,
               const wpg_kdesc *desc, wpg_prec prec, void *d_grid,
               void *d_workspace, size_t workspace_bytes, wpg_stats *h_stats_or_null);
+/* wpg_grid without a workspace argument and without any device allocation (csrc/wpg_static.cu), for callers that
+ * cannot call cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid it.  The scratch
+ * (counters, bucket table, sorted records) is a file-scope device array of WPG_STATIC_SCRATCH_BYTES that every GPU
+ * holding this library's module keeps until the process exits; its device address is looked up once per device
+ * (cudaGetSymbolAddress, with the context's device current) on the first call.
+ *   Arguments, layouts, result and h_stats_or_null exactly as wpg_grid; d_grid is ACCUMULATED INTO.
+ *   Limit: wpg_grid_workspace_bytes(ctx, nrow, nchan, desc, prec) <= wpg_static_scratch_bytes() = 64 MiB — fp32:
+ *   3.1e6 visibilities per call at N = 2048, 3.9e6 at N = 1024 or 8192 (fp64: two thirds of that); N = 4096 and
+ *   ragged stacks need option "key_bits" <= 23 (their default 2^24-entry bucket table alone is 64 MiB).  Larger problems return
+ *   WPG_ENOMEM with the two sizes in wpg_last_error and launch nothing (split the rows over several calls —
+ *   gridding is additive — or use wpg_grid with a workspace of your own).
+ *   Calls no cudaMalloc / cudaFree / allocating library routine (a ragged stack's first call on a context creates
+ *   its three side streams, which hold no device memory).  Does not synchronise unless h_stats is given.
+ *   The array is shared by every call on the device and keeps the last call's contents; the call clears what must
+ *   start at zero on the context's stream.  Calls that overlap on the GPU (several contexts or streams) race. */
+#define WPG_STATIC_SCRATCH_BYTES ((size_t)64 << 20)
+size_t wpg_static_scratch_bytes(void);
+int  wpg_grid_static(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,
+                     const double *d_freq, int64_t nrow, int nchan, const void *d_kernels,
+                     const wpg_kdesc *desc, wpg_prec prec, void *d_grid, wpg_stats *h_stats_or_null);
 /* Same result by the naive design: one global atomic per update, no sorting (the measured
  * "atomic roofline" the tiled gridder must beat; "write access ... in an atomic manner"). */
 int  wpg_grid_naive(wpg_ctx *ctx, const void *d_vis, const double *d_uvw, const float *d_weight,

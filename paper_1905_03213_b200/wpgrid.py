@@ -23,6 +23,7 @@ EXPORTS = (
     "wpg_dirty_image", "wpg_launch_count", "wpg_phase_ms", "wpg_microbench",
     "wpg_baseline_workspace_bytes", "wpg_baseline_reorder", "wpg_grid_baseline_order",
     "wpg_degrid_workspace_bytes", "wpg_degrid", "wpg_grid_pol_workspace_bytes", "wpg_grid_pol", "wpg_shard_rows",
+    "wpg_static_scratch_bytes", "wpg_grid_static",
 )
 
 
@@ -83,6 +84,9 @@ def load():
     lib.wpg_grid_workspace_bytes.argtypes = [vp, i64, cint, kd, cint]; lib.wpg_grid_workspace_bytes.restype = sz
     lib.wpg_grid.argtypes = [vp, vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, vp, sz, stp]
     lib.wpg_grid.restype = cint
+    lib.wpg_static_scratch_bytes.argtypes = []; lib.wpg_static_scratch_bytes.restype = sz
+    lib.wpg_grid_static.argtypes = [vp, vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, stp]
+    lib.wpg_grid_static.restype = cint
     lib.wpg_grid_naive.argtypes = [vp, vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, stp]
     lib.wpg_grid_naive.restype = cint
     lib.wpg_grid_host.argtypes = [vp, vp, vp, vp, vp, i64, cint, vp, kd, cint, vp, stp, vp, dbl]
@@ -286,6 +290,21 @@ class Context:
                                       grid.data_ptr(), workspace.data_ptr(), workspace.numel(),
                                       ctypes.byref(st) if stats else None))
         return grid, (st.as_dict() if stats else None)
+
+    def grid_static(self, vis, uvw, weight, freq, stack, grid, stats=False):
+        """grid += gridding(vis) through wpg_grid_static: no workspace argument and no device allocation — the scratch
+        is the library's static device array (static_scratch_bytes(); larger problems raise WpgError ENOMEM).  The
+        caller supplies the grid.  Calls on one device share the array: do not overlap them on the GPU."""
+        nrow, nchan = self._inputs(vis, uvw, weight, freq)
+        self._check_grid(grid, stack)
+        st = Stats()
+        self._check(self.lib.wpg_grid_static(self.h, vis.data_ptr(), uvw.data_ptr(), weight.data_ptr(), freq.data_ptr(),
+                                             nrow, nchan, stack.data.data_ptr(), ctypes.byref(stack.desc), stack.prec,
+                                             grid.data_ptr(), ctypes.byref(st) if stats else None))
+        return grid, (st.as_dict() if stats else None)
+
+    def static_scratch_bytes(self):
+        return int(self.lib.wpg_static_scratch_bytes())
 
     def grid_naive(self, vis, uvw, weight, freq, stack, grid=None, stats=False):
         nrow, nchan = self._inputs(vis, uvw, weight, freq)
