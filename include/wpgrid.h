@@ -256,7 +256,9 @@ int  wpg_shard_rows(int64_t nrow, int64_t row_block, int world, int rank, int64_
  *            in shared memory;
  *        7 / 8 = the inner loop of a shared-memory subgrid accumulator (64 x 64-cell tile + halo per CTA, S = 8, one
  *            L1-resident coefficient slice per record): 7 with red.shared.add.f32, 8 with plain load / add / store
- *            (the ceiling of a warp-owned tile); h_out[0] = grid updates/s.  2, 7, 8 need buf_bytes >= 16 MiB.
+ *            (the ceiling of a warp-owned tile); h_out[0] = grid updates/s;
+ *        9 = 16-byte loads of whole 512-byte slices at pseudo-random places of an L2-resident, L1-missing 32 MiB
+ *            region (the coefficient feed when the slices do not stay in L1).  2, 7, 8, 9 need buf_bytes >= 16 MiB.
  * d_buf: device scratch, buf_bytes >= 1 MiB (the reductions use the largest power-of-two number of 8-byte cells
  * that fits; its contents are overwritten).  h_out[0] = operations/s, h_out[1] = kernel ms.  Synchronises. */
 int  wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_bytes, double *h_out /*[2]*/);

@@ -140,20 +140,43 @@ micro_subgrid_kernel(const float4 *src, float2 *sink, int iters, int atomic) {
     if (acc.x == 123.456f) sink[0] = acc;
 }
 
+// which = 9: the same 16-byte loads as which = 2, but every trip a warp reads a 512-byte slice (32 lanes x 16 B, four
+// whole 128-byte lines) at a pseudo-random place of a buffer that fits the L2 and not the L1 (32 MiB), 8 loads in
+// flight: the coefficient feed when the slices do NOT stay in L1 — what the gridder sees, ncu: 8 % L1 hit rate at
+// S = 12 (a 2.4 MB stack streamed through a 200 KB cache), each missing line costing a second data-pipe wavefront.
+__global__ void __launch_bounds__(256)
+micro_l2_kernel(const float4 *src, float *sink, int iters, unsigned slice_mask) {
+    const unsigned gwarp = (blockIdx.x * 256u + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
+    unsigned x = gwarp * 2654435761u + 12345u;
+    float acc = 0.f;
+    for (int i = 0; i < iters; ++i) {
+        float4 v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            x = x * 1664525u + 1013904223u;
+            const float4 *p = src + (size_t)((x >> 8) & slice_mask) * 32u + lane;
+            asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v[k].x), "=f"(v[k].y), "=f"(v[k].z), "=f"(v[k].w) : "l"(p));
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc += v[k].x + v[k].w;
+    }
+    if (acc == 123.456f) sink[0] = acc;
+}
+
 }  // namespace
 
 // h_out[0] = operations per second (reductions of one cell, 16-byte loads, packed FMAs = 2 FMA, FMAs, grid updates),
 // h_out[1] = kernel milliseconds.  d_buf: device scratch of at least buf_bytes >= 1 MiB (power of two used).
 extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, size_t buf_bytes, double *h_out) {
     if (!ctx || !h_out || !d_buf) return WPG_EINVAL;
-    if (which < 0 || which > 8 || iters < 1 || buf_bytes < ((size_t)1 << 20))
-        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which 0..8, iters >= 1, buffer >= 1 MiB");
+    if (which < 0 || which > 9 || iters < 1 || buf_bytes < ((size_t)1 << 20))
+        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which 0..9, iters >= 1, buffer >= 1 MiB");
     WPG_DEVICE(ctx);
     size_t ncell = 1;
     while (ncell * 2 * sizeof(float2) <= buf_bytes) ncell *= 2;
     if ((which == 2 || which >= 7) && buf_bytes < ((size_t)16 << 20))
-        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which = 2, 7, 8 need a 16 MiB buffer");
-    const int blocks = ctx->sm_count * (which == 2 ? 2 : which >= 7 ? 4 : 8);
+        return wpg_fail(ctx, WPG_EINVAL, "wpg_microbench: which = 2, 7, 8, 9 need a 16 MiB buffer");
+    const int blocks = ctx->sm_count * (which == 2 ? 2 : which == 9 ? 6 : which >= 7 ? 4 : 8);
     constexpr int kSubgridBytes = 71 * 72 * (int)sizeof(float2);
     if (which >= 7) WPG_CUDA(ctx, cudaFuncSetAttribute(micro_subgrid_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSubgridBytes));
     cudaEvent_t e0, e1;
@@ -165,6 +188,11 @@ extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, s
         if (which <= 1) micro_red_kernel<<<blocks, 256, 0, s>>>((float2 *)d_buf, (unsigned)(ncell - 1), iters, which);
         else if (which == 2) micro_l1_kernel<<<blocks, 256, 0, s>>>((const float4 *)d_buf, (float *)d_buf, iters);
         else if (which == 3) micro_ffma2_kernel<<<blocks, 256, 0, s>>>((float *)d_buf, iters, 1.0f);
+        else if (which == 9) {                       // slices of 512 bytes in the largest power of two <= min(buffer, 32 MiB)
+            size_t nsl = 1;
+            while (nsl * 2 * 512 <= buf_bytes && nsl * 2 * 512 <= ((size_t)32 << 20)) nsl *= 2;
+            micro_l2_kernel<<<blocks, 256, 0, s>>>((const float4 *)d_buf, (float *)d_buf, iters, (unsigned)(nsl - 1));
+        }
         else if (which >= 7) micro_subgrid_kernel<<<blocks, 256, kSubgridBytes, s>>>((const float4 *)d_buf, (float2 *)d_buf, iters, which == 7);
         else if (which >= 5) micro_bulkred_kernel<<<blocks, 256, 0, s>>>((float2 *)d_buf, (unsigned)(ncell - 1), iters, which == 5 ? 32 : 8);
         else micro_dfma_kernel<<<blocks, 256, 0, s>>>((double *)d_buf, iters, 1.0);
@@ -178,7 +206,8 @@ extern "C" int wpg_microbench(wpg_ctx *ctx, int which, int iters, void *d_buf, s
     WPG_CUDA(ctx, cudaGetLastError());
     const double threads = (double)blocks * 256.0;
     // reductions of one cell (0, 1: one per lane; 5, 6: 32 or 8 per warp), else 8 operations per thread and trip
-    const double ops = which >= 7 ? threads / 32.0 * (double)iters * 64.0           // 7, 8: grid updates (64 per record)
+    const double ops = which == 9 ? threads * (double)iters * 8.0                   // 9: 16-byte loads
+                     : which >= 7 ? threads / 32.0 * (double)iters * 64.0           // 7, 8: grid updates (64 per record)
                      : which >= 5 ? threads / 32.0 * (double)iters * (which == 5 ? 32.0 : 8.0)
                                   : threads * (double)iters * (which == 0 || which == 1 ? 1.0 : 8.0);
     h_out[0] = ops / (ms * 1e-3);
