@@ -291,6 +291,13 @@ def measured_peaks(ctx, f32):
     return alu_tflops, l1_loads_per_s * 16 / 1e9, hbm_gbs, hbm_src
 
 
+def l2_feed_gbs(ctx):
+    """GB/s of 16-byte loads of whole 512-byte slices from an L2-resident region that does not stay in L1
+    (wpg_microbench 9): the coefficient feed when the slices miss L1, bounded by the L2 -> L1 fill path."""
+    loads_per_s, _ = ctx.microbench(9, 2000)
+    return loads_per_s * 16 / 1e9
+
+
 def traffic_from_profiles(workload, prec):
     """dram bytes per gridder launch from the committed ncu --set full capture, if there is one."""
     path = os.path.join(ROOT, "profiles", "gridder_traffic.json")
@@ -455,6 +462,14 @@ def run_b200(args):
                         "frac": upd_per_s * FLOP_PER_UPDATE / 1e12 / alu_tflops, "peak_source": "measured in this run"},
                 "l1": {"achieved": upd_per_s * coef_bytes / 1e9, "peak": l1_gbs, "unit": "GB/s",
                        "frac": upd_per_s * coef_bytes / 1e9 / l1_gbs, "peak_source": "measured in this run"}}
+    # beside it: the same feed when the slices do NOT stay in L1 (ncu finds 61-98 % of the gridder's
+    # coefficient sectors missing L1 — the stack is 1-30 MB — and then the L2 -> L1 fill path, 64 B/clk/SM, is the limit)
+    l2_gbs = l2_feed_gbs(ctx)
+    roofline["l2_feed"] = {"achieved": upd_per_s * coef_bytes / 1e9, "peak": l2_gbs, "unit": "GB/s",
+                           "frac": upd_per_s * coef_bytes / 1e9 / l2_gbs,
+                           "peak_source": "measured in this run (wpg_microbench 9: LDG.128 of 512-byte slices, L2-resident, L1-missing)",
+                           "note": "achieved counts %d B per update; merged records (compression) and L1 hits load less, "
+                                   "so this fraction can exceed 1" % coef_bytes}
     # second entry: the binning pass (a1), HBM-bound.  Algorithmic bytes per visibility: the raw
     # inputs read once (24 / nchan + 12), the sorted record written (16 | 24), 8 B of key / offset traffic.
     bin_bytes_per_vis = 24.0 / nchan + 12 + rec_bytes + 8
