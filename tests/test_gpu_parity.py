@@ -577,3 +577,19 @@ def test_sharded_gridding_one_rank_nccl(ctx):
     finally:
         dist.destroy_process_group()
         ctx.set_option("row_block", 0)
+
+
+def test_microbenchmarks_run_and_order_sensibly(ctx):
+    """wpg_microbench (the machine limits bench.py reads its rooflines against): every pattern runs, rejects a bad
+    selector, and the measured rates keep the order the hardware fixes — L1-resident loads beat L1-missing ones,
+    packed fp32 FMAs beat fp64 FMAs, row-segment reductions beat scattered ones."""
+    r = {w: ctx.microbench(w, 200, 32 << 20)[0] for w in range(10)}
+    assert all(v > 0 for v in r.values())
+    assert r[2] > 1.3 * r[9]                   # L1-resident vs L2-resident, L1-missing 16-byte loads
+    assert r[3] * 2 > r[4]                     # f32x2 (two FMAs each) vs f64 FMAs
+    assert r[0] > r[1]                         # a warp per row segment vs every lane its own cell
+    assert r[8] > r[7]                         # plain tile updates vs shared-memory atomics
+    with pytest.raises(wpgrid.WpgError):
+        ctx.microbench(10, 10)
+    with pytest.raises(wpgrid.WpgError):
+        ctx.microbench(2, 10, 1 << 20)         # needs a 16 MiB buffer
